@@ -1,0 +1,533 @@
+/* dgrhd_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see dgrhd_oracle.h).
+ *
+ * Plain fp64 CPU oracle for one SSP-RK stage of the DG-RHD method of arxiv 2205.00095.
+ * Every function cites the PAPER.md passage it restates.  Build: gcc -O2 -ffp-contract=off
+ * (no fast-math, no FMA contraction) [-fopenmp: outer loops over elements / states only, which
+ * does not change any arithmetic or summation order].
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): every function below is pinned; see DESIGN.md
+ * "Oracle pins".  No function here is "parity unpinned".
+ */
+#include "dgrhd_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O4  Basis: Gauss-Lobatto-Legendre nodes/weights, N = p+1 (reading R1; PAPER.md:110-119 gives a
+ * nodal Lagrange basis, Eq. 13-14, without naming the node family).  D[q*N+i] = l_i'(x_q).
+ * ------------------------------------------------------------------------------------------ */
+void orc_gll(int N, double *x, double *w, double *D) {
+  switch (N) {
+    case 1: x[0] = 0.0; w[0] = 2.0; break;
+    case 2: x[0] = -1.0; x[1] = 1.0; w[0] = 1.0; w[1] = 1.0; break;
+    case 3: x[0] = -1.0; x[1] = 0.0; x[2] = 1.0;
+            w[0] = 1.0 / 3.0; w[1] = 4.0 / 3.0; w[2] = 1.0 / 3.0; break;
+    case 4: x[0] = -1.0; x[1] = -sqrt(1.0 / 5.0); x[2] = sqrt(1.0 / 5.0); x[3] = 1.0;
+            w[0] = 1.0 / 6.0; w[1] = 5.0 / 6.0; w[2] = 5.0 / 6.0; w[3] = 1.0 / 6.0; break;
+    case 5: x[0] = -1.0; x[1] = -sqrt(3.0 / 7.0); x[2] = 0.0; x[3] = sqrt(3.0 / 7.0); x[4] = 1.0;
+            w[0] = 1.0 / 10.0; w[1] = 49.0 / 90.0; w[2] = 32.0 / 45.0; w[3] = 49.0 / 90.0;
+            w[4] = 1.0 / 10.0; break;
+    default: return;
+  }
+  /* l_i'(x_q) = sum_{m!=i} 1/(x_i-x_m) prod_{k!=i,m} (x_q-x_k)/(x_i-x_k)   (Lagrange, Eq. 14) */
+  for (int q = 0; q < N; ++q)
+    for (int i = 0; i < N; ++i) {
+      double s = 0.0;
+      for (int m = 0; m < N; ++m) {
+        if (m == i) continue;
+        double t = 1.0 / (x[i] - x[m]);
+        for (int k = 0; k < N; ++k) {
+          if (k == i || k == m) continue;
+          t *= (x[q] - x[k]) / (x[i] - x[k]);
+        }
+        s += t;
+      }
+      D[q * N + i] = s;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O1  EOS, prim->con, flux, wave speeds  (PAPER.md:45-56 Eq. 2-4, :79-93 Eq. 8-11, :163-167)
+ * ------------------------------------------------------------------------------------------ */
+/* Eq. 8 (ideal) / Eq. 10 (Taub-Matthews), Theta = P/rho, c = 1 */
+double orc_enthalpy(int eos, double G, double rho, double P) {
+  double Th = P / rho;
+  if (eos == ORC_EOS_IDEAL) return 1.0 + G / (G - 1.0) * Th;
+  return 2.5 * Th + 1.5 * sqrt(Th * Th + 4.0 / 9.0);
+}
+
+/* Eq. 9 (ideal) / Eq. 11 (Taub-Matthews) */
+double orc_cs2(int eos, double G, double rho, double P) {
+  double Th = P / rho;
+  if (eos == ORC_EOS_IDEAL) return G * Th / orc_enthalpy(eos, G, rho, P);
+  double r = sqrt(Th * Th + 4.0 / 9.0);
+  return (3.0 * Th * Th + 5.0 * Th * r) / (12.0 * Th * Th + 2.0 + 12.0 * Th * r);
+}
+
+/* Eq. 4 with W = [rho, u, P], u = gamma v, gamma = sqrt(1+|u|^2) */
+void orc_prim2con(int eos, double G, const double W[5], double U[5]) {
+  double rho = W[0], P = W[4];
+  double u2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  double g = sqrt(1.0 + u2);
+  double h = orc_enthalpy(eos, G, rho, P);
+  U[0] = g * rho;                 /* D = gamma rho          */
+  U[1] = g * rho * h * W[1];      /* M = gamma rho h u      */
+  U[2] = g * rho * h * W[2];
+  U[3] = g * rho * h * W[3];
+  U[4] = g * g * rho * h - P;     /* E = gamma^2 rho h - P  */
+}
+
+/* Eq. 2 in direction dir:  [rho u_d, rho h u u_d + P e_d, gamma rho h u_d]
+ *   = [D v_d, M v_d + P e_d, (E+P) v_d]  with v = u/gamma */
+void orc_flux(int eos, double G, const double W[5], int dir, double F[5]) {
+  double U[5];
+  orc_prim2con(eos, G, W, U);
+  double u2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  double g = sqrt(1.0 + u2);
+  double vd = W[1 + dir] / g;
+  F[0] = U[0] * vd;
+  F[1] = U[1] * vd;
+  F[2] = U[2] * vd;
+  F[3] = U[3] * vd;
+  F[1 + dir] += W[4];
+  F[4] = (U[4] + W[4]) * vd;
+}
+
+/* Eq. 21-22, "v_x" = velocity component normal to the face */
+void orc_wavespeeds(int eos, double G, const double W[5], int dir, double *lm, double *lp) {
+  double u2 = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  double g2 = 1.0 + u2;
+  double vd = W[1 + dir] / sqrt(g2);
+  double cs2 = orc_cs2(eos, G, W[0], W[4]);
+  double sig = cs2 / (g2 * (1.0 - cs2));                       /* Eq. 22 */
+  double root = sqrt(sig * (1.0 - vd * vd + sig));
+  *lm = (vd - root) / (1.0 + sig);                             /* Eq. 21 */
+  *lp = (vd + root) / (1.0 + sig);
+}
+
+/* HLL two-wave flux (PAPER.md:161 cites Schneider et al.; formula not printed: reading R9),
+ * lambda_L, lambda_R by Eq. 23-24; U_{L,R} recomputed from W_{L,R} by Eq. 4 (reading R8). */
+void orc_hll(int eos, double G, const double WL[5], const double WR[5], int dir, double F[5]) {
+  double lmL, lpL, lmR, lpR;
+  orc_wavespeeds(eos, G, WL, dir, &lmL, &lpL);
+  orc_wavespeeds(eos, G, WR, dir, &lmR, &lpR);
+  double lL = fmin(lmL, lmR);                                   /* Eq. 23 */
+  double lR = fmax(lpL, lpR);                                   /* Eq. 24 */
+  double FL[5], FR[5], UL[5], UR[5];
+  orc_flux(eos, G, WL, dir, FL);
+  orc_flux(eos, G, WR, dir, FR);
+  if (lL >= 0.0) { for (int v = 0; v < 5; ++v) F[v] = FL[v]; return; }
+  if (lR <= 0.0) { for (int v = 0; v < 5; ++v) F[v] = FR[v]; return; }
+  orc_prim2con(eos, G, WL, UL);
+  orc_prim2con(eos, G, WR, UR);
+  for (int v = 0; v < 5; ++v)
+    F[v] = (lR * FL[v] - lL * FR[v] + lL * lR * (UR[v] - UL[v])) / (lR - lL);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7 predicate: Eq. 25 with the PLUS sign under the root (reading R13a; Eq. 27/31/32), the
+ * safety factor (1-eps) on E (R13c), separately rounded operations in this order (R13e).
+ * NaN anywhere => not admissible.
+ * ------------------------------------------------------------------------------------------ */
+int orc_admissible(const double U[5], double eps) {
+  double D = U[0];
+  double m2 = D * D;
+  m2 = m2 + U[1] * U[1];
+  m2 = m2 + U[2] * U[2];
+  m2 = m2 + U[3] * U[3];
+  double Es = (1.0 - eps) * U[4];
+  return (D > 0.0) && (Es > sqrt(m2));
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O2  con2prim, ideal EOS: Newton on the quartic of Eq. 59 in w, beta = 2w/(1+w^2) (Eq. 58,
+ * reading R5), finishing by Eq. 55-57.  PAPER.md:262-263 (Eq. 38), :329-345.
+ * ------------------------------------------------------------------------------------------ */
+static void ideal_coeffs(double al, double xi, double eta, double c[5]) {
+  c[4] = (al - 1.0) * xi;            /* Eq. 59, w^4 */
+  c[3] = -2.0 * (al * eta + 1.0);    /* w^3 */
+  c[2] = 2.0 * (al + 1.0) * xi;      /* w^2 */
+  c[1] = -2.0 * (al * eta - 1.0);    /* w^1 */
+  c[0] = (al - 1.0) * xi;            /* w^0 */
+}
+
+static void ideal_finish(double G, const double U[5], double Mabs, double w, double W[5]) {
+  double D = U[0], E = U[4];
+  double w2 = w * w;
+  double beta = 2.0 * w / (1.0 + w2);                 /* Eq. 58 */
+  double ig = (1.0 - w2) / (1.0 + w2);                /* 1/gamma = sqrt(1-beta^2), exact identity */
+  double rho = D * ig;                                /* Eq. 55 */
+  double nx = 0.0, ny = 0.0, nz = 0.0;
+  if (Mabs > 0.0) { nx = U[1] / Mabs; ny = U[2] / Mabs; nz = U[3] / Mabs; }
+  double ug = 2.0 * w / (1.0 - w2);                   /* gamma*beta */
+  W[0] = rho;
+  W[1] = ug * nx;                                     /* u = gamma v, v = beta M/|M|  (Eq. 56) */
+  W[2] = ug * ny;
+  W[3] = ug * nz;
+  W[4] = (G - 1.0) * (E - beta * Mabs - rho);         /* Eq. 57, M.v = beta |M| */
+}
+
+static int finite5(const double W[5]) {
+  for (int v = 0; v < 5; ++v) if (!isfinite(W[v])) return 0;
+  return 1;
+}
+
+static int con2prim_ideal(double G, const double U[5], double W[5], int *niter_out, int fixed_iter) {
+  double D = U[0], E = U[4];
+  double Mabs = sqrt(U[1] * U[1] + U[2] * U[2] + U[3] * U[3]);
+  double xi = Mabs / D, eta = E / D;                  /* Eq. 38 */
+  double al = G / (G - 1.0);
+  double w;
+  int it = 0;
+  if (xi == 0.0) {
+    w = 0.0;
+  } else if (xi < 1e-4 && fixed_iter < 0) {
+    /* Eq. 60, small-xi cubic series (reading R4) */
+    double a1 = al * eta - 1.0;
+    double a14 = a1 * a1 * a1 * a1;
+    w = (al - 1.0) / (2.0 * a1) * xi +
+        (al - 1.0) * (al - 1.0) / (8.0 * a14) * ((al + 3.0) * (al * eta + 1.0) - 4.0 * (al + 1.0)) *
+            xi * xi * xi;
+  } else {
+    double c[5];
+    ideal_coeffs(al, xi, eta, c);
+    double b0 = xi / eta;                             /* reading R2: beta_0 = |M|/E >= beta */
+    w = b0 / (1.0 + sqrt(1.0 - b0 * b0));
+    int maxit = fixed_iter >= 0 ? fixed_iter : 16;    /* reading R3 */
+    for (it = 0; it < maxit;) {
+      double p = (((c[4] * w + c[3]) * w + c[2]) * w + c[1]) * w + c[0];
+      double dp = ((4.0 * c[4] * w + 3.0 * c[3]) * w + 2.0 * c[2]) * w + c[1];
+      double dw = p / dp;
+      w = w - dw;
+      ++it;
+      if (fixed_iter < 0 && fabs(dw) <= 1e-14 * w) break;
+    }
+  }
+  if (niter_out) *niter_out = it;
+  ideal_finish(G, U, Mabs, w, W);
+  if (!(w >= 0.0 && w < 1.0) || !finite5(W) || !(W[4] > 0.0)) return 2;
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O3  con2prim, Taub-Matthews: analytic cubic in W = gamma^2 - 1, Eq. 61-73, finishing by
+ * Eq. 74-75, safeguards of reading R7.
+ * ------------------------------------------------------------------------------------------ */
+static int con2prim_tm(const double U[5], double Wp[5]) {
+  double D = U[0], E = U[4];
+  double Mabs = sqrt(U[1] * U[1] + U[2] * U[2] + U[3] * U[3]);
+  double xi = Mabs / D, eta = E / D;                  /* Eq. 38 */
+  double x2 = xi * xi, e2 = eta * eta;
+  double dif = (eta - xi) * (eta + xi);               /* eta^2 - xi^2 (R7) */
+  double den = dif * dif;
+  double sum = e2 + x2;
+  double br = 4.0 * sum - (x2 + 1.0);
+  double c1 = (sum * br - 14.0 * x2 * e2) / (2.0 * den);      /* Eq. 62 */
+  double c2 = (br * br - 57.0 * x2 * e2) / (16.0 * den);      /* Eq. 63 */
+  double c3 = -9.0 * x2 * e2 / (16.0 * den);                  /* Eq. 64 */
+  double Q = (3.0 * c2 - c1 * c1) / 9.0;                      /* Eq. 66 */
+  double R = (9.0 * c1 * c2 - 27.0 * c3 - 2.0 * c1 * c1 * c1) / 54.0;   /* Eq. 67 */
+  double d = Q * Q * Q + R * R;                               /* Eq. 65 */
+  double Wv;
+  if (d < 0.0) {
+    double arg = R / sqrt(-(Q * Q * Q));
+    if (arg > 1.0) arg = 1.0;
+    if (arg < -1.0) arg = -1.0;
+    double iota = acos(arg);                                  /* Eq. 70 */
+    Wv = 2.0 * sqrt(-Q) * cos(iota / 3.0) - c1 / 3.0;         /* Eq. 69 */
+  } else {
+    double sd = sqrt(d);
+    Wv = -c1 / 3.0 + cbrt(R + sd) + cbrt(R - sd);             /* Eq. 71-73, real cube roots */
+  }
+  if (Wv < 0.0) Wv = 0.0;                                     /* R7 */
+  double g = sqrt(Wv + 1.0);                                  /* Eq. 74 */
+  double beta = sqrt(Wv / (Wv + 1.0));
+  double rho = D / g;
+  double nx = 0.0, ny = 0.0, nz = 0.0;
+  if (Mabs > 0.0) { nx = U[1] / Mabs; ny = U[2] / Mabs; nz = U[3] / Mabs; }
+  double ug = sqrt(Wv);                                       /* gamma beta */
+  double X = E - beta * Mabs;                                 /* E - M.v */
+  Wp[0] = rho;
+  Wp[1] = ug * nx;
+  Wp[2] = ug * ny;
+  Wp[3] = ug * nz;
+  Wp[4] = (X - rho) * (X + rho) / (3.0 * X);                  /* Eq. 75 */
+  if (!finite5(Wp) || !(Wp[4] > 0.0)) return 2;
+  return 0;
+}
+
+int orc_con2prim(int eos, double G, const double U[5], double W[5], int *niter_out) {
+  if (niter_out) *niter_out = 0;
+  if (!orc_admissible(U, 0.0)) {            /* Eq. 25: the solvers are specified on admissible U */
+    for (int v = 0; v < 5; ++v) W[v] = NAN;
+    return 1;
+  }
+  if (eos == ORC_EOS_IDEAL) return con2prim_ideal(G, U, W, niter_out, -1);
+  return con2prim_tm(U, W);
+}
+
+int orc_con2prim_ideal_fixed(double G, const double U[5], double W[5], int niter) {
+  return con2prim_ideal(G, U, W, 0, niter);
+}
+
+void orc_prim2con_batch(int eos, double G, int64_t n, const double *W, double *U) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    double w[5], u[5];
+    for (int v = 0; v < 5; ++v) w[v] = W[v * n + i];
+    orc_prim2con(eos, G, w, u);
+    for (int v = 0; v < 5; ++v) U[v * n + i] = u[v];
+  }
+}
+
+void orc_con2prim_batch(int eos, double G, int64_t n, const double *U, double *W, int *status) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    double w[5], u[5];
+    for (int v = 0; v < 5; ++v) u[v] = U[v * n + i];
+    int st = orc_con2prim(eos, G, u, w, 0);
+    for (int v = 0; v < 5; ++v) W[v * n + i] = w[v];
+    if (status) status[i] = st;
+  }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Mesh helpers
+ * ------------------------------------------------------------------------------------------ */
+static int ipow(int b, int e) { int r = 1; while (e-- > 0) r *= b; return r; }
+
+int64_t orc_ndof(const orc_config *c) {
+  int64_t ne = 1;
+  for (int d = 0; d < c->ndim; ++d) ne *= c->nelem[d];
+  return ne * ipow(c->order_p + 1, c->ndim);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O5  Spatial operator L(U)  (Eq. 15-18; steps in the order of :128-145).
+ *   R_i = sum_d (2/h_d)(1/w_{i_d}) [ sum_q w_q D_{q,i_d} F_d(W_{..q..})
+ *                                    - (delta_{i_d,p} Fhat_{d,+} - delta_{i_d,0} Fhat_{d,-}) ]
+ * GLL collocation: "interpolation to quadrature points" (:132) is the identity in the volume and
+ * a gather of the face node on faces, because l_i(+-1) = delta (reading R1).
+ * ------------------------------------------------------------------------------------------ */
+void orc_rhs(const orc_config *c, const double *U, double *R, int64_t *n_c2p_fail) {
+  const int nd = c->ndim, N = c->order_p + 1, nn = ipow(N, nd);
+  const int64_t nx = c->nelem[0], ny = nd > 1 ? c->nelem[1] : 1, nz = nd > 2 ? c->nelem[2] : 1;
+  const int64_t ne = nx * ny * nz, ndof = ne * nn;
+  double x[5], w[5], D[25], h[3];
+  orc_gll(N, x, w, D);
+  for (int d = 0; d < nd; ++d) h[d] = (c->xmax[d] - c->xmin[d]) / (double)c->nelem[d];
+  const int64_t nel[3] = {nx, ny, nz};
+  const int str[3] = {1, N, N * N};          /* node stride per direction */
+
+  /* step 1 (Eq. 16): W_i = p(U_i) at every nodal point */
+  double *W = (double *)malloc(sizeof(double) * 5 * (size_t)ndof);
+  int64_t nfail = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nfail)
+  for (int64_t i = 0; i < ndof; ++i) {
+    double u[5], p[5];
+    for (int v = 0; v < 5; ++v) u[v] = U[v * ndof + i];
+    if (orc_con2prim(c->eos, c->gamma_ad, u, p, 0) != 0) nfail++;
+    for (int v = 0; v < 5; ++v) W[v * ndof + i] = p[v];
+  }
+  if (n_c2p_fail) *n_c2p_fail += nfail;
+
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    int64_t ie[3] = {e % nx, (e / nx) % ny, e / (nx * ny)};
+    /* physical flux at every node of the element, every direction (Eq. 2) */
+    double Fe[3][125][5];
+    for (int n = 0; n < nn; ++n) {
+      double p[5];
+      for (int v = 0; v < 5; ++v) p[v] = W[v * ndof + e * nn + n];
+      for (int d = 0; d < nd; ++d) orc_flux(c->eos, c->gamma_ad, p, d, Fe[d][n]);
+    }
+    for (int n = 0; n < nn; ++n) {
+      int in[3] = {n % N, (n / N) % N, n / (N * N)};
+      double acc[5] = {0, 0, 0, 0, 0};
+      for (int d = 0; d < nd; ++d) {
+        double term[5] = {0, 0, 0, 0, 0};
+        /* volume quadrature, Eq. 17 */
+        for (int q = 0; q < N; ++q) {
+          int nq = n + (q - in[d]) * str[d];
+          for (int v = 0; v < 5; ++v) term[v] += w[q] * D[q * N + in[d]] * Fe[d][nq][v];
+        }
+        /* surface quadrature, Eq. 18/20 */
+        for (int side = 0; side < 2; ++side) {
+          if (side == 0 && in[d] != 0) continue;        /* l_i(-1) = delta_{i,0} */
+          if (side == 1 && in[d] != N - 1) continue;    /* l_i(+1) = delta_{i,p} */
+          int64_t je[3] = {ie[0], ie[1], ie[2]};
+          je[d] += side ? 1 : -1;
+          int has_nb = 1;
+          if (je[d] < 0 || je[d] >= nel[d]) {
+            if (c->bc[d] == ORC_BC_PERIODIC) je[d] = (je[d] + nel[d]) % nel[d];
+            else has_nb = 0;                            /* outflow: ghost = own face state (R12) */
+          }
+          int64_t en = je[0] + nx * (je[1] + ny * je[2]);
+          int n_nb = n + ((side ? 0 : N - 1) - in[d]) * str[d];   /* neighbour's facing node */
+          double Wown[5], Wnb[5], Fh[5];
+          for (int v = 0; v < 5; ++v) {
+            Wown[v] = W[v * ndof + e * nn + n];
+            Wnb[v] = has_nb ? W[v * ndof + en * nn + n_nb] : Wown[v];
+          }
+          if (side) orc_hll(c->eos, c->gamma_ad, Wown, Wnb, d, Fh);   /* left = own  */
+          else      orc_hll(c->eos, c->gamma_ad, Wnb, Wown, d, Fh);   /* left = neighbour */
+          for (int v = 0; v < 5; ++v) term[v] -= side ? Fh[v] : -Fh[v];
+        }
+        for (int v = 0; v < 5; ++v) acc[v] += (2.0 / h[d]) * (1.0 / w[in[d]]) * term[v];
+      }
+      for (int v = 0; v < 5; ++v) R[v * ndof + e * nn + n] = acc[v];
+    }
+  }
+  free(W);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O7  Physicality-enforcing operator (steps 1-4 of :242-252).
+ * ------------------------------------------------------------------------------------------ */
+/* Per-node largest smoothing factor s_i = s1*s2 toward an admissible mean Ubar
+ * (Eq. 28-37; Eq. 37's root evaluated in the cancellation-free form of reading R14;
+ * E is replaced by (1-eps_q)E in the predicate and in c, n, g -- reading R13c). */
+double orc_limiter_node_s(const double Ubar[5], const double Ui[5], double eps_q) {
+  /* stage 1, Eq. 28-30 */
+  double sD = Ui[0] > 0.0 ? 1.0 : Ubar[0] / (Ubar[0] - Ui[0]);
+  double sE = Ui[4] > 0.0 ? 1.0 : Ubar[4] / (Ubar[4] - Ui[4]);
+  double s1 = fmin(sD, sE);
+  double U1[5];
+  for (int v = 0; v < 5; ++v) U1[v] = Ubar[v] + s1 * (Ui[v] - Ubar[v]);
+  if (orc_admissible(U1, eps_q)) return s1;                         /* step 3(c) */
+  /* stage 2, Eq. 31-37 with <A,B> = A_E B_E - A_D B_D - A_M.B_M, E -> (1-eps_q)E */
+  double f = 1.0 - eps_q;
+  double Eb = f * Ubar[4], E1 = f * U1[4];
+  double nb = sqrt(Ubar[0] * Ubar[0] + Ubar[1] * Ubar[1] + Ubar[2] * Ubar[2] + Ubar[3] * Ubar[3]);
+  double n1 = sqrt(U1[0] * U1[0] + U1[1] * U1[1] + U1[2] * U1[2] + U1[3] * U1[3]);
+  double cc = (Eb - nb) * (Eb + nb);                                /* Eq. 36: <Ubar,Ubar> > 0 */
+  double nn = (E1 - n1) * (E1 + n1);                                /* <U1,U1> */
+  if (!(nn < 0.0)) return s1;            /* q(U1) >= 0: only D1 <= 0 failed; delta_s handles it */
+  double g = Eb * E1 - Ubar[0] * U1[0] - Ubar[1] * U1[1] - Ubar[2] * U1[2] - Ubar[3] * U1[3];
+  double r = sqrt(g * g - cc * nn);
+  double A = g >= 0.0 ? g + r : -cc * nn / (r - g);
+  double s2 = A / (A - nn);                                         /* = Eq. 37's root */
+  return s1 * s2;
+}
+
+void orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag, double *s_out,
+                             int64_t counters[2]) {
+  const int nd = c->ndim, N = c->order_p + 1, nn = ipow(N, nd);
+  int64_t ne = 1;
+  for (int d = 0; d < nd; ++d) ne *= c->nelem[d];
+  const int64_t ndof = ne * nn;
+  double x[5], w[5], D[25];
+  orc_gll(N, x, w, D);
+  int64_t nflag = 0, nbad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nflag, nbad)
+  for (int64_t e = 0; e < ne; ++e) {
+    /* cell volume average, tensor GLL weights, fixed node order */
+    double Ub[5] = {0, 0, 0, 0, 0}, wsum = 0.0;
+    int bad = 0;
+    for (int n = 0; n < nn; ++n) {
+      double wn = w[n % N];
+      if (nd > 1) wn *= w[(n / N) % N];
+      if (nd > 2) wn *= w[n / (N * N)];
+      wsum += wn;
+      double u[5];
+      for (int v = 0; v < 5; ++v) { u[v] = U[v * ndof + e * nn + n]; Ub[v] += wn * u[v]; }
+      if (!orc_admissible(u, 0.5 * c->eps_q)) bad = 1;              /* step 1: screen */
+    }
+    if (flag) flag[e] = (unsigned char)bad;
+    if (!bad) { if (s_out) s_out[e] = 1.0; continue; }
+    nflag++;
+    for (int v = 0; v < 5; ++v) Ub[v] /= wsum;
+    double s = 1.0;
+    if (!orc_admissible(Ub, c->eps_q)) {                            /* step 2; R13d */
+      nbad++;
+      s = 0.0;
+    } else {
+      for (int n = 0; n < nn; ++n) {                                /* step 3 */
+        double u[5];
+        for (int v = 0; v < 5; ++v) u[v] = U[v * ndof + e * nn + n];
+        double si = orc_limiter_node_s(Ub, u, c->eps_q);
+        if (!(si >= 0.0)) si = 0.0;                                 /* NaN guard */
+        if (si < s) s = si;                                         /* step 4: s = min s_i */
+      }
+      s = (1.0 - c->delta_s) * s;                                   /* R13c */
+    }
+    if (s_out) s_out[e] = s;
+    double t = 1.0 - s;
+    for (int n = 0; n < nn; ++n)                                    /* Eq. 26, nearer end (R14) */
+      for (int v = 0; v < 5; ++v) {
+        double ui = U[v * ndof + e * nn + n];
+        U[v * ndof + e * nn + n] = (s > 0.5) ? ui + t * (Ub[v] - ui) : Ub[v] + s * (ui - Ub[v]);
+      }
+  }
+  if (counters) { counters[0] += nflag; counters[1] += nbad; }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * R11  CFL time step ("adaptive time stepping ... to maintain a certain CFL"):
+ *   dt = CFL / max_nodes sum_d (2p+1) max(|lambda-_d|,|lambda+_d|)/h_d
+ * ------------------------------------------------------------------------------------------ */
+double orc_cfl_dt(const orc_config *c, const double *U, double cfl) {
+  const int nd = c->ndim;
+  const int64_t ndof = orc_ndof(c);
+  double h[3];
+  for (int d = 0; d < nd; ++d) h[d] = (c->xmax[d] - c->xmin[d]) / (double)c->nelem[d];
+  double amax = 0.0;
+#pragma omp parallel for schedule(static) reduction(max : amax)
+  for (int64_t i = 0; i < ndof; ++i) {
+    double u[5], p[5];
+    for (int v = 0; v < 5; ++v) u[v] = U[v * ndof + i];
+    orc_con2prim(c->eos, c->gamma_ad, u, p, 0);
+    double a = 0.0;
+    for (int d = 0; d < nd; ++d) {
+      double lm, lp;
+      orc_wavespeeds(c->eos, c->gamma_ad, p, d, &lm, &lp);
+      a += (double)(2 * c->order_p + 1) * fmax(fabs(lm), fabs(lp)) / h[d];
+    }
+    if (a > amax) amax = a;       /* NaN never wins (comparison false) */
+  }
+  return cfl / amax;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * O6  SSP-RK in Shu-Osher form (coefficients: reading R10); the
+ * physicality operator after every stage's combine (reading R15).
+ *   stage: U_out = a U0 + b (U_s + dt L(U_s)),  (a,b) = (0,1), (3/4,1/4), (1/3,2/3)
+ *   SSPRK2 second stage (1/2,1/2).
+ * ------------------------------------------------------------------------------------------ */
+void orc_step(const orc_config *c, double *U, double dt_in, int nsteps, double *t_inout,
+              int64_t counters[3]) {
+  const int64_t ndof = orc_ndof(c);
+  const size_t nb = sizeof(double) * 5 * (size_t)ndof;
+  double *U0 = (double *)malloc(nb), *R = (double *)malloc(nb);
+  double A[3], B[3];
+  A[0] = 0.0; B[0] = 1.0;
+  if (c->rk_stages == 2) { A[1] = 0.5; B[1] = 0.5; }
+  else { A[1] = 0.75; B[1] = 0.25; A[2] = 1.0 / 3.0; B[2] = 2.0 / 3.0; }
+  for (int step = 0; step < nsteps; ++step) {
+    double dt = dt_in > 0.0 ? dt_in : orc_cfl_dt(c, U, -dt_in);
+    memcpy(U0, U, nb);
+    for (int st = 0; st < c->rk_stages; ++st) {
+      int64_t nf = 0, lim[2] = {0, 0};
+      orc_rhs(c, U, R, &nf);
+#pragma omp parallel for schedule(static)
+      for (int64_t i = 0; i < 5 * ndof; ++i) U[i] = A[st] * U0[i] + B[st] * (U[i] + dt * R[i]);
+      orc_enforce_physicality(c, U, 0, 0, lim);
+      if (counters) { counters[0] += lim[0]; counters[1] += lim[1]; counters[2] += nf; }
+    }
+    if (t_inout) *t_inout += dt;
+  }
+  free(U0);
+  free(R);
+}

@@ -1,0 +1,70 @@
+/* dgrhd_oracle.h -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU restatement of the DG special-relativistic-hydro stage of
+ * arxiv 2205.00095 ("PAPER.md"), written from the paper's equations in the paper's order.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may use anything under oracle/.  It shares no code, header, table or constant generator
+ * with paper_2205_00095_b200/ (the CUDA path); neither includes the other.
+ *
+ * Units: c = 1 throughout (PAPER.md keeps c; every workload here is in units of c).
+ * Layout (canonical, SoA by variable): X[v][e][n], v in {D|rho, Mx|ux, My|uy, Mz|uz, E|P},
+ *   e = ix + nx*(iy + ny*iz), n = i + N*(j + N*k), N = p+1.   Primitive velocity is the
+ *   spatial 4-velocity u = gamma*v.
+ *
+ * Readings of the paper (R#) are the ones listed in DESIGN.md "Readings".
+ */
+#ifndef DGRHD_ORACLE_H
+#define DGRHD_ORACLE_H
+#include <stdint.h>
+
+enum { ORC_EOS_IDEAL = 0, ORC_EOS_TM = 1 };
+enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1 };
+
+typedef struct {
+  int     ndim;          /* 1,2,3 */
+  int64_t nelem[3];      /* elements per axis (unused = 1) */
+  double  xmin[3], xmax[3];
+  int     bc[3];
+  int     order_p;       /* 0..4 */
+  int     eos;
+  double  gamma_ad;
+  int     rk_stages;     /* 1,2,3 */
+  double  eps_q, delta_s;
+} orc_config;
+
+/* O4: GLL tables for N = p+1 nodes: x[N], w[N], D[q*N+i] = l_i'(x_q). */
+void orc_gll(int N, double *x, double *w, double *D);
+
+/* O1 */
+double orc_enthalpy(int eos, double G, double rho, double P);
+double orc_cs2(int eos, double G, double rho, double P);
+void   orc_prim2con(int eos, double G, const double W[5], double U[5]);
+void   orc_flux(int eos, double G, const double W[5], int dir, double F[5]);
+void   orc_wavespeeds(int eos, double G, const double W[5], int dir, double *lm, double *lp);
+void   orc_hll(int eos, double G, const double WL[5], const double WR[5], int dir, double F[5]);
+
+/* O2/O3: returns status 0 ok, 1 inadmissible input (W = NaN), 2 solver/pressure failure.
+ * niter_out (may be NULL) receives the Newton iteration count (ideal EOS). */
+int    orc_con2prim(int eos, double G, const double U[5], double W[5], int *niter_out);
+/* ideal EOS Newton with a caller-fixed iteration count and no stopping test (Fig. 2 protocol) */
+int    orc_con2prim_ideal_fixed(double G, const double U[5], double W[5], int niter);
+
+void   orc_prim2con_batch(int eos, double G, int64_t n, const double *W, double *U);
+void   orc_con2prim_batch(int eos, double G, int64_t n, const double *U, double *W, int *status);
+
+/* O7 building blocks (exposed for the pins) */
+int    orc_admissible(const double U[5], double eps);
+double orc_limiter_node_s(const double Ubar[5], const double Ui[5], double eps_q);
+
+/* O5..O7, R10, R11 on the canonical layout; ndof = nelem_total * N^ndim */
+int64_t orc_ndof(const orc_config *c);
+void   orc_rhs(const orc_config *c, const double *U, double *R, int64_t *n_c2p_fail);
+void   orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag, double *s,
+                               int64_t counters[2]);
+double orc_cfl_dt(const orc_config *c, const double *U, double cfl);
+/* dt > 0 fixed; dt <= 0: CFL number -dt, recomputed every step.  counters[3] accumulates
+ * n_flagged, n_bad_mean, n_c2p_fail over all stages. */
+void   orc_step(const orc_config *c, double *U, double dt, int nsteps, double *t_inout,
+                int64_t counters[3]);
+int    orc_num_threads(void);
+#endif

@@ -1,0 +1,461 @@
+"""Pins for the oracle's DG operator (O5), time integration (O6, R10, R11) and the
+physicality-enforcing operator (O7).
+
+Nothing here compares the oracle with itself: the residual is checked against the strong-form
+divergence of the (separately pinned) pointwise flux, against conservation / free-stream /
+symmetry invariants, and against the exact solution of the entropy wave; the limiter against
+its stated properties and a brute-force bisection on s; the CFL step
+against a closed form.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_2205_00095_b200 import inputs as I
+
+
+def _cfg(d):
+    return O.make_config(d["ndim"], d["nelem"], d["xmin"], d["xmax"], d["bc"], d["order_p"],
+                         d["eos"], d["gamma_ad"], d["rk_stages"], d["eps_q"], d["delta_s"])
+
+
+def _node_weights(nd, N):
+    _, w, _ = O.gll(N)
+    wn = w.copy()
+    for _ in range(nd - 1):
+        wn = np.multiply.outer(w, wn)      # index order [k][j][i] -> flat n = i + N(j + N k)
+    return wn.reshape(-1)
+
+
+def _smooth_field(nd, nelem, N, xmin, xmax, seed):
+    """Smooth periodic primitives on the node grid + a callable W(x) for the same field."""
+    rng = np.random.default_rng(seed)
+    ph = rng.uniform(0, 2 * np.pi, size=(5, 3))
+    L = [xmax[d] - xmin[d] for d in range(nd)]
+
+    def field(X):          # X: [nd, npts]
+        s = [sum(np.sin(2 * np.pi * (X[d] - xmin[d]) / L[d] + ph[v, d]) for d in range(nd))
+             for v in range(5)]
+        rho = 1.0 + 0.3 * s[0] / nd
+        P = 0.7 + 0.2 * s[4] / nd
+        u = [0.4 * s[1 + k] / nd for k in range(3)]
+        return np.stack([rho, u[0], u[1], u[2], P])
+
+    axes = [I.axis_coords(xmin[d], xmax[d], nelem[d], N).numpy() for d in range(nd)]
+    if nd == 1:
+        Xg = axes[0][None, :]
+        shape = (nelem[0] * N,)
+    elif nd == 2:
+        yy, xx = np.meshgrid(axes[1], axes[0], indexing="ij")
+        Xg = np.stack([xx.ravel(), yy.ravel()])
+        shape = (nelem[1] * N, nelem[0] * N)
+    else:
+        zz, yy, xx = np.meshgrid(axes[2], axes[1], axes[0], indexing="ij")
+        Xg = np.stack([xx.ravel(), yy.ravel(), zz.ravel()])
+        shape = (nelem[2] * N, nelem[1] * N, nelem[0] * N)
+    import torch
+    Wg = torch.from_numpy(field(Xg)).reshape(5, *shape)
+    Xc = torch.from_numpy(Xg).reshape(nd, *shape)
+    W = I.grid_to_canonical(Wg, list(nelem), N).numpy()
+    X = I.grid_to_canonical(Xc, list(nelem), N).numpy()
+    return np.ascontiguousarray(W), np.ascontiguousarray(X), field
+
+
+# ---------------------------------------------------------------- O5: residual ----------------
+@pytest.mark.parametrize("nd,nelem,p,eos,G", [
+    (1, [24], 3, O.EOS_IDEAL, 5.0 / 3.0),
+    (2, [12, 20], 3, O.EOS_TM, 0.0),
+    (3, [6, 8, 10], 3, O.EOS_IDEAL, 4.0 / 3.0),
+    (2, [16, 10], 4, O.EOS_IDEAL, 4.0 / 3.0),
+])
+def test_rhs_is_minus_divergence_of_flux_for_smooth_fields(nd, nelem, p, eos, G):
+    """R_i -> -sum_d dF_d/dx_d at the node (strong form of Eq. 1) as h -> 0: pins sign, the 2/h_d
+    scaling per axis (h differs per axis here), the D-matrix orientation, the axis<->flux
+    pairing and the surface term (a wrong lift leaves an O(1/h) error at face nodes)."""
+    N = p + 1
+    xmin, xmax = [0.0, -1.0, 0.5][:nd], [1.0, 0.5, 2.5][:nd]
+    cfg = O.make_config(nd, nelem, xmin, xmax, [O.BC_PERIODIC] * nd, p, eos, G)
+    W, X, field = _smooth_field(nd, nelem, N, xmin, xmax, seed=3)
+    U = O.prim2con_batch(eos, G, W)
+    R, nf = O.rhs(cfg, U)
+    assert nf == 0
+    rng = np.random.default_rng(0)
+    idx = rng.choice(W.shape[1], size=60, replace=False)
+    # make sure face/corner nodes are in the sample
+    idx[:8] = np.arange(8) * (N ** nd // 8 if N ** nd >= 8 else 1)
+    eps = 1e-5
+    errs = []
+    for j in idx:
+        div = np.zeros(5)
+        for d in range(nd):
+            xp, xm = X[:, j].copy(), X[:, j].copy()
+            xp[d] += eps; xm[d] -= eps
+            Fp = O.flux(eos, G, field(xp[:, None])[:, 0], d)
+            Fm = O.flux(eos, G, field(xm[:, None])[:, 0], d)
+            div += (Fp - Fm) / (2 * eps)
+        errs.append(np.abs(R[:, j] + div).max())
+    scale = np.abs(R).max()
+    assert scale > 0.1
+    assert max(errs) < 2e-2 * scale, (max(errs), scale)
+    # and it converges: halve h, error drops by about 2^p (accept >= 2^(p-1))
+    nelem2 = [2 * n for n in nelem] if nd < 3 else None
+    if nelem2:
+        cfg2 = O.make_config(nd, nelem2, xmin, xmax, [O.BC_PERIODIC] * nd, p, eos, G)
+        W2, X2, _ = _smooth_field(nd, nelem2, N, xmin, xmax, seed=3)
+        R2, _ = O.rhs(cfg2, O.prim2con_batch(eos, G, W2))
+        errs2 = []
+        for j in rng.choice(W2.shape[1], size=60, replace=False):
+            div = np.zeros(5)
+            for d in range(nd):
+                xp, xm = X2[:, j].copy(), X2[:, j].copy()
+                xp[d] += eps; xm[d] -= eps
+                div += (O.flux(eos, G, field(xp[:, None])[:, 0], d)
+                        - O.flux(eos, G, field(xm[:, None])[:, 0], d)) / (2 * eps)
+            errs2.append(np.abs(R2[:, j] + div).max())
+        assert max(errs2) < max(errs) / 2 ** (p - 1)
+
+
+@pytest.mark.parametrize("nd,nelem,p,eos,G,bc", [
+    (1, [7], 2, O.EOS_IDEAL, 5.0 / 3.0, [O.BC_OUTFLOW]),
+    (2, [5, 4], 2, O.EOS_TM, 0.0, [O.BC_PERIODIC, O.BC_OUTFLOW]),
+    (3, [3, 4, 2], 3, O.EOS_IDEAL, 5.0 / 3.0, [O.BC_PERIODIC] * 3),
+    (3, [2, 2, 3], 1, O.EOS_TM, 0.0, [O.BC_OUTFLOW] * 3),
+    (2, [4, 3], 0, O.EOS_IDEAL, 4.0 / 3.0, [O.BC_PERIODIC] * 2),
+])
+def test_rhs_free_stream_is_zero(nd, nelem, p, eos, G, bc):
+    cfg = O.make_config(nd, nelem, [0.0] * nd, [1.0, 2.0, 0.5][:nd], bc, p, eos, G)
+    n = O.ndof(cfg)
+    W = np.tile(np.array([0.8, 0.9, -0.4, 0.3, 1.7])[:, None], (1, n))
+    U = O.prim2con_batch(eos, G, W)
+    R, nf = O.rhs(cfg, U)
+    assert nf == 0
+    assert np.abs(R).max() < 1e-11 * np.abs(U).max() * max(nelem)
+
+
+@pytest.mark.parametrize("nd,nelem,p,eos,G", [
+    (1, [9], 2, O.EOS_IDEAL, 5.0 / 3.0),
+    (2, [5, 6], 2, O.EOS_TM, 0.0),
+    (3, [3, 4, 3], 3, O.EOS_IDEAL, 5.0 / 3.0),
+])
+def test_rhs_conserves_on_periodic_domain(nd, nelem, p, eos, G):
+    """sum_e sum_i w_i R_i = 0 per variable: interface fluxes cancel pairwise and the volume term
+    sums to the boundary term (SBP).  Rough (discontinuous, random) data so HLL is really used."""
+    N = p + 1
+    cfg = O.make_config(nd, nelem, [0.0] * nd, [1.0, 0.7, 1.3][:nd], [O.BC_PERIODIC] * nd, p, eos, G)
+    n = O.ndof(cfg)
+    rng = np.random.default_rng(5)
+    W = np.stack([10 ** rng.uniform(-1, 1, n), *(rng.normal(size=(3, n)) * 0.8),
+                  10 ** rng.uniform(-2, 1, n)])
+    U = O.prim2con_batch(eos, G, W)
+    R, _ = O.rhs(cfg, U)
+    wn = np.tile(_node_weights(nd, N), n // N ** nd)
+    tot = (R * wn).sum(1)
+    ref = (np.abs(R) * wn).sum(1)
+    assert np.all(np.abs(tot) < 1e-13 * ref.max()), (tot, ref)
+
+
+def test_rhs_mirror_symmetry_1d():
+    """x -> -x with u_x -> -u_x maps R(D,My,Mz,E) to itself reversed and R(Mx) to its negative."""
+    p, ne = 3, 11
+    N = p + 1
+    cfg = O.make_config(1, [ne], [0.0], [1.0], [O.BC_PERIODIC], p, O.EOS_TM, 0.0)
+    rng = np.random.default_rng(8)
+    n = ne * N
+    W = np.stack([10 ** rng.uniform(-1, 1, n), *(rng.normal(size=(3, n)) * 0.5),
+                  10 ** rng.uniform(-1, 1, n)])
+    Wm = W[:, ::-1].copy()
+    Wm[1] *= -1
+    R, _ = O.rhs(cfg, O.prim2con_batch(O.EOS_TM, 0.0, W))
+    Rm, _ = O.rhs(cfg, O.prim2con_batch(O.EOS_TM, 0.0, Wm))
+    sgn = np.array([1, -1, 1, 1, 1.0])[:, None]
+    assert np.allclose(Rm[:, ::-1] * sgn, R, rtol=0, atol=1e-12 * np.abs(R).max())
+
+
+def test_rhs_axis_permutation_3d():
+    """Relabelling axes (x,y,z)->(y,z,x) of data, mesh and velocity components permutes R the
+    same way: catches any axis-specific indexing slip in the 3D loops."""
+    p, N = 2, 3
+    ne = [3, 4, 5]
+    xmax = [1.0, 0.8, 1.5]
+    rng = np.random.default_rng(9)
+    Wg = np.stack([10 ** rng.uniform(-1, 1, (ne[2] * N, ne[1] * N, ne[0] * N)),
+                   *(rng.normal(size=(3, ne[2] * N, ne[1] * N, ne[0] * N)) * 0.5),
+                   10 ** rng.uniform(-1, 1, (ne[2] * N, ne[1] * N, ne[0] * N))])
+    import torch
+    cfgA = O.make_config(3, ne, [0.0] * 3, xmax, [O.BC_PERIODIC] * 3, p, O.EOS_IDEAL, 5 / 3)
+    WA = I.grid_to_canonical(torch.from_numpy(Wg), ne, N).numpy()
+    RA, _ = O.rhs(cfgA, O.prim2con_batch(0, 5 / 3, np.ascontiguousarray(WA)))
+    # new axes: x' = y, y' = z, z' = x  => grid[z',y',x'] = old[x? ...]: old index order (z,y,x)
+    WgB = np.transpose(Wg, (0, 3, 1, 2))[[0, 2, 3, 1, 4]]      # [v, x, z, y] ; u' = (uy, uz, ux)
+    neB = [ne[1], ne[2], ne[0]]
+    xmaxB = [xmax[1], xmax[2], xmax[0]]
+    cfgB = O.make_config(3, neB, [0.0] * 3, xmaxB, [O.BC_PERIODIC] * 3, p, O.EOS_IDEAL, 5 / 3)
+    WB = I.grid_to_canonical(torch.from_numpy(np.ascontiguousarray(WgB)), neB, N).numpy()
+    RB, _ = O.rhs(cfgB, O.prim2con_batch(0, 5 / 3, np.ascontiguousarray(WB)))
+
+    def to_grid(Rc, nel):     # canonical -> [v, Z, Y, X]
+        nx, ny, nz = nel
+        return Rc.reshape(5, nz, ny, nx, N, N, N).transpose(0, 1, 4, 2, 5, 3, 6).reshape(
+            5, nz * N, ny * N, nx * N)
+    RgA, RgB = to_grid(RA, ne), to_grid(RB, neB)
+    RgA_perm = np.transpose(RgA, (0, 3, 1, 2))[[0, 2, 3, 1, 4]]
+    assert np.allclose(RgB, RgA_perm, rtol=0, atol=1e-12 * np.abs(RA).max())
+
+
+# ---------------------------------------------------------------- O6: SSP-RK, CFL -------------
+def _wave_l1(ne, p, cfl=None, dt=None, T=2.0, amp=1e-4, seed=1):
+    d, W, x, phi = I.wave1d(seed, ne, p, amp=amp)
+    cfg = _cfg(d)
+    U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+    if dt is None:
+        dt0 = O.cfl_dt(cfg, U, cfl)
+        nst = int(math.ceil(T / dt0))
+        dt = T / nst
+    else:
+        nst = int(round(T / dt))
+    U1, t1, cnt = O.step(cfg, U, dt, nst)
+    assert abs(t1 - T) < 1e-12 and cnt == (0, 0, 0)
+    Wex = I.wave1d_exact(x, T, phi, amp=amp).numpy()
+    W1, st = O.con2prim_batch(cfg.eos, cfg.gamma_ad, U1)
+    wn = np.tile(_node_weights(1, p + 1), ne) * (0.5 / ne)
+    return float((np.abs(W1[0] - Wex[0]) * wn).sum())
+
+
+@pytest.mark.parametrize("p,nes", [(1, [32, 64, 128]), (2, [16, 32, 64]), (3, [8, 16, 32])])
+def test_entropy_wave_converges_at_order_p_plus_1(p, nes):
+    """expected order p+1 on smooth linear waves (config 2; exact solution known).
+    For p=3 the RK3 time error is kept below the spatial one by dt ~ h^(4/3)."""
+    errs = []
+    for ne in nes:
+        if p < 3:
+            errs.append(_wave_l1(ne, p, cfl=0.3))
+        else:
+            errs.append(_wave_l1(ne, p, dt=2.0 / math.ceil(2.0 / (0.02 * (8.0 / ne) ** (4.0 / 3.0)))))
+    orders = [math.log2(errs[k] / errs[k + 1]) for k in range(len(errs) - 1)]
+    assert all(e > 1e-11 for e in errs[:-1])
+    assert all(abs(o - (p + 1)) < 0.35 for o in orders), (errs, orders)
+
+
+def test_ssprk3_is_third_order_in_time_and_lower_schemes_match_their_order():
+    """R10: temporal self-convergence of the semi-discrete ODE system (the spatial error cancels
+    in differences): (U(dt)-U(dt/2)) / (U(dt/2)-U(dt/4)) -> 2^order with order 3 for SSPRK3,
+    2 for SSPRK2, 1 for RK1 -- a property of the Shu-Osher coefficients, not of this code."""
+    for stages, want in ((3, 3), (2, 2), (1, 1)):
+        sols = []
+        for dt in (0.004, 0.002, 0.001):
+            d, W, x, phi = I.wave1d(4, 8, 1, amp=0.05)
+            d["rk_stages"] = stages
+            cfg = _cfg(d)
+            U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+            T = 0.1
+            U1, _, _ = O.step(cfg, U, dt, int(round(T / dt)))
+            sols.append(U1[0])
+        e1 = np.abs(sols[0] - sols[1]).max()
+        e2 = np.abs(sols[1] - sols[2]).max()
+        order = math.log2(e1 / e2)
+        assert e2 > 1e-13 and abs(order - want) < 0.25, (stages, e1, e2, order)
+
+
+def test_step_keeps_uniform_state_and_counts_time():
+    d, W = I.riemann1d(0, ne=8, p=2, states=((1.0, 0.3, 0.1, 2.0), (1.0, 0.3, 0.1, 2.0)))
+    cfg = _cfg(d)
+    U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+    U1, t1, cnt = O.step(cfg, U, 1e-3, 7, t=0.5)
+    assert abs(t1 - 0.507) < 1e-15 and cnt == (0, 0, 0)
+    assert np.abs(U1 - U).max() < 1e-13
+
+
+@pytest.mark.parametrize("eos,G", [(O.EOS_IDEAL, 5.0 / 3.0), (O.EOS_TM, 0.0)])
+def test_cfl_dt_closed_form_at_rest(eos, G):
+    """R11 at rest: lambda+- = +-cs in every direction => dt = cfl / ((2p+1) cs sum_d 1/h_d)."""
+    p = 2
+    cfg = O.make_config(3, [4, 5, 8], [0.0] * 3, [1.0, 1.0, 4.0], [O.BC_PERIODIC] * 3, p, eos, G)
+    n = O.ndof(cfg)
+    W = np.tile(np.array([1.0, 0, 0, 0, 0.1])[:, None], (1, n))
+    W[:, 37] = [0.5, 0, 0, 0, 3.0]           # the hottest node sets the step
+    U = O.prim2con_batch(eos, G, W)
+    cs = math.sqrt(O.cs2(eos, G, 0.5, 3.0))
+    want = 0.3 / ((2 * p + 1) * cs * (4 / 1.0 + 5 / 1.0 + 8 / 4.0))
+    assert abs(O.cfl_dt(cfg, U, 0.3) / want - 1) < 1e-13
+
+
+def test_cfl_dt_moving_state_uses_the_faster_characteristic():
+    cfg = O.make_config(1, [10], [0.0], [2.0], [O.BC_OUTFLOW], 1, O.EOS_IDEAL, 5.0 / 3.0)
+    v = -0.6
+    W = np.tile(np.array([1.0, v / math.sqrt(1 - v * v), 0, 0, 1.0])[:, None], (1, 20))
+    cs = math.sqrt(O.cs2(0, 5 / 3, 1.0, 1.0))
+    lam = (abs(v) + cs) / (1 + abs(v) * cs)
+    dt = O.cfl_dt(cfg, O.prim2con_batch(0, 5 / 3, W), 0.5)
+    assert abs(dt / (0.5 * 0.2 / (3 * lam)) - 1) < 1e-13
+
+
+def test_periodic_evolution_conserves_integrals_with_limiter_active():
+    """Periodic-domain conservation of int D, M, E over full SSPRK3 steps, limiter firing
+    (the operator preserves the cell average)."""
+    d, W = I.box3d(3, n=6, p=2, kmax=1)
+    cfg = _cfg(d)
+    U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+    wn = np.tile(_node_weights(3, 3), U.shape[1] // 27)
+    U1, t1, cnt = O.step(cfg, U, -0.3, 4)
+    assert cnt[0] > 0 and cnt[1] == 0 and cnt[2] == 0           # fired; no bad mean; no c2p failure
+    drift = np.abs(((U1 - U) * wn).sum(1))
+    ref = (np.abs(U) * wn).sum(1)
+    assert np.all(drift < 1e-13 * ref[4]), (drift, ref)
+    assert np.all(np.isfinite(U1))
+
+
+# ---------------------------------------------------------------- O7: physicality operator ----
+def _q(U, eps=0.0):
+    return (1 - eps) * U[4] - np.sqrt(U[0] ** 2 + U[1] ** 2 + U[2] ** 2 + U[3] ** 2)
+
+
+def _bisect_s(Ub, Ui, eps):
+    """largest s in [0,1] with Ubar + s (U_i - Ubar) admissible, by brute-force bisection
+    (the admissible set is convex, so the admissible s form an interval [0, s*))."""
+    f = lambda s: O.admissible(Ub + s * (Ui - Ub), eps)
+    if f(1.0):
+        return 1.0
+    lo, hi = 0.0, 1.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        if f(mid):
+            lo = mid
+        else:
+            hi = mid
+    return lo
+
+
+def test_limiter_node_s_equals_bisection_on_random_pairs():
+    rng = np.random.default_rng(12)
+    eps = 1e-12
+    ncheck = 0
+    for _ in range(3000):
+        # admissible mean
+        D = 10 ** rng.uniform(-3, 1)
+        M = rng.normal(size=3) * 10 ** rng.uniform(-2, 1)
+        E = math.sqrt(D * D + M @ M) * (1 + 10 ** rng.uniform(-4, 1))
+        Ub = np.array([D, *M, E])
+        # node: random, often inadmissible in different ways
+        kind = rng.integers(4)
+        Ui = np.array([10 ** rng.uniform(-3, 1), *(rng.normal(size=3) * 10 ** rng.uniform(-2, 1)),
+                       10 ** rng.uniform(-3, 1.5)])
+        if kind == 0:
+            Ui[0] = -abs(Ui[0])
+        elif kind == 1:
+            Ui[4] = -abs(Ui[4])
+        elif kind == 2:
+            Ui[4] = 0.9 * math.sqrt(Ui[0] ** 2 + (Ui[1:4] ** 2).sum())
+        if O.admissible(Ui, eps):
+            assert O.limiter_node_s(Ub, Ui, eps) == 1.0
+            continue
+        s = O.limiter_node_s(Ub, Ui, eps)
+        sb = _bisect_s(Ub, Ui, eps)
+        assert 0.0 <= s <= 1.0
+        # same boundary point: compare in terms of where the blended state lands
+        assert abs(s - sb) < 1e-9 * max(sb, 1e-3) + 1e-12, (Ub, Ui, s, sb)
+        ncheck += 1
+    assert ncheck > 1500
+
+
+def test_limiter_node_s_lands_on_q_equals_zero_in_near_vacuum():
+    """R14: the cancellation-free root puts the limiting node on q = 0 to ~eps*E even when node and
+    mean differ by 1e6..1e9 (where Eq. 37 as printed loses digits or goes NaN)."""
+    rng = np.random.default_rng(13)
+    eps = 0.0
+    for _ in range(2000):
+        scale = 10 ** rng.uniform(-9, 0)
+        D = 10 ** rng.uniform(-1, 1)
+        M = rng.normal(size=3)
+        Ub = np.array([D, *M, math.sqrt(D * D + M @ M) * (1 + 10 ** rng.uniform(-3, 0))])
+        Di = D * scale
+        Mi = rng.normal(size=3) * scale * 10 ** rng.uniform(0, 2)
+        Ui = np.array([Di, *Mi, math.sqrt(Di * Di + Mi @ Mi) * rng.uniform(0.2, 0.999)])
+        if rng.random() < 0.5:
+            Ub, Ui = Ub * scale, Ui / scale
+            if _q(Ui) >= 0 or _q(Ub) <= 0:
+                continue
+        s = O.limiter_node_s(Ub, Ui, eps)
+        assert np.isfinite(s) and 0 <= s < 1
+        Us = Ub + s * (Ui - Ub) if s <= 0.5 else Ui + (1 - s) * (Ub - Ui)
+        # s itself is rounded to fp64 (abs. error <= 1.1e-16), which moves the blend by that much
+        # times |Ubar - U_i|; on top of that a few ulp of the landed state
+        assert abs(_q(Us)) < 2e-14 * Us[4] + 4e-16 * (Ub[4] + Ui[4]), (s, _q(Us), Us[4])
+
+
+def _limiter_case(nd, p, eos=O.EOS_IDEAL, G=5 / 3, seed=0):
+    if nd == 1:
+        d, W = I.riemann1d(seed, ne=40, p=p)
+    elif nd == 2:
+        d, W = I.kh2d(seed, nx=8, ny=16, p=p)
+    else:
+        d, W = I.box3d(seed, n=5, p=p, kmax=1)
+    cfg = _cfg(d)
+    U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+    nn = (p + 1) ** nd
+    import torch
+    Ub, cells = I.limiter_stress(torch.from_numpy(U), nn, seed + 100, frac=0.3)
+    return cfg, Ub.numpy(), np.sort(cells.numpy()), nn
+
+
+@pytest.mark.parametrize("nd,p", [(1, 2), (1, 4), (2, 2), (3, 3), (3, 1)])
+def test_enforce_physicality_properties(nd, p):
+    cfg, U, cells, nn = _limiter_case(nd, p)
+    wn = np.tile(_node_weights(nd, p + 1), U.shape[1] // nn)
+    U1, flag, s, (nflag, nbad) = O.enforce_physicality(cfg, U)
+    # exactly the stressed cells are flagged (the clean input is admissible everywhere)
+    assert np.array_equal(np.nonzero(flag)[0], cells) and nflag == len(cells)
+    # cell averages preserved to roundoff
+    mean0 = (U * wn).reshape(5, -1, nn).sum(2)
+    mean1 = (U1 * wn).reshape(5, -1, nn).sum(2)
+    ref = np.abs(U).reshape(5, -1, nn).max(2).max(0) * wn.reshape(-1, nn).sum(1)
+    assert np.all(np.abs(mean1 - mean0) < 4e-15 * ref[None, :] * nn)
+    # every node admissible afterwards (with the screening threshold)
+    ok = np.array([O.admissible(U1[:, j], 0.5 * cfg.eps_q) for j in range(U1.shape[1])])
+    bad_mean_cells = np.nonzero((s == 0.0) & (flag == 1))[0]
+    assert nbad == len(bad_mean_cells)
+    okc = ok.reshape(-1, nn).all(1)
+    assert okc[np.setdiff1d(np.arange(len(okc)), bad_mean_cells)].all()
+    # unflagged cells bit-identical, s = 1 there; 0 <= s < 1 in flagged cells
+    un = np.repeat(flag == 0, nn)
+    assert np.array_equal(U1[:, un], U[:, un]) and np.all(s[flag == 0] == 1.0)
+    assert np.all((s[flag == 1] >= 0) & (s[flag == 1] < 1))
+    # idempotent: second application flags nothing (screen eps_q/2, solve eps_q; R13c)
+    U2, flag2, s2, (nflag2, _) = O.enforce_physicality(cfg, U1)
+    assert nflag2 == nbad          # only cells flattened to an inadmissible mean stay flagged
+    assert np.array_equal(U2[:, np.repeat(flag2 == 0, nn)], U1[:, np.repeat(flag2 == 0, nn)])
+    # the limiting node sits (almost) on the boundary: s is the LARGEST admissible factor.
+    for e in np.nonzero(flag)[0][:20]:
+        if s[e] == 0.0:
+            continue
+        Ubar = mean0[:, e] / wn[:nn].sum()
+        sl = e * nn + np.arange(nn)
+        s_big = min(1.0, s[e] * (1 + 1e-6) / (1 - cfg.delta_s))
+        blended = Ubar[:, None] + s_big * (U[:, sl] - Ubar[:, None])
+        assert not all(O.admissible(blended[:, k], cfg.eps_q) for k in range(nn))
+
+
+def test_enforce_physicality_inadmissible_mean_flattens_cell_and_counts():
+    """R13d: a cell whose average is itself inadmissible cannot be fixed: it is
+    counted and flattened to the mean (s = 0); all other cells are untouched."""
+    d, W = I.riemann1d(2, ne=6, p=2)
+    cfg = _cfg(d)
+    U = O.prim2con_batch(cfg.eos, cfg.gamma_ad, W.numpy())
+    U[0, 3:6] = -1.0                                   # whole cell 1 has D < 0
+    U1, flag, s, (nflag, nbad) = O.enforce_physicality(cfg, U)
+    assert nflag == 1 and nbad == 1 and flag[1] == 1 and s[1] == 0.0
+    _, w, _ = O.gll(3)
+    mean = (U[:, 3:6] * w).sum(1) / 2
+    assert np.allclose(U1[:, 3:6], mean[:, None], rtol=1e-15, atol=0)
+    keep = np.r_[0:3, 6:18]
+    assert np.array_equal(U1[:, keep], U[:, keep])
+
+
+def test_admissible_predicate_uses_plus_sign_and_rejects_nan():
+    """R13a: q = E - sqrt(D^2 + |M|^2) (Eq. 27/31/32), not Eq. 25's printed minus."""
+    assert O.admissible([1.0, 0.5, 0, 0, 1.2]) and not O.admissible([1.0, 0.5, 0, 0, 1.1])
+    assert not O.admissible([1.0, 0, 0, 0, 1.0])                 # q = 0 is not > 0
+    assert not O.admissible([0.0, 0, 0, 0, 1.0])                 # D = 0 is not > 0
+    assert not O.admissible([1.0, float("nan"), 0, 0, 5.0])
+    assert O.admissible([1.0, 0, 0, 0, 1.0 + 1e-9], 1e-12) and not O.admissible([1.0, 0, 0, 0, 1.0 + 1e-13], 1e-12)

@@ -1,0 +1,141 @@
+/* dgrhd.h -- C ABI of the B200-native (sm_100a, fp64) hot path of the discontinuous-Galerkin
+ * special-relativistic-hydrodynamics method of arxiv 2205.00095 ("PAPER.md"): one SSP
+ * Runge-Kutta stage = conserved->primitive recovery at every nodal point, physical flux, element
+ * volume integrals, face states + HLL interface flux + surface lift, SSP-RK combine, the
+ * physicality-enforcing operator, and the CFL wave-speed reduction.
+ *
+ * Conventions (all entry points):
+ *   - units c = 1; fp64 everywhere; NV = 5 variables.
+ *   - conserved  U = [D, Mx, My, Mz, E]                         (PAPER.md:39-43 Eq. 1, :53-56 Eq. 4)
+ *     primitive  W = [rho, ux, uy, uz, P], u = gamma*v the spatial 4-velocity
+ *   - canonical layout, SoA by variable:  X[v][e][n],  v in 0..4,
+ *       e = ix + nx*(iy + ny*iz)  (element),  n = i + N*(j + N*k)  (node in element), N = p+1,
+ *       i.e. element of a 5 x ndof array with ndof = nelem_total * N^ndim, row stride ndof.
+ *     Nodes are tensor-product Gauss-Lobatto-Legendre points (reading R1).
+ *   - every pointer named *_dev is a DEVICE pointer (8-byte aligned at least), every pointer named
+ *     *_host is a HOST pointer.  The caller owns all buffers, including the workspace: the library
+ *     allocates no device memory and frees none.
+ *   - every call returns an int status (DGRHD_OK = 0) and never throws or aborts; argument errors
+ *     are detected before any launch.  Numerical trouble is not an error return: it is counted on
+ *     the device (see dgrhd_get_counters) or reported per state (dgrhd_con2prim_batch).
+ *   - calls enqueue work on the CUDA stream given at create (or in the call) and return without
+ *     waiting, except where a *_host out-parameter is documented to synchronise that stream.
+ *   - there is no CPU fallback: without a CUDA device every compute call returns DGRHD_ECUDA.
+ */
+#ifndef DGRHD_H
+#define DGRHD_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dgrhd_ctx dgrhd_ctx;          /* opaque, owned by the library, freed by destroy */
+
+enum { DGRHD_EOS_IDEAL = 0,                  /* h = 1 + Gamma/(Gamma-1) Theta   (Eq. 8)  */
+       DGRHD_EOS_TAUB_MATTHEWS = 1 };        /* h = 5/2 Theta + 3/2 sqrt(Theta^2+4/9)  (:89 Eq. 10)  */
+enum { DGRHD_BC_PERIODIC = 0,                /* wrap                                                  */
+       DGRHD_BC_OUTFLOW = 1 };               /* transmissive: ghost face state = own face state (:621)*/
+enum { DGRHD_OK = 0, DGRHD_EINVAL = 1, DGRHD_ENOMEM = 2, DGRHD_ECUDA = 3, DGRHD_ESTATE = 4 };
+
+/* Problem statement: mesh, order, EOS. */
+typedef struct {
+  int     ndim;            /* 1, 2 or 3                                                            */
+  int64_t nelem[3];        /* elements per axis (unused axes must be 1)                            */
+  double  xmin[3], xmax[3];/* domain; uniform Cartesian mesh, h_d = (xmax_d - xmin_d)/nelem_d     */
+  int     bc[3];           /* DGRHD_BC_* per axis (both ends of the axis)                          */
+  int     order_p;         /* polynomial order 0..4; N = p+1 nodes per direction                  */
+  int     eos;             /* DGRHD_EOS_*                                                          */
+  double  gamma_ad;        /* adiabatic index Gamma (ideal EOS, > 1); ignored for Taub-Matthews    */
+  int     rk_stages;       /* 1 (RK1), 2 (SSPRK2) or 3 (SSPRK3), Shu-Osher form */
+  double  eps_q, delta_s;  /* safety knobs of the physicality operator (reading R13c);
+                              0,0 = the paper verbatim; defaults used by the tests: 1e-12, 1e-10   */
+} dgrhd_config;
+
+/* Bytes of device workspace dgrhd_create needs for this configuration (0 if cfg is invalid). */
+size_t dgrhd_workspace_bytes(const dgrhd_config* cfg);
+
+/* Create a context.  workspace_dev: device buffer of at least dgrhd_workspace_bytes(cfg) bytes,
+ * 256-byte aligned, owned by the caller and kept alive until dgrhd_destroy.  cuda_stream: a
+ * cudaStream_t (NULL = the legacy default stream) on which every call of this context enqueues.
+ * Errors: EINVAL (bad config / NULL / misaligned), ENOMEM (workspace too small), ECUDA. */
+int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t workspace_bytes,
+                 void* cuda_stream, dgrhd_ctx** out);
+int dgrhd_destroy(dgrhd_ctx* ctx);
+
+/* Copy the caller's conserved state U_dev[5][ndof] (canonical layout) into / out of the context.
+ * set_state also recovers the primitives of every node (Eq. 16) and computes the
+ * CFL wave-speed maximum of the new state; it does not apply the physicality operator (R15). */
+int dgrhd_set_state(dgrhd_ctx* ctx, const double* U_dev);
+int dgrhd_get_state(dgrhd_ctx* ctx, double* U_dev);
+/* Primitives W[5][ndof] of the internal state (as recovered by the last stage / set_state). */
+int dgrhd_get_prims(dgrhd_ctx* ctx, double* W_dev);
+
+/* R = L(U): the DG spatial operator, Eq. 15-18, on caller buffers in the canonical
+ * layout: nodal con2prim (Eq. 16), flux (Eq. 2), volume quadrature (Eq. 17), face states and HLL
+ * interface flux with lambda_L/R of Eq. 21-24, surface lift (Eq. 18).  Does not touch the internal
+ * state.  U_dev and R_dev must not overlap. */
+int dgrhd_rhs(dgrhd_ctx* ctx, const double* U_dev, double* R_dev);
+
+/* The physicality-enforcing operator of PAPER.md:175-254 (Eq. 25-37), in place on U_dev[5][ndof]
+ * (NULL = the internal state, whose primitives are then refreshed): per cell, blend toward the
+ * volume average with the largest s in [0,1] that makes every node admissible (D > 0,
+ * E > sqrt(D^2+|M|^2)).  flag_dev[n_elem] (or NULL) receives 1 for cells where it acted, 0
+ * otherwise; s_dev[n_elem] (or NULL) the blend factor (1 where it did not act, 0 where the cell
+ * average itself is inadmissible).  counters_host[2] (or NULL) receives {n_flagged, n_bad_mean} of
+ * this call and makes the call synchronise the stream. */
+int dgrhd_enforce_physicality(dgrhd_ctx* ctx, double* U_dev, unsigned char* flag_dev,
+                              double* s_dev, int64_t counters_host[2]);
+
+/* CFL time step (formula: DESIGN.md reading R11):
+ *   dt = cfl / max_nodes sum_d (2p+1) max(|lambda-_d|, |lambda+_d|) / h_d,  lambda+- of Eq. 21-22.
+ * U_dev = NULL uses the internal state.  Synchronises; *dt_host receives dt. */
+int dgrhd_cfl_dt(dgrhd_ctx* ctx, const double* U_dev, double cfl, double* dt_host);
+
+/* Advance the internal state by nsteps SSP-RK steps; each stage is
+ *   U <- a U0 + b (U_s + dt L(U_s)), then the physicality operator (R15), then con2prim of the new
+ * state; the last stage also reduces the CFL maximum for the next step.
+ * dt > 0: fixed step.  dt <= 0: CFL number = -dt, the step is recomputed on the device every step
+ * from the state at the start of the step (no host round trip).
+ * t_inout_host (or NULL): *t += sum of the steps taken; non-NULL makes the call synchronise. */
+int dgrhd_step(dgrhd_ctx* ctx, double dt, int nsteps, double* t_inout_host);
+
+/* Device counters accumulated since create / the last reset (synchronises):
+ *   out_host[0] n_flagged   cell-activations of the physicality operator inside dgrhd_step
+ *   out_host[1] n_bad_mean  cells whose average was itself inadmissible (flattened)
+ *   out_host[2] n_c2p_fail  nodes where con2prim failed (inadmissible input or P <= 0)
+ *   out_host[3] n_stages    RK stages executed by dgrhd_step
+ * reset != 0 zeroes them afterwards. */
+int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[4], int reset);
+
+/* Conserved -> primitive recovery of a flat SoA batch U_dev[5][n] -> W_dev[5][n]:
+ * ideal EOS by Newton iteration on the quartic of Eq. 59 (beta = 2w/(1+w^2), Eq. 58; small-xi
+ * series Eq. 60; finishing Eq. 55-57); Taub-Matthews by the analytic cubic Eq. 61-75.
+ * status_dev[n] (or NULL): 0 ok; 1 input not admissible by Eq. 25 (outputs NaN); 2 recovered
+ * pressure not positive / non-finite.  Enqueues on cuda_stream; does not synchronise.  n = 0 ok. */
+int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const double* U_dev, double* W_dev,
+                         int* status_dev, void* cuda_stream);
+
+/* Primitive -> conserved, Eq. 4, flat SoA batch W_dev[5][n] -> U_dev[5][n]. */
+int dgrhd_prim2con_batch(int eos, double gamma_ad, int64_t n, const double* W_dev, double* U_dev,
+                         void* cuda_stream);
+
+/* Host-buffer convenience wrapper around dgrhd_con2prim_batch: copies U_host[5][n] to the device
+ * (chunked, through the caller's staging buffer stage_dev of stage_bytes >= 80 bytes per state of
+ * one chunk), runs the kernel, copies W_host[5][n] back, synchronises.  Used for end-to-end timing. */
+int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, const double* U_host,
+                              double* W_host, void* stage_dev, size_t stage_bytes,
+                              void* cuda_stream);
+
+/* Text of the last error of this context (ctx = NULL: of the last context-free call on this
+ * thread).  Never NULL; valid until the next call on the same context / thread. */
+const char* dgrhd_last_error(const dgrhd_ctx* ctx);
+
+/* Library version string, e.g. "dgrhd 0.1 (sm_100a)". */
+const char* dgrhd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DGRHD_H */

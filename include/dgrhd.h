@@ -128,6 +128,12 @@ int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, const double*
                               double* W_host, void* stage_dev, size_t stage_bytes,
                               void* cuda_stream);
 
+/* End-to-end wrapper with HOST buffers (pinned memory for full copy speed): copies
+ * U_host_in[5][ndof] to the device, dgrhd_set_state, dgrhd_step(dt, nsteps), copies the new state
+ * to U_host_out[5][ndof], synchronises.  *t_inout_host (or NULL) += elapsed time. */
+int dgrhd_run_host(dgrhd_ctx* ctx, const double* U_host_in, double* U_host_out, double dt,
+                   int nsteps, double* t_inout_host);
+
 /* Text of the last error of this context (ctx = NULL: of the last context-free call on this
  * thread).  Never NULL; valid until the next call on the same context / thread. */
 const char* dgrhd_last_error(const dgrhd_ctx* ctx);

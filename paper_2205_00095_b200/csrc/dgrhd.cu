@@ -1,0 +1,507 @@
+// dgrhd.cu -- host side of the C ABI declared in include/dgrhd.h: argument checks, the context
+// (operator tables, buffer carving inside the caller's workspace, device scalars), kernel
+// dispatch and the step orchestration.  No device memory is allocated here; every launch goes to
+// the caller's stream; there is no CPU fallback (every compute call needs a CUDA device).
+#include "../../include/dgrhd.h"
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "basis.h"
+#include "flat_kernels.cuh"
+
+// launchers of the fused stage kernel, one translation unit per (ndim, EOS): stage_inst.cu
+#define DG_DECL(nd, eos) cudaError_t dg_launch_stage_##nd##_##eos(int N, const StageArgs& a, cudaStream_t st);
+DG_DECL(1, 0) DG_DECL(1, 1) DG_DECL(2, 0) DG_DECL(2, 1) DG_DECL(3, 0) DG_DECL(3, 1)
+#undef DG_DECL
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+void set_err(char* dst, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+}
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+// device scalars at the head of the workspace
+struct DevScalars {
+  double dt;          // time step of the step in flight
+  double t_acc;       // sum of the steps taken by the current dgrhd_step call
+  dg_ull amax;        // ordered-int image of the CFL maximum of the internal state
+  dg_ull amax_tmp;    // same, for dgrhd_cfl_dt on a caller state
+  dg_ull counters[4]; // n_flagged, n_bad_mean, n_c2p_fail, n_stages
+  dg_ull call_cnt[2]; // per-call counters of dgrhd_enforce_physicality
+  double wnode[125];  // tensor GLL weights, node order
+};
+
+bool valid_cfg(const dgrhd_config* c) {
+  if (!c) return false;
+  if (c->ndim < 1 || c->ndim > 3) return false;
+  for (int d = 0; d < 3; ++d) {
+    if (c->nelem[d] < 1 || c->nelem[d] > 2147483647LL) return false;
+    if (d >= c->ndim && c->nelem[d] != 1) return false;
+    if (d < c->ndim && !(c->xmax[d] > c->xmin[d])) return false;
+    if (d < c->ndim && c->bc[d] != DGRHD_BC_PERIODIC && c->bc[d] != DGRHD_BC_OUTFLOW) return false;
+  }
+  if (c->order_p < 0 || c->order_p > 4) return false;
+  if (c->eos != DGRHD_EOS_IDEAL && c->eos != DGRHD_EOS_TAUB_MATTHEWS) return false;
+  if (c->eos == DGRHD_EOS_IDEAL && !(c->gamma_ad > 1.0)) return false;
+  if (c->rk_stages < 1 || c->rk_stages > 3) return false;
+  if (!(c->eps_q >= 0.0 && c->eps_q < 0.5) || !(c->delta_s >= 0.0 && c->delta_s < 0.5)) return false;
+  return true;
+}
+
+int ipow(int b, int e) { int r = 1; while (e-- > 0) r *= b; return r; }
+
+EosPar make_eos(int eos, double G) {
+  EosPar e;
+  e.G = G;
+  e.al = (eos == DGRHD_EOS_IDEAL) ? G / (G - 1.0) : 0.0;
+  return e;
+}
+
+}  // namespace
+
+struct dgrhd_ctx {
+  dgrhd_config cfg;
+  int N, NN;
+  long long nelem, ndof;
+  size_t state_bytes;
+  cudaStream_t stream;
+  DevScalars* sc;
+  double *Ua, *Ub, *W[2];
+  int wcur;                 // W[wcur] holds the primitives of the internal state Ua
+  bool has_state;
+  BasisTables basis;
+  double wsum;
+  EosPar eos;
+  char err[512];
+};
+
+static int fail(dgrhd_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) snprintf(c->err, sizeof c->err, "%s", buf);
+  snprintf(g_err, sizeof g_err, "%s", buf);
+  return code;
+}
+
+static int cuda_fail(dgrhd_ctx* c, cudaError_t e, const char* where) {
+  return fail(c, DGRHD_ECUDA, "%s: %s", where, cudaGetErrorString(e));
+}
+
+#define DG_CUDA(c, call)                                  \
+  do {                                                    \
+    cudaError_t e__ = (call);                             \
+    if (e__ != cudaSuccess) return cuda_fail(c, e__, #call); \
+  } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// kernel dispatch helpers
+// ------------------------------------------------------------------------------------------------
+static cudaError_t launch_stage(dgrhd_ctx* c, const StageArgs& a) {
+  const int key = c->cfg.ndim * 2 + c->cfg.eos;
+  switch (key) {
+    case 2: return dg_launch_stage_1_0(c->N, a, c->stream);
+    case 3: return dg_launch_stage_1_1(c->N, a, c->stream);
+    case 4: return dg_launch_stage_2_0(c->N, a, c->stream);
+    case 5: return dg_launch_stage_2_1(c->N, a, c->stream);
+    case 6: return dg_launch_stage_3_0(c->N, a, c->stream);
+    case 7: return dg_launch_stage_3_1(c->N, a, c->stream);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// W = p(U) over a state (+ failure count, + CFL maximum when amax != NULL)
+static cudaError_t launch_c2p_state(dgrhd_ctx* c, const double* U, double* W, dg_ull* amax,
+                                    dg_ull* counters) {
+  const long long n = c->ndof;
+  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
+  double cw[3] = {0, 0, 0};
+  for (int d = 0; d < c->cfg.ndim; ++d)
+    cw[d] = (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]);
+#define DG_GO(E, D) \
+  dg_c2p_state_kernel<E, D><<<nb, DG_FLAT_NT, 0, c->stream>>>(n, U, W, c->eos, cw[0], cw[1], cw[2], amax, counters)
+  if (c->cfg.eos == DGRHD_EOS_IDEAL) {
+    if (c->cfg.ndim == 1) DG_GO(0, 1); else if (c->cfg.ndim == 2) DG_GO(0, 2); else DG_GO(0, 3);
+  } else {
+    if (c->cfg.ndim == 1) DG_GO(1, 1); else if (c->cfg.ndim == 2) DG_GO(1, 2); else DG_GO(1, 3);
+  }
+#undef DG_GO
+  return cudaGetLastError();
+}
+
+template <int ND>
+static cudaError_t launch_limiter_nd(dgrhd_ctx* c, double* U, unsigned char* flag, double* s,
+                                     dg_ull* counters) {
+  const double fs = 1.0 - 0.5 * c->cfg.eps_q, fv = 1.0 - c->cfg.eps_q, od = 1.0 - c->cfg.delta_s;
+#define DG_GO(NV)                                                                                   \
+  {                                                                                                 \
+    using LS = LimShape<dg_ipow(NV, ND)>;                                                           \
+    const unsigned nb = (unsigned)((c->nelem + LS::NE - 1) / LS::NE);                               \
+    dg_limiter_kernel<ND, NV><<<nb, LS::NT, 0, c->stream>>>(c->nelem, c->ndof, U, flag, s,          \
+                                                            c->sc->wnode, c->wsum, fs, fv, od,      \
+                                                            counters);                              \
+  }
+  switch (c->N) {
+    case 1: DG_GO(1) break;
+    case 2: DG_GO(2) break;
+    case 3: DG_GO(3) break;
+    case 4: DG_GO(4) break;
+    case 5: DG_GO(5) break;
+  }
+#undef DG_GO
+  return cudaGetLastError();
+}
+
+static cudaError_t launch_limiter(dgrhd_ctx* c, double* U, unsigned char* flag, double* s,
+                                  dg_ull* counters) {
+  if (c->cfg.ndim == 1) return launch_limiter_nd<1>(c, U, flag, s, counters);
+  if (c->cfg.ndim == 2) return launch_limiter_nd<2>(c, U, flag, s, counters);
+  return launch_limiter_nd<3>(c, U, flag, s, counters);
+}
+
+static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
+  memset(&a, 0, sizeof a);
+  a.ndof = c->ndof;
+  for (int d = 0; d < 3; ++d) {
+    a.ne[d] = (int)c->cfg.nelem[d];
+    a.bc[d] = c->cfg.bc[d];
+    if (d < c->cfg.ndim) {
+      const double h = (c->cfg.xmax[d] - c->cfg.xmin[d]) / (double)c->cfg.nelem[d];
+      a.rh[d] = 2.0 / h;
+      a.cw[d] = (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]);
+    }
+  }
+  a.f_screen = 1.0 - 0.5 * c->cfg.eps_q;
+  a.f_solve = 1.0 - c->cfg.eps_q;
+  a.one_m_delta = 1.0 - c->cfg.delta_s;
+  a.eos = c->eos;
+  a.dt_ptr = &c->sc->dt;
+  a.amax = &c->sc->amax;
+  a.counters = c->sc->counters;
+  for (int i = 0; i < c->N; ++i) {
+    a.w[i] = c->basis.w[i];
+    for (int q = 0; q < c->N; ++q) a.Dhat[i * c->N + q] = c->basis.Dhat[i][q];
+  }
+  a.lift = c->basis.lift;
+  a.wsum = c->wsum;
+}
+
+// ------------------------------------------------------------------------------------------------
+// create / destroy
+// ------------------------------------------------------------------------------------------------
+extern "C" size_t dgrhd_workspace_bytes(const dgrhd_config* cfg) {
+  if (!valid_cfg(cfg)) return 0;
+  long long ne = 1;
+  for (int d = 0; d < cfg->ndim; ++d) ne *= cfg->nelem[d];
+  const long long ndof = ne * ipow(cfg->order_p + 1, cfg->ndim);
+  const size_t sb = align_up((size_t)ndof * 5 * sizeof(double));
+  return align_up(sizeof(DevScalars)) + 4 * sb;
+}
+
+extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t workspace_bytes,
+                            void* cuda_stream, dgrhd_ctx** out) {
+  if (out) *out = nullptr;
+  if (!out || !valid_cfg(cfg)) return fail(nullptr, DGRHD_EINVAL, "dgrhd_create: invalid configuration");
+  if (!workspace_dev || ((uintptr_t)workspace_dev % ALIGN) != 0)
+    return fail(nullptr, DGRHD_EINVAL, "dgrhd_create: workspace NULL or not 256-byte aligned");
+  const size_t need = dgrhd_workspace_bytes(cfg);
+  if (workspace_bytes < need)
+    return fail(nullptr, DGRHD_ENOMEM, "dgrhd_create: workspace %zu < %zu bytes", workspace_bytes, need);
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(nullptr, DGRHD_ECUDA, "dgrhd_create: no CUDA device (there is no CPU fallback)");
+  dgrhd_ctx* c = new (std::nothrow) dgrhd_ctx;
+  if (!c) return fail(nullptr, DGRHD_ENOMEM, "dgrhd_create: host allocation failed");
+  memset(c, 0, sizeof *c);
+  c->cfg = *cfg;
+  c->N = cfg->order_p + 1;
+  c->NN = ipow(c->N, cfg->ndim);
+  c->nelem = 1;
+  for (int d = 0; d < cfg->ndim; ++d) c->nelem *= cfg->nelem[d];
+  c->ndof = c->nelem * c->NN;
+  c->state_bytes = (size_t)c->ndof * 5 * sizeof(double);
+  c->stream = (cudaStream_t)cuda_stream;
+  c->eos = make_eos(cfg->eos, cfg->gamma_ad);
+  dgbasis::build(c->N, c->basis);
+  char* p = (char*)workspace_dev;
+  c->sc = (DevScalars*)p;  p += align_up(sizeof(DevScalars));
+  const size_t sb = align_up(c->state_bytes);
+  c->Ua = (double*)p;  p += sb;
+  c->Ub = (double*)p;  p += sb;
+  c->W[0] = (double*)p;  p += sb;
+  c->W[1] = (double*)p;
+  // tensor weights in node order and their sum (summed in node order)
+  DevScalars h;
+  memset(&h, 0, sizeof h);
+  c->wsum = 0.0;
+  for (int n = 0; n < c->NN; ++n) {
+    double w = c->basis.w[n % c->N];
+    if (cfg->ndim > 1) w *= c->basis.w[(n / c->N) % c->N];
+    if (cfg->ndim > 2) w *= c->basis.w[n / (c->N * c->N)];
+    h.wnode[n] = w;
+    c->wsum += w;
+  }
+  cudaError_t e = cudaMemcpyAsync(c->sc, &h, sizeof h, cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) {
+    int r = cuda_fail(nullptr, e, "dgrhd_create");
+    delete c;
+    return r;
+  }
+  *out = c;
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_destroy(dgrhd_ctx* ctx) {
+  if (!ctx) return DGRHD_EINVAL;
+  delete ctx;
+  return DGRHD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// state access
+// ------------------------------------------------------------------------------------------------
+extern "C" int dgrhd_set_state(dgrhd_ctx* c, const double* U_dev) {
+  if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_set_state: NULL argument");
+  DG_CUDA(c, cudaMemcpyAsync(c->Ua, U_dev, c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  DG_CUDA(c, cudaMemsetAsync(&c->sc->amax, 0, sizeof(dg_ull), c->stream));
+  c->wcur = 0;
+  DG_CUDA(c, launch_c2p_state(c, c->Ua, c->W[0], &c->sc->amax, c->sc->counters));
+  c->has_state = true;
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_get_state(dgrhd_ctx* c, double* U_dev) {
+  if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_get_state: NULL argument");
+  if (!c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_get_state: no state set");
+  DG_CUDA(c, cudaMemcpyAsync(U_dev, c->Ua, c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_get_prims(dgrhd_ctx* c, double* W_dev) {
+  if (!c || !W_dev) return fail(c, DGRHD_EINVAL, "dgrhd_get_prims: NULL argument");
+  if (!c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_get_prims: no state set");
+  DG_CUDA(c, cudaMemcpyAsync(W_dev, c->W[c->wcur], c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  return DGRHD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// R = L(U) on caller buffers: nodal con2prim into the spare primitive buffer, then the fused
+// kernel in MODE_RHS
+// ------------------------------------------------------------------------------------------------
+extern "C" int dgrhd_rhs(dgrhd_ctx* c, const double* U_dev, double* R_dev) {
+  if (!c || !U_dev || !R_dev) return fail(c, DGRHD_EINVAL, "dgrhd_rhs: NULL argument");
+  if (U_dev == R_dev) return fail(c, DGRHD_EINVAL, "dgrhd_rhs: U_dev and R_dev overlap");
+  double* Wtmp = c->W[c->wcur ^ 1];
+  DG_CUDA(c, launch_c2p_state(c, U_dev, Wtmp, nullptr, c->sc->counters));
+  StageArgs a;
+  fill_stage_args(c, a);
+  a.mode = DG_MODE_RHS;
+  a.Win = Wtmp;
+  a.Us = U_dev;
+  a.Rout = R_dev;
+  DG_CUDA(c, launch_stage(c, a));
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_enforce_physicality(dgrhd_ctx* c, double* U_dev, unsigned char* flag_dev,
+                                         double* s_dev, int64_t counters_host[2]) {
+  if (!c) return fail(c, DGRHD_EINVAL, "dgrhd_enforce_physicality: NULL context");
+  const bool internal = (U_dev == nullptr);
+  if (internal && !c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_enforce_physicality: no state set");
+  double* U = internal ? c->Ua : U_dev;
+  DG_CUDA(c, cudaMemsetAsync(c->sc->call_cnt, 0, 2 * sizeof(dg_ull), c->stream));
+  DG_CUDA(c, launch_limiter(c, U, flag_dev, s_dev, c->sc->call_cnt));
+  if (internal) {                       // refresh the primitives and the CFL maximum of the state
+    DG_CUDA(c, cudaMemsetAsync(&c->sc->amax, 0, sizeof(dg_ull), c->stream));
+    DG_CUDA(c, launch_c2p_state(c, c->Ua, c->W[c->wcur], &c->sc->amax, c->sc->counters));
+  }
+  if (counters_host) {
+    dg_ull h[2];
+    DG_CUDA(c, cudaMemcpyAsync(h, c->sc->call_cnt, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    DG_CUDA(c, cudaStreamSynchronize(c->stream));
+    counters_host[0] = (int64_t)h[0];
+    counters_host[1] = (int64_t)h[1];
+  }
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_cfl_dt(dgrhd_ctx* c, const double* U_dev, double cfl, double* dt_host) {
+  if (!c || !dt_host) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: NULL argument");
+  if (!(cfl > 0.0)) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: cfl must be > 0");
+  dg_ull* slot = &c->sc->amax;
+  if (U_dev) {
+    slot = &c->sc->amax_tmp;
+    DG_CUDA(c, cudaMemsetAsync(slot, 0, sizeof(dg_ull), c->stream));
+    DG_CUDA(c, launch_c2p_state(c, U_dev, nullptr, slot, nullptr));
+  } else if (!c->has_state) {
+    return fail(c, DGRHD_ESTATE, "dgrhd_cfl_dt: no state set");
+  }
+  dg_ull h = 0;
+  DG_CUDA(c, cudaMemcpyAsync(&h, slot, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  DG_CUDA(c, cudaStreamSynchronize(c->stream));
+  double m;
+  memcpy(&m, &h, sizeof m);
+  *dt_host = cfl / m;
+  return DGRHD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// SSP-RK steps (Shu-Osher form, reading R10): per step one dt kernel + one fused kernel per stage,
+// all on the context's stream, dt and the CFL maximum resident on the device.
+//   buffers: Ua = U at the start of the step (and the state between calls), Ub = stage state,
+//   W[wcur] = primitives of the stage input, W[wcur^1] = primitives of the stage output.
+// ------------------------------------------------------------------------------------------------
+static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
+  const int S = c->cfg.rk_stages;
+  static const double A3[3] = {0.0, 0.75, 1.0 / 3.0}, B3[3] = {1.0, 0.25, 2.0 / 3.0};
+  static const double A2[2] = {0.0, 0.5}, B2[2] = {1.0, 0.5};
+  dg_dt_kernel<<<1, 1, 0, c->stream>>>(dt, -dt, &c->sc->amax, &c->sc->dt, &c->sc->t_acc,
+                                       &c->sc->counters[3], S);
+  DG_CUDA(c, cudaGetLastError());
+  for (int s = 0; s < S; ++s) {
+    const bool last = (s == S - 1);
+    a.a = (S == 2) ? A2[s] : A3[s];
+    a.b = (S == 2) ? B2[s] : B3[s];
+    a.Win = c->W[c->wcur];
+    a.Wout = c->W[c->wcur ^ 1];
+    a.Us = (s == 0) ? c->Ua : c->Ub;
+    a.U0 = c->Ua;
+    a.Uout = last ? c->Ua : c->Ub;
+    a.do_cfl = last ? 1 : 0;
+    DG_CUDA(c, launch_stage(c, a));
+    c->wcur ^= 1;
+  }
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_step(dgrhd_ctx* c, double dt, int nsteps, double* t_inout_host) {
+  if (!c) return fail(c, DGRHD_EINVAL, "dgrhd_step: NULL context");
+  if (nsteps < 0 || !(dt == dt)) return fail(c, DGRHD_EINVAL, "dgrhd_step: bad nsteps or dt");
+  if (dt == 0.0) return fail(c, DGRHD_EINVAL, "dgrhd_step: dt must be > 0 (fixed) or < 0 (-CFL)");
+  if (!c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_step: no state set");
+  DG_CUDA(c, cudaMemsetAsync(&c->sc->t_acc, 0, sizeof(double), c->stream));
+  StageArgs a;
+  fill_stage_args(c, a);
+  a.mode = DG_MODE_STAGE;
+  for (int i = 0; i < nsteps; ++i) {
+    int r = enqueue_step(c, dt, a);
+    if (r != DGRHD_OK) return r;
+  }
+  if (t_inout_host) {
+    double h = 0.0;
+    DG_CUDA(c, cudaMemcpyAsync(&h, &c->sc->t_acc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+    DG_CUDA(c, cudaStreamSynchronize(c->stream));
+    *t_inout_host += h;
+  }
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_run_host(dgrhd_ctx* c, const double* U_host_in, double* U_host_out, double dt,
+                              int nsteps, double* t_inout_host) {
+  if (!c || !U_host_in || !U_host_out) return fail(c, DGRHD_EINVAL, "dgrhd_run_host: NULL argument");
+  DG_CUDA(c, cudaMemcpyAsync(c->Ub, U_host_in, c->state_bytes, cudaMemcpyHostToDevice, c->stream));
+  int r = dgrhd_set_state(c, c->Ub);
+  if (r != DGRHD_OK) return r;
+  r = dgrhd_step(c, dt, nsteps, nullptr);
+  if (r != DGRHD_OK) return r;
+  DG_CUDA(c, cudaMemcpyAsync(U_host_out, c->Ua, c->state_bytes, cudaMemcpyDeviceToHost, c->stream));
+  double h = 0.0;
+  DG_CUDA(c, cudaMemcpyAsync(&h, &c->sc->t_acc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  DG_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (t_inout_host) *t_inout_host += h;
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[4], int reset) {
+  if (!c || !out_host) return fail(c, DGRHD_EINVAL, "dgrhd_get_counters: NULL argument");
+  dg_ull h[4];
+  DG_CUDA(c, cudaMemcpyAsync(h, c->sc->counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  if (reset) DG_CUDA(c, cudaMemsetAsync(c->sc->counters, 0, sizeof h, c->stream));
+  DG_CUDA(c, cudaStreamSynchronize(c->stream));
+  for (int i = 0; i < 4; ++i) out_host[i] = (int64_t)h[i];
+  return DGRHD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// context-free batch calls
+// ------------------------------------------------------------------------------------------------
+static int check_batch(const char* who, int eos, double G, int64_t n, const void* a, const void* b) {
+  if (eos != DGRHD_EOS_IDEAL && eos != DGRHD_EOS_TAUB_MATTHEWS)
+    return fail(nullptr, DGRHD_EINVAL, "%s: unknown EOS %d", who, eos);
+  if (eos == DGRHD_EOS_IDEAL && !(G > 1.0)) return fail(nullptr, DGRHD_EINVAL, "%s: Gamma must be > 1", who);
+  if (n < 0 || n > (int64_t)2147483647 * DG_FLAT_NT) return fail(nullptr, DGRHD_EINVAL, "%s: bad n", who);
+  if (n > 0 && (!a || !b)) return fail(nullptr, DGRHD_EINVAL, "%s: NULL buffer", who);
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const double* U_dev,
+                                    double* W_dev, int* status_dev, void* cuda_stream) {
+  int r = check_batch("dgrhd_con2prim_batch", eos, gamma_ad, n, U_dev, W_dev);
+  if (r != DGRHD_OK || n == 0) return r;
+  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
+  const EosPar e = make_eos(eos, gamma_ad);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (eos == DGRHD_EOS_IDEAL)
+    dg_c2p_batch_kernel<0><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+  else
+    dg_c2p_batch_kernel<1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+  DG_CUDA(nullptr, cudaGetLastError());
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_prim2con_batch(int eos, double gamma_ad, int64_t n, const double* W_dev,
+                                    double* U_dev, void* cuda_stream) {
+  int r = check_batch("dgrhd_prim2con_batch", eos, gamma_ad, n, W_dev, U_dev);
+  if (r != DGRHD_OK || n == 0) return r;
+  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
+  const EosPar e = make_eos(eos, gamma_ad);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (eos == DGRHD_EOS_IDEAL)
+    dg_p2c_batch_kernel<0><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, W_dev, U_dev, e);
+  else
+    dg_p2c_batch_kernel<1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, W_dev, U_dev, e);
+  DG_CUDA(nullptr, cudaGetLastError());
+  return DGRHD_OK;
+}
+
+// Host-buffer wrapper: chunks of m states go through the staging buffer as [U: 5 x m][W: 5 x m].
+extern "C" int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, const double* U_host,
+                                         double* W_host, void* stage_dev, size_t stage_bytes,
+                                         void* cuda_stream) {
+  int r = check_batch("dgrhd_con2prim_batch_host", eos, gamma_ad, n, U_host, W_host);
+  if (r != DGRHD_OK || n == 0) return r;
+  if (!stage_dev || stage_bytes < 80) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_host: staging buffer too small");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int64_t cap = (int64_t)(stage_bytes / 80);
+  double* Ud = (double*)stage_dev;
+  for (int64_t s = 0; s < n; s += cap) {
+    const int64_t m = (n - s < cap) ? (n - s) : cap;
+    double* Wd = Ud + 5 * m;
+    DG_CUDA(nullptr, cudaMemcpy2DAsync(Ud, m * sizeof(double), U_host + s, n * sizeof(double),
+                                       m * sizeof(double), 5, cudaMemcpyHostToDevice, st));
+    r = dgrhd_con2prim_batch(eos, gamma_ad, m, Ud, Wd, nullptr, cuda_stream);
+    if (r != DGRHD_OK) return r;
+    DG_CUDA(nullptr, cudaMemcpy2DAsync(W_host + s, n * sizeof(double), Wd, m * sizeof(double),
+                                       m * sizeof(double), 5, cudaMemcpyDeviceToHost, st));
+  }
+  DG_CUDA(nullptr, cudaStreamSynchronize(st));
+  return DGRHD_OK;
+}
+
+extern "C" const char* dgrhd_last_error(const dgrhd_ctx* c) { return c ? c->err : g_err; }
+
+extern "C" const char* dgrhd_version(void) { return "dgrhd 0.1 (sm_100a)"; }

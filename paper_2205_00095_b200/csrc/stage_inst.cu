@@ -1,0 +1,41 @@
+// stage_inst.cu -- instantiations of the fused stage kernel for one (ndim, EOS) pair and every
+// order p = 0..4; compiled once per pair (-DDG_INST_ND=1|2|3 -DDG_INST_EOS=0|1) so that the
+// translation units build in parallel.  Exports one launcher, declared in dgrhd.cu.
+#include "stage_kernel.cuh"
+
+#ifndef DG_INST_ND
+#error "compile with -DDG_INST_ND=... -DDG_INST_EOS=..."
+#endif
+
+#define DG_CAT_(a, b, c) a##b##_##c
+#define DG_CAT(a, b, c) DG_CAT_(a, b, c)
+#define DG_LAUNCH_NAME DG_CAT(dg_launch_stage_, DG_INST_ND, DG_INST_EOS)
+
+template <int N>
+static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
+  using TS = TileShape<DG_INST_ND, N>;
+  auto k = dg_stage_kernel<DG_INST_ND, N, DG_INST_EOS>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, TS::SMEM_BYTES);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  const long long ntx = (a.ne[0] + TS::TX - 1) / TS::TX, nty = (a.ne[1] + TS::TY - 1) / TS::TY,
+                  ntz = (a.ne[2] + TS::TZ - 1) / TS::TZ;
+  const long long nb = ntx * nty * ntz;
+  if (nb <= 0 || nb > 2147483647LL) return cudaErrorInvalidConfiguration;
+  k<<<(unsigned)nb, TS::NT, TS::SMEM_BYTES, st>>>(a);
+  return cudaGetLastError();
+}
+
+cudaError_t DG_LAUNCH_NAME(int N, const StageArgs& a, cudaStream_t st) {
+  switch (N) {
+    case 1: return launch_n<1>(a, st);
+    case 2: return launch_n<2>(a, st);
+    case 3: return launch_n<3>(a, st);
+    case 4: return launch_n<4>(a, st);
+    case 5: return launch_n<5>(a, st);
+  }
+  return cudaErrorInvalidValue;
+}

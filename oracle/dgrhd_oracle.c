@@ -252,6 +252,17 @@ static int con2prim_tm(const double U[5], double Wp[5]) {
     Wv = -c1 / 3.0 + cbrt(R + sd) + cbrt(R - sd);             /* Eq. 71-73, real cube roots */
   }
   if (Wv < 0.0) Wv = 0.0;                                     /* R7 */
+  /* R7b: one Newton correction of the root on the cubic of Eq. 61 itself.  The closed forms above
+   * return W as a difference of O(c1) terms, i.e. with an ABSOLUTE error ~1e-16 c1, which is a
+   * large relative error when W = gamma^2-1 -> 0; f(W) = ((W+c1)W+c2)W+c3 has no such cancellation
+   * near the (simple, only positive) root, so one step restores full relative accuracy. */
+  {
+    double f = ((Wv + c1) * Wv + c2) * Wv + c3;
+    double df = (3.0 * Wv + 2.0 * c1) * Wv + c2;
+    double Wn = Wv - f / df;
+    if (isfinite(Wn)) Wv = Wn;
+    if (Wv < 0.0) Wv = 0.0;
+  }
   double g = sqrt(Wv + 1.0);                                  /* Eq. 74 */
   double beta = sqrt(Wv / (Wv + 1.0));
   double rho = D / g;

@@ -208,7 +208,8 @@ DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
 
 // Taub-Matthews: cubic in Wv = gamma^2 - 1 with c1..c3 of Eq. 62-64, Q, R, d of
 // Eq. 65-67, trigonometric branch Eq. 69-70 (d < 0) or Cardano Eq. 71-73 (d >= 0), then Eq. 74-75.
-// Safeguards of reading R7: eta^2-xi^2 = (eta-xi)(eta+xi), acos argument clamped, Wv >= 0.
+// Safeguards of reading R7: eta^2-xi^2 = (eta-xi)(eta+xi), acos argument clamped, Wv >= 0; R7b: one
+// Newton correction of the root on the cubic itself (full relative accuracy as gamma -> 1).
 DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
   const double D = U[0], E = U[4];
   const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
@@ -237,6 +238,13 @@ DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
     Wv = cbrt(R + sd) + cbrt(R - sd) - c1 * (1.0 / 3.0);         // Eq. 71-73
   }
   Wv = fmax(Wv, 0.0);
+  {                                                              // R7b: one Newton step on Eq. 61
+    const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
+    const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
+    const double Wn = Wv - f / df;
+    if (isfinite(Wn)) Wv = Wn;
+    Wv = fmax(Wv, 0.0);
+  }
   const double g2 = Wv + 1.0;
   const double rg = rsqrt(g2);                                   // 1/gamma, Eq. 74
   const double ug = sqrt(Wv);                                    // gamma beta

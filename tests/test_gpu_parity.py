@@ -145,8 +145,13 @@ def test_con2prim_edge_cases(eos, G):
     Wg = b.dgrhd_con2prim_batch(eos, G, to_dev(U), status=st).cpu().numpy()
     assert np.array_equal(st.cpu().numpy(), sto) and list(sto) == [0, 0, 0, 1, 1, 1]
     assert np.isnan(Wg[:, 3:]).all()
-    # TM at |M| -> 0: W = gamma^2 - 1 is a difference of O(1) terms (abs. error ~1e-16, R6)
-    np.testing.assert_allclose(Wg[:, :3], Wo[:, :3], rtol=1e-10, atol=1e-13 if eos else 1e-18)
+    if eos == 0:
+        np.testing.assert_allclose(Wg[:, :3], Wo[:, :3], rtol=1e-10, atol=1e-18)
+    else:
+        # TM at |M| -> 0: the cubic's root W = gamma^2 - 1 = |u|^2 is a difference of O(1) terms, so
+        # it carries an ABSOLUTE error ~1e-16 (R6/R7) and u = sqrt(W) is only comparable through u^2
+        np.testing.assert_allclose(Wg[[0, 4], :3], Wo[[0, 4], :3], rtol=1e-10)
+        np.testing.assert_allclose(Wg[1:4, :3] ** 2, Wo[1:4, :3] ** 2, rtol=1e-10, atol=2e-15)
 
 
 def test_con2prim_batch_host_wrapper_chunks():
@@ -250,9 +255,10 @@ def test_enforce_physicality_matches_oracle(nd, nelem, p, eos, G):
     assert np.array_equal(Ug[:, un], Ubad[:, un])                    # untouched cells bit-identical
     scale = np.abs(Uo).max(axis=0) + 1e-300
     assert np.max(np.abs(Ug - Uo) / scale) <= 1e-11
-    # idempotent: a second application flags nothing
+    # idempotent: a second application flags nothing, except the cells whose mean is itself
+    # inadmissible (flattened to that mean, R13d), which it flags and counts again
     _, _, cnt2 = ctx.dgrhd_enforce_physicality(to_dev(Ug))
-    assert cnt2 == (0, 0)
+    assert cnt2 == (cnt_o[1], cnt_o[1])
 
 
 def test_enforce_physicality_inadmissible_mean_is_flattened_and_counted():

@@ -290,6 +290,27 @@ def test_tm_both_cubic_branches_are_exercised_and_agree():
         assert np.max(np.abs(W2[0, mask] / W[0, mask] - 1) / g2[mask]) < 50 * 2.2e-16
 
 
+def test_tm_recovers_slow_flows_to_full_relative_accuracy():
+    """Reading R7b: as gamma -> 1 the closed-form root of Eq. 61 (W = gamma^2 - 1 = |u|^2) carries an
+    absolute error ~1e-16, i.e. no correct digits of u below |u| ~ 1e-8; with one Newton correction on
+    the cubic the round trip from exactly known primitives recovers u to ~1e-13 relative over
+    |u| in [1e-9, 1e-1], for cold and hot gas alike (Fig. 2 protocol :405)."""
+    rng = np.random.default_rng(4)
+    n = 4000
+    umag = 10.0 ** rng.uniform(-9, -1, n)
+    dirn = rng.normal(size=(3, n)); dirn /= np.sqrt((dirn ** 2).sum(0))
+    rho = 10.0 ** rng.uniform(-3, 2, n)
+    P = rho * 10.0 ** rng.uniform(-6, 3, n)
+    W = np.vstack([rho[None], umag * dirn, P[None]])
+    U = O.prim2con_batch(O.EOS_TM, 0.0, W)
+    W2, st = O.con2prim_batch(O.EOS_TM, 0.0, U)
+    assert st.max() == 0
+    u2 = np.sqrt((W2[1:4] ** 2).sum(0))
+    assert np.max(np.abs(u2 / umag - 1)) < 2e-12
+    assert np.max(np.abs(W2[0] / rho - 1)) < 1e-14
+    assert np.max(np.abs(W2[4] - P) / (P + 1e-3 * U[4])) < 1e-11
+
+
 def test_ideal_newton_iteration_claims_of_the_paper():
     """tests/golden/con2prim_iteration_claims.txt: on the Fig. 2 grid the
     iterative ideal solver reaches (near) machine precision in velocity with 6 iterations for

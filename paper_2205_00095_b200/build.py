@@ -47,6 +47,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             o = os.path.join(OBJ, f"stage_{nd}_{eos}.o")
             jobs.append(([nvcc, *NVCC_FLAGS, f"-DDG_INST_ND={nd}", f"-DDG_INST_EOS={eos}", "-c",
                           os.path.join(CSRC, "stage_inst.cu"), "-o", o], o))
+    extra = os.environ.get("DGRHD_NVCC_EXTRA", "").split()      # kernel-tuning experiments only
+    for j in jobs:
+        j[0][1:1] = extra
     if verbose:
         for j in jobs:
             j[0].insert(1, "-Xptxas=-v")

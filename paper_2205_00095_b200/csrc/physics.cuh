@@ -61,76 +61,96 @@ DG_INL void dg_prim2con(const EosPar& e, const double W[5], double U[5]) {
   U[4] = fma(g2, rh, -W[4]);
 }
 
-// Everything a face needs from one side, for direction dir (runtime, 0..2; selects keep W and F in
-// registers):
-//   U (Eq. 4), F_dir (Eq. 2: F = U v_d + P e_d, F_E = (E+P) v_d) and lambda-+ (Eq. 21-22).
+// sigma_s = num/den of Eq. 22 as an unevaluated fraction (same algebra as dg_sigma).
 template <int EOS>
-DG_INL void dg_side(const EosPar& e, const double W[5], int dir, double U[5], double F[5],
-                    double& lm, double& lp) {
-  double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  double rg = rsqrt(g2);
-  double g = g2 * rg;
-  double rho = W[0], P = W[4];
-  double rh = dg_rho_h<EOS>(e, rho, P);
-  double grh = g * rh;
-  U[0] = g * rho;
-  U[1] = grh * W[1];
-  U[2] = grh * W[2];
-  U[3] = grh * W[3];
-  U[4] = fma(g2, rh, -P);
-  double ud = (dir == 0) ? W[1] : ((dir == 1) ? W[2] : W[3]);
-  double vd = ud * rg;
-  F[0] = U[0] * vd;
-  F[1] = fma(U[1], vd, (dir == 0) ? P : 0.0);
-  F[2] = fma(U[2], vd, (dir == 1) ? P : 0.0);
-  F[3] = fma(U[3], vd, (dir == 2) ? P : 0.0);
-  F[4] = (U[4] + P) * vd;
-  double sig = dg_sigma<EOS>(e, rho, P, g2);
-  double root = sqrt(sig * (fma(-vd, vd, 1.0) + sig));
-  double r1 = 1.0 / (1.0 + sig);
-  lm = (vd - root) * r1;
-  lp = (vd + root) * r1;
+DG_INL void dg_sigma_frac(const EosPar& e, double rho, double P, double g2, double& num, double& den) {
+  if (EOS == DG_EOS_IDEAL) {
+    num = e.G * P;
+    den = g2 * (fma(e.al, P, rho) - num);
+  } else {
+    const double R = sqrt(fma(P, P, (4.0 / 9.0) * rho * rho));
+    const double PR = P * R;
+    num = fma(3.0 * P, P, 5.0 * PR);
+    den = g2 * fma(9.0 * P, P, fma(2.0 * rho, rho, 7.0 * PR));
+  }
+}
+
+// lambda-+ of Eq. 21 with sigma = num/den substituted, so that one square root and one division
+// remain:  lambda-+ = (v den -+ sqrt(num ((1 - v^2) den + num))) / (den + num).
+template <int EOS>
+DG_INL void dg_speeds(const EosPar& e, double rho, double P, double g2, double vd, double& lm, double& lp) {
+  double num, den;
+  dg_sigma_frac<EOS>(e, rho, P, g2, num, den);
+  const double root = sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
+  const double r = 1.0 / (den + num);
+  const double c = vd * den;
+  lm = (c - root) * r;
+  lp = (c + root) * r;
+}
+
+// One side's contribution to the interface flux:  acc += cF F_dir(W) + cU U(W)   (Eq. 2, Eq. 4).
+template <int EOS>
+DG_INL void dg_side_accum(const EosPar& e, const double W[5], int dir, double g2, double rg, double vd,
+                          double cF, double cU, double acc[5]) {
+  const double rho = W[0], P = W[4];
+  const double rh = dg_rho_h<EOS>(e, rho, P);
+  const double g = g2 * rg;
+  const double grh = g * rh;
+  const double k = fma(cF, vd, cU);                 // cF U v_d + cU U = U (cF v_d + cU)
+  const double cP = cF * P;
+  acc[0] = fma(k, g * rho, acc[0]);
+  acc[1] = fma(k, grh * W[1], acc[1] + ((dir == 0) ? cP : 0.0));
+  acc[2] = fma(k, grh * W[2], acc[2] + ((dir == 1) ? cP : 0.0));
+  acc[3] = fma(k, grh * W[3], acc[3] + ((dir == 2) ? cP : 0.0));
+  const double E = fma(g2, rh, -P);
+  acc[4] = fma(k, E, fma(cP, vd, acc[4]));          // cF (E+P) v_d + cU E
 }
 
 // HLL two-wave flux (PAPER.md:161 cites Schneider et al.; reading R9) with lambda_L,
-// lambda_R of Eq. 23-24; U_{L,R} from W_{L,R} by Eq. 4 (reading R8).
+// lambda_R of Eq. 23-24; U_{L,R} from W_{L,R} by Eq. 4 (reading R8).  Branch-free: the three cases
+// of R9 are the coefficient triples (1,0,0), (0,1,0), (lR,-lL,lL lR)/(lR-lL) of
+//   F = cL F_L + cR F_R + cU (U_R - U_L).
 template <int EOS>
 DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], int dir, double F[5]) {
-  double UL[5], UR[5], FL[5], FR[5], lmL, lpL, lmR, lpR;
-  dg_side<EOS>(e, WL, dir, UL, FL, lmL, lpL);
-  dg_side<EOS>(e, WR, dir, UR, FR, lmR, lpR);
-  double lL = fmin(lmL, lmR);
-  double lR = fmax(lpL, lpR);
-  if (lL >= 0.0) {
-#pragma unroll
-    for (int v = 0; v < 5; ++v) F[v] = FL[v];
-  } else if (lR <= 0.0) {
-#pragma unroll
-    for (int v = 0; v < 5; ++v) F[v] = FR[v];
-  } else {
-    double rd = 1.0 / (lR - lL);
-    double ll = lL * lR;
-#pragma unroll
-    for (int v = 0; v < 5; ++v)
-      F[v] = (fma(lR, FL[v], -lL * FR[v]) + ll * (UR[v] - UL[v])) * rd;
+  const double g2L = fma(WL[1], WL[1], fma(WL[2], WL[2], fma(WL[3], WL[3], 1.0)));
+  const double g2R = fma(WR[1], WR[1], fma(WR[2], WR[2], fma(WR[3], WR[3], 1.0)));
+  const double rgL = rsqrt(g2L), rgR = rsqrt(g2R);
+  const double vL = ((dir == 0) ? WL[1] : ((dir == 1) ? WL[2] : WL[3])) * rgL;
+  const double vR = ((dir == 0) ? WR[1] : ((dir == 1) ? WR[2] : WR[3])) * rgR;
+  double lmL, lpL, lmR, lpR;
+  dg_speeds<EOS>(e, WL[0], WL[4], g2L, vL, lmL, lpL);
+  dg_speeds<EOS>(e, WR[0], WR[4], g2R, vR, lmR, lpR);
+  const double lL = fmin(lmL, lmR);                 // Eq. 23
+  const double lR = fmax(lpL, lpR);                 // Eq. 24
+  double cL, cR, cU;
+  if (lL >= 0.0) { cL = 1.0; cR = 0.0; cU = 0.0; }
+  else if (lR <= 0.0) { cL = 0.0; cR = 1.0; cU = 0.0; }
+  else {
+    const double rd = 1.0 / (lR - lL);
+    cL = lR * rd; cR = -lL * rd; cU = lL * lR * rd;
   }
+#pragma unroll
+  for (int v = 0; v < 5; ++v) F[v] = 0.0;
+  dg_side_accum<EOS>(e, WL, dir, g2L, rgL, vL, cL, -cU, F);
+  dg_side_accum<EOS>(e, WR, dir, g2R, rgR, vR, cR, cU, F);
 }
 
 // sum_d cw[d] max(|lambda-_d|, |lambda+_d|) for the CFL reduction (reading R11, Eq. 21-22).
 template <int EOS, int ND>
 DG_INL double dg_cfl_speed(const EosPar& e, const double W[5], const double cw[3]) {
-  double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  double rg = rsqrt(g2);
-  double sig = dg_sigma<EOS>(e, W[0], W[4], g2);
-  double r1 = 1.0 / (1.0 + sig);
+  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
+  const double rg = rsqrt(g2);
+  double num, den;
+  dg_sigma_frac<EOS>(e, W[0], W[4], g2, num, den);
+  const double r1 = 1.0 / (den + num);
   double a = 0.0;
 #pragma unroll
   for (int d = 0; d < ND; ++d) {
-    double vd = W[1 + d] * rg;
-    double root = sqrt(sig * (fma(-vd, vd, 1.0) + sig));
-    a = fma(cw[d], (fabs(vd) + root) * r1, a);      // max(|v-r|,|v+r|) = |v| + r  (r >= 0)
+    const double vd = W[1 + d] * rg;
+    const double root = sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
+    a = fma(cw[d], fma(fabs(vd), den, root), a);    // max(|l-|,|l+|) (den+num) = |v| den + root
   }
-  return a;
+  return a * r1;
 }
 
 // Admissibility predicate, Eq. 25 with the plus sign (Eq. 27/31/32; reading R13a) and the safety
@@ -142,8 +162,16 @@ DG_INL bool dg_admissible(const double U[5], double one_minus_eps) {
   m2 = __dadd_rn(m2, __dmul_rn(U[1], U[1]));
   m2 = __dadd_rn(m2, __dmul_rn(U[2], U[2]));
   m2 = __dadd_rn(m2, __dmul_rn(U[3], U[3]));
-  double Es = __dmul_rn(one_minus_eps, U[4]);
-  return (U[0] > 0.0) && (Es > __dsqrt_rn(m2));
+  const double Es = __dmul_rn(one_minus_eps, U[4]);
+  if (!(U[0] > 0.0) || !(Es > 0.0)) return false;
+  // The decision Es > sqrt(m2) is taken without the square root wherever Es^2 and m2 differ by
+  // more than 1e-12 relative (>> the 2-ulp rounding of Es*Es); only marginal states pay for the
+  // correctly rounded sqrt, so the result is identical to the reference expression in every case.
+  const double t = __dmul_rn(Es, Es);
+  if (!(t > 1e-280 && t < 1e300)) return Es > __dsqrt_rn(m2);   // outside the safely normal range
+  if (t > __dmul_rn(m2, 1.0 + 1e-12)) return true;
+  if (!(t >= __dmul_rn(m2, 1.0 - 1e-12))) return false;
+  return Es > __dsqrt_rn(m2);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -153,50 +181,75 @@ DG_INL bool dg_finite5(const double W[5]) {
   return isfinite(W[0]) && isfinite(W[1]) && isfinite(W[2]) && isfinite(W[3]) && isfinite(W[4]);
 }
 
+// single-precision reciprocal / square root of a double (MUFU): only where the result feeds a
+// self-correcting iteration (Newton's step size, its starting point), never a final value.
+DG_INL double dg_rcp_lo(double x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(__double2float_rn(x)));
+  return (double)r;
+}
+DG_INL double dg_sqrt_lo(double x) {
+  float r;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(__double2float_rn(x)));
+  return (double)r;
+}
+
 // Ideal EOS: Newton on the quartic of Eq. 59 in w, beta = 2w/(1+w^2) (Eq. 58),
 // start beta_0 = |M|/E (reading R2), stop |dw| <= 1e-14 w or 16 iterations (R3), small-xi series
 // Eq. 60 for xi < 1e-4 (R4); finishing Eq. 55-57 with 1/gamma = (1-w^2)/(1+w^2).
+// fp64 divisions are the expensive operation here, so: xi, eta share 1/D; the Newton step p/p' and
+// the starting point use single-precision reciprocals (the iteration corrects them: a step with
+// relative error 6e-8 still contracts the error by that factor, and the stopping test is on the
+// fp64 step); the three divisions of the finishing formulas share one reciprocal.
 DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
   const double D = U[0], E = U[4];
   const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
   const double Mabs = sqrt(M2);
-  const double xi = Mabs / D, eta = E / D;                       // Eq. 38
+  const double rD = 1.0 / D;
+  const double xi = Mabs * rD, eta = E * rD;                     // Eq. 38
   const double al = e.al;
+  if (xi == 0.0) {                                               // v = 0 (R4)
+    W[0] = D; W[1] = 0.0; W[2] = 0.0; W[3] = 0.0;
+    W[4] = (e.G - 1.0) * (E - D);
+    return (isfinite(W[4]) && W[4] > 0.0) ? 0 : 2;
+  }
   double w;
-  if (xi < 1e-4) {
-    if (xi == 0.0) {
-      w = 0.0;
-    } else {                                                     // Eq. 60
-      double a1 = fma(al, eta, -1.0);
-      double a12 = a1 * a1;
-      double am = al - 1.0;
-      double t3 = am * am / (8.0 * a12 * a12) *
-                  ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
-      w = am / (2.0 * a1) * xi + t3 * xi * xi * xi;
-    }
+  if (xi < 1e-4) {                                               // Eq. 60
+    double a1 = fma(al, eta, -1.0);
+    double a12 = a1 * a1;
+    double am = al - 1.0;
+    double t3 = am * am / (8.0 * a12 * a12) * ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
+    w = am / (2.0 * a1) * xi + t3 * xi * xi * xi;
   } else {
     const double c4 = (al - 1.0) * xi;                           // Eq. 59 (c0 = c4)
     const double c3 = -2.0 * fma(al, eta, 1.0);
     const double c2 = 2.0 * (al + 1.0) * xi;
     const double c1 = -2.0 * fma(al, eta, -1.0);
-    const double b0 = xi / eta;
-    w = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
+    const double d3 = 4.0 * c4, d2 = 3.0 * c3, d1 = 2.0 * c2;   // p'(w) coefficients
+    const bool lo_ok = (eta < 1e30);                             // single-precision range of p'
+    if (lo_ok) {
+      const double b0 = fmin(xi * dg_rcp_lo(eta), 1.0);
+      w = fmin(b0 * dg_rcp_lo(1.0 + dg_sqrt_lo(fmax(fma(-b0, b0, 1.0), 0.0))), 0.999999);
+    } else {
+      const double b0 = xi / eta;
+      w = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
+    }
 #pragma unroll 1
     for (int it = 0; it < 16; ++it) {
-      double p = fma(fma(fma(fma(c4, w, c3), w, c2), w, c1), w, c4);
-      double dp = fma(fma(fma(4.0 * c4, w, 3.0 * c3), w, 2.0 * c2), w, c1);
-      double dw = p / dp;
+      const double p = fma(fma(fma(fma(c4, w, c3), w, c2), w, c1), w, c4);
+      const double dp = fma(fma(fma(d3, w, d2), w, d1), w, c1);
+      const double dw = lo_ok ? p * dg_rcp_lo(dp) : p / dp;
       w -= dw;
       if (fabs(dw) <= 1e-14 * w) break;
     }
   }
   const double w2 = w * w;
-  const double r1 = 1.0 / (1.0 + w2);
-  const double om = 1.0 - w2;
+  const double op = 1.0 + w2, om = 1.0 - w2;
+  const double r = 1.0 / (op * om * Mabs);                       // one reciprocal for Eq. 55-58
+  const double r1 = r * om * Mabs;                               // 1/(1+w^2)
   const double beta = 2.0 * w * r1;                              // Eq. 58
   const double rho = D * om * r1;                                // Eq. 55, 1/gamma = (1-w^2)/(1+w^2)
-  const double ug = 2.0 * w / om;                                // gamma beta
-  const double sc = (Mabs > 0.0) ? ug / Mabs : 0.0;              // u = gamma beta M/|M|  (Eq. 56)
+  const double sc = 2.0 * w * op * r;                            // gamma beta / |M|  (Eq. 56)
   W[0] = rho;
   W[1] = sc * U[1];
   W[2] = sc * U[2];

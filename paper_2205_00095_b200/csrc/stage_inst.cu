@@ -19,6 +19,8 @@ static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, TS::SMEM_BYTES);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
     attr_done = true;
   }
   const long long ntx = (a.ne[0] + TS::TX - 1) / TS::TX, nty = (a.ne[1] + TS::TY - 1) / TS::TY,

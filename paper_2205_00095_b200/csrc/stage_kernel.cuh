@@ -30,15 +30,17 @@ typedef unsigned long long dg_ull;
 
 __host__ __device__ constexpr int dg_ipow(int b, int e) { return e <= 0 ? 1 : b * dg_ipow(b, e - 1); }
 
-#ifndef DG_T3N4
-#define DG_T3N4 2, 2, 2
+#ifndef DG_T3N4X       // tile of the 3D p=3 kernel (tuning knob)
+#define DG_T3N4X 2
+#define DG_T3N4Y 2
+#define DG_T3N4Z 1
 #endif
 // elements per thread block along x,y,z for [ndim-1][N-1]
 __host__ __device__ constexpr int dg_tile(int nd, int N, int d) {
   constexpr int t[3][5][3] = {
-      {{256, 1, 1}, {128, 1, 1}, {64, 1, 1}, {64, 1, 1}, {48, 1, 1}},
-      {{32, 8, 1}, {16, 4, 1}, {8, 4, 1}, {4, 4, 1}, {4, 2, 1}},
-      {{8, 8, 4}, {4, 4, 2}, {4, 2, 2}, {DG_T3N4}, {2, 1, 1}}};
+      {{256, 1, 1}, {128, 1, 1}, {60, 1, 1}, {64, 1, 1}, {48, 1, 1}},
+      {{32, 8, 1}, {16, 4, 1}, {6, 4, 1}, {4, 4, 1}, {4, 2, 1}},
+      {{8, 8, 4}, {4, 4, 2}, {2, 2, 2}, {DG_T3N4X, DG_T3N4Y, DG_T3N4Z}, {2, 1, 1}}};
   return t[nd - 1][N - 1][d];
 }
 
@@ -49,7 +51,16 @@ struct TileShape {
   static constexpr int TX = dg_tile(ND, N, 0), TY = dg_tile(ND, N, 1), TZ = dg_tile(ND, N, 2);
   static constexpr int NE = TX * TY * TZ;            // elements per tile
   static constexpr int NTN = NE * NN;                // nodes per tile
-  static constexpr int NT = (NTN + 31) / 32 * 32;    // threads per block
+  // Threads are organised in warp groups that own whole elements, so that everything cell-local
+  // (tensor-line contractions, cell mean, min s) synchronises a group, not the block:
+  //   NN <= 32: one warp holds EPG = 32/NN elements (lanes >= EPG*NN idle);  NN > 32: G warps per element.
+  static constexpr int G = (NN <= 32) ? 1 : (NN + 31) / 32;   // warps per group
+  static constexpr int EPG = (NN <= 32) ? 32 / NN : 1;        // elements per group
+  static constexpr int GT = 32 * G;                           // threads per group
+  static constexpr int NG = NE / EPG;                         // groups per block
+  static_assert(NE % EPG == 0, "tile must hold a whole number of warp groups");
+  static_assert(G == 1 || NG <= 15, "named barriers 1..15");
+  static constexpr int NT = NG * GT;                 // threads per block
   __host__ __device__ static constexpr int T(int d) { return d == 0 ? TX : (d == 1 ? TY : TZ); }
   __host__ __device__ static constexpr int SE(int d) { return d == 0 ? 1 : (d == 1 ? TX : TX * TY); }
   __host__ __device__ static constexpr int SN(int d) { return dg_ipow(N, d); }
@@ -69,7 +80,8 @@ struct TileShape {
   static constexpr int O_MEAN = O_D + 32;                // [NE][5]
   static constexpr int O_SMIN = O_MEAN + 5 * NE;         // [NE] (ull)
   static constexpr int O_RED = O_SMIN + NE;              // [32]
-  static constexpr int O_FLAG = O_RED + 32;              // ints: [NE] flags + [4] counters
+  static constexpr int O_PART = O_RED + 32;              // [NE][4][5] partial sums of the cell mean
+  static constexpr int O_FLAG = O_PART + 20 * NE;        // ints: [NE] flags + [4] counters
   static constexpr int SMEM_BYTES = O_FLAG * 8 + (NE + 4) * 4 + 16;
 };
 
@@ -237,66 +249,148 @@ __device__ __forceinline__ bool dg_face_ptrs(const double* Ws, const double* Hs,
   return true;
 }
 
+
+// Barrier over one warp group (G warps): __syncwarp for G = 1, else the named barrier grp+1.
+template <int G>
+__device__ __forceinline__ void dg_gsync(int grp) {
+  if (G == 1) __syncwarp();
+  else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(32 * G) : "memory");
+}
+
 // Lift of the interface flux onto a node (Eq. 18 over the diagonal mass matrix) for direction D:
-//   + lift * Fhat at the element's minus face if the node sits on it, - lift * Fhat at its plus face.
+//   + c * Fhat at the element's minus face if the node sits on it, - c * Fhat at its plus face,
+//   c = (2/h_D) / w_0.
 template <int ND, int N, int D>
 __device__ __forceinline__ void dg_add_surface(const double* Fh, const int lc[3], const int in[3],
-                                               double lift, double acc[5]) {
+                                               double c, double R[5]) {
   using TS = TileShape<ND, N>;
   using DI = DirInfo<ND, N, D>;
   constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
+  if (in[D] != 0 && in[D] != N - 1) return;
   const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
   const double* base = Fh + 5 * TS::FOFF(D) + fp;
   if (in[D] == 0) {
     const double* p = base + lc[D] * 5 * FPD;
 #pragma unroll
-    for (int v = 0; v < 5; ++v) acc[v] = fma(lift, p[v * FPD], acc[v]);
+    for (int v = 0; v < 5; ++v) R[v] = fma(c, p[v * FPD], R[v]);
   }
   if (in[D] == N - 1) {
     const double* p = base + (lc[D] + 1) * 5 * FPD;
 #pragma unroll
-    for (int v = 0; v < 5; ++v) acc[v] = fma(-lift, p[v * FPD], acc[v]);
+    for (int v = 0; v < 5; ++v) R[v] = fma(-c, p[v * FPD], R[v]);
   }
 }
 
-// One direction of the spatial operator for this thread's node: flux (Eq. 2) of the node into shared
-// memory, then the tensor-line contraction with Dhat (Eq. 17) and the surface lift (Eq. 18).
+// One direction of the volume term for this thread's node: flux (Eq. 2) of the node into the
+// shared buffer Fb, group barrier, tensor-line contraction with Dhat (Eq. 17).  The caller
+// alternates Fb between two buffers, so no barrier is needed after the reads.
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_direction(const StageArgs& a, const double* sD, double* Fs,
-                                             const double* Fh, int t, bool active, const int lc[3],
-                                             const int in[3], const double Un[5], double P, double vd,
-                                             double R[5]) {
+__device__ __forceinline__ void dg_direction(const StageArgs& a, const double* sD, double* Fb, int ti,
+                                             bool active, int grp, const int in[3], const double Un[5],
+                                             double P, double vd, double R[5]) {
   using TS = TileShape<ND, N>;
   constexpr int NTN = TS::NTN;
-  if (D > 0) __syncthreads();                                    // previous direction's reads done
   if (active) {
-    Fs[0 * NTN + t] = Un[0] * vd;
-    Fs[1 * NTN + t] = fma(Un[1], vd, (D == 0) ? P : 0.0);
-    Fs[2 * NTN + t] = fma(Un[2], vd, (D == 1) ? P : 0.0);
-    Fs[3 * NTN + t] = fma(Un[3], vd, (D == 2) ? P : 0.0);
-    Fs[4 * NTN + t] = (Un[4] + P) * vd;
+    Fb[0 * NTN + ti] = Un[0] * vd;
+    Fb[1 * NTN + ti] = fma(Un[1], vd, (D == 0) ? P : 0.0);
+    Fb[2 * NTN + ti] = fma(Un[2], vd, (D == 1) ? P : 0.0);
+    Fb[3 * NTN + ti] = fma(Un[3], vd, (D == 2) ? P : 0.0);
+    Fb[4 * NTN + ti] = (Un[4] + P) * vd;
   }
-  __syncthreads();
+  dg_gsync<TS::G>(grp);
   if (active) {
     const int id = in[D];
-    const double* line = Fs + (t - id * TS::SN(D));
+    const double* line = Fb + (ti - id * TS::SN(D));
     const double* dh = sD + id * N;
-    double acc[5];
+    double dq[N];
+#pragma unroll
+    for (int q = 0; q < N; ++q) dq[q] = a.rh[D] * dh[q];
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double s = 0.0;
 #pragma unroll
-      for (int q = 0; q < N; ++q) s = fma(dh[q], line[v * NTN + q * TS::SN(D)], s);
-      acc[v] = s;
+      for (int q = 0; q < N; ++q) R[v] = fma(dq[q], line[v * NTN + q * TS::SN(D)], R[v]);
     }
-    dg_add_surface<ND, N, D>(Fh, lc, in, a.lift, acc);
-#pragma unroll
-    for (int v = 0; v < 5; ++v) R[v] = fma(a.rh[D], acc[v], R[v]);
   }
 }
 
+// Physicality operator on the cells of one warp group (PAPER.md:242-252 steps 1-4), one thread per
+// node; cell-local reductions through shared memory with group barriers only.  Must be called by
+// every thread of the group.  Uo: the node's state, limited in place.
+template <int ND, int N>
+__device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int ti, int le, int n, int grp,
+                                                 double wn, const StageArgs& a, double* scratch,
+                                                 double* sPart, double* sMean, dg_ull* sSmin, int* sFlag,
+                                                 int* sCnt) {
+  using TS = TileShape<ND, N>;
+  constexpr int NN = TS::NN, NTN = TS::NTN;
+  const bool bad = active && !dg_admissible(Uo, a.f_screen);         // step 1: screen (R13e)
+  if (bad) sFlag[le] = 1;
+  dg_gsync<TS::G>(grp);
+  const bool flagged = active && (sFlag[le] != 0);
+  if (flagged) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) scratch[v * NTN + ti] = wn * Uo[v];
+  }
+  dg_gsync<TS::G>(grp);
+  // cell average: J interleaved partial sums per variable (5 J lanes), then their sum by 5 lanes
+  constexpr int J = (NN >= 20) ? 4 : NN / 5;
+  if (J == 0) {                                                     // tiny cells: one lane sums
+    if (flagged && n == 0) {
+      for (int v = 0; v < 5; ++v) {
+        double acc = 0.0;
+        for (int m = 0; m < NN; ++m) acc += scratch[v * NTN + le * NN + m];
+        sMean[le * 5 + v] = acc / a.wsum;
+      }
+    }
+  } else {
+    if (flagged && n < 5 * J) {
+      const int v = n % 5, j = n / 5;
+      const double* p = scratch + v * NTN + le * NN;
+      double acc = 0.0;
+      for (int m = j; m < NN; m += J) acc += p[m];
+      sPart[le * 20 + n] = acc;
+    }
+    dg_gsync<TS::G>(grp);
+    if (flagged && n < 5) {
+      double acc = 0.0;
+#pragma unroll
+      for (int j = 0; j < J; ++j) acc += sPart[le * 20 + 5 * j + n];
+      sMean[le * 5 + n] = acc / a.wsum;
+    }
+  }
+  dg_gsync<TS::G>(grp);
+  double Ub[5];
+  if (flagged) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) Ub[v] = sMean[le * 5 + v];
+    const bool mean_ok = dg_admissible(Ub, a.f_solve);               // step 2 (reading R13d)
+    double si = 0.0;
+    if (mean_ok) {
+      si = dg_limiter_node_s(Ub, Uo, a.f_solve);                     // step 3
+      if (!(si >= 0.0)) si = 0.0;
+    }
+    if (si < 1.0) atomicMin(&sSmin[le], dg_ord(si));                 // step 4: s = min_i s_i
+    if (n == 0) {
+      atomicAdd(&sCnt[0], 1);
+      if (!mean_ok) atomicAdd(&sCnt[1], 1);
+    }
+  }
+  dg_gsync<TS::G>(grp);
+  if (flagged) {
+    const double s = a.one_m_delta * dg_unord(sSmin[le]);            // R13c
+    const double tt = 1.0 - s;
+#pragma unroll
+    for (int v = 0; v < 5; ++v)                                      // Eq. 26 from the nearer end (R14)
+      Uo[v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[v], Uo[v]) : fma(s, Uo[v] - Ub[v], Ub[v]);
+  }
+}
+
+// resident blocks per SM the register allocation must allow: 1024 threads (32 warps) per SM
+#ifndef DG_MINB
+#define DG_MINB (1024 / TileShape<ND, N>::NT)
+#endif
 template <int ND, int N, int EOS>
-__global__ void __launch_bounds__(TileShape<ND, N>::NT)
+__global__ void __launch_bounds__(TileShape<ND, N>::NT, DG_MINB)
 dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
   constexpr int NN = TS::NN, NTN = TS::NTN, NT = TS::NT, NE = TS::NE;
@@ -309,6 +403,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   double* sMean = sm + TS::O_MEAN;
   dg_ull* sSmin = reinterpret_cast<dg_ull*>(sm + TS::O_SMIN);
   double* sRed = sm + TS::O_RED;
+  double* sPart = sm + TS::O_PART;
   int* sFlag = reinterpret_cast<int*>(sm + TS::O_FLAG);
   int* sCnt = sFlag + NE;
 
@@ -318,12 +413,14 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   const int org[3] = {(bt % ntx) * TS::TX, ((bt / ntx) % nty) * TS::TY, (bt / (ntx * nty)) * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
-  // node of this thread
+  // warp group, element and node of this thread
   const int t = threadIdx.x;
-  const int le = t / NN, n = t - le * NN;
+  const int grp = t / TS::GT, r = t - grp * TS::GT;
+  const int le = grp * TS::EPG + r / NN, n = r % NN;
+  const int ti = le * NN + n;                                        // node slot in the tile arrays
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
   const int in[3] = {n % N, (n / N) % N, n / (N * N)};
-  const bool active = (t < NTN) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
+  const bool active = (r < TS::EPG * NN) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
   long long g = 0;
   if (active) {
     const long long e = (org[0] + lc[0]) +
@@ -334,15 +431,19 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   if (t < 4) sCnt[t] = 0;
   if (t < N * N) sD[t] = a.Dhat[t];
 
-  // 1. stage W of the tile and of the neighbours' facing nodal layers
-  double Wn[5] = {1.0, 0.0, 0.0, 0.0, 1.0}, Un[5] = {0, 0, 0, 0, 0};
+  // 1. stage W of the tile and of the neighbours' facing nodal layers; U_s of the node in flight
+  double P = 1.0, v0 = 0.0, v1 = 0.0, v2 = 0.0, Un[5] = {0, 0, 0, 0, 0};
   if (active) {
+    double Wn[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
       Wn[v] = __ldg(a.Win + v * a.ndof + g);
-      Ws[v * NTN + t] = Wn[v];
-      Un[v] = a.Us[v * a.ndof + g];
+      Ws[v * NTN + ti] = Wn[v];
     }
+#pragma unroll
+    for (int v = 0; v < 5; ++v) Un[v] = a.Us[v * a.ndof + g];
+    const double rg = rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
+    P = Wn[4]; v0 = Wn[1] * rg; v1 = Wn[2] * rg; v2 = Wn[3] * rg;
   }
   for (int hl = t; hl < 2 * TS::FP(0); hl += NT) dg_load_halo<ND, N, 0>(a, Hs, hl, org, teff);
   if constexpr (ND > 1)
@@ -351,7 +452,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     for (int hl = t; hl < 2 * TS::FP(2); hl += NT) dg_load_halo<ND, N, 2>(a, Hs, hl, org, teff);
   __syncthreads();
 
-  // 2. interface flux at every face point of the tile, once each
+  // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
     const double *pL = nullptr, *pR = nullptr;
     double* pF = nullptr;
@@ -373,15 +474,20 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       for (int v = 0; v < 5; ++v) pF[v * sF] = F[v];
     }
   }
-  __syncthreads();
 
-  // 3.-4. volume quadrature + surface lift, one direction at a time; F(W_i) = U_i v_d + P e_d
+  // 3. volume quadrature, direction by direction, F(W_i) = U_i v_d + P e_d; the first direction
+  //    overlaps other warps' face fluxes, the block barrier then frees Ws as the second F buffer
   double R[5] = {0, 0, 0, 0, 0};
-  {
-    const double rg = rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
-    dg_direction<ND, N, 0>(a, sD, Fs, Fh, t, active, lc, in, Un, Wn[4], Wn[1] * rg, R);
-    if constexpr (ND > 1) dg_direction<ND, N, 1>(a, sD, Fs, Fh, t, active, lc, in, Un, Wn[4], Wn[2] * rg, R);
-    if constexpr (ND > 2) dg_direction<ND, N, 2>(a, sD, Fs, Fh, t, active, lc, in, Un, Wn[4], Wn[3] * rg, R);
+  dg_direction<ND, N, 0>(a, sD, Fs, ti, active, grp, in, Un, P, v0, R);
+  __syncthreads();
+  if constexpr (ND > 1) dg_direction<ND, N, 1>(a, sD, Ws, ti, active, grp, in, Un, P, v1, R);
+  if constexpr (ND > 2) dg_direction<ND, N, 2>(a, sD, Fs, ti, active, grp, in, Un, P, v2, R);
+
+  // 4. surface lift
+  if (active) {
+    dg_add_surface<ND, N, 0>(Fh, lc, in, a.rh[0] * a.lift, R);
+    if constexpr (ND > 1) dg_add_surface<ND, N, 1>(Fh, lc, in, a.rh[1] * a.lift, R);
+    if constexpr (ND > 2) dg_add_surface<ND, N, 2>(Fh, lc, in, a.rh[2] * a.lift, R);
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
@@ -405,9 +511,8 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   double wn = a.w[in[0]];
   if (ND > 1) wn *= a.w[in[1]];
   if (ND > 2) wn *= a.w[in[2]];
-  double s_cell;
-  dg_limiter_block<NN, NE, NTN>(Uo, active, t, le, n, wn, a.wsum, a.f_screen, a.f_solve, a.one_m_delta,
-                                Fs, sMean, sSmin, sFlag, sCnt, s_cell);
+  dg_limiter_group<ND, N>(Uo, active, ti, le, n, grp, wn, a, (ND == 2) ? Fs : Ws, sPart, sMean, sSmin,
+                          sFlag, sCnt);
 
   // 7. primitives of the new state, CFL maximum
   double speed = 0.0;

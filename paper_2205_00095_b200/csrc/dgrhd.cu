@@ -55,6 +55,11 @@ bool valid_cfg(const dgrhd_config* c) {
   if (c->eos != DGRHD_EOS_IDEAL && c->eos != DGRHD_EOS_TAUB_MATTHEWS) return false;
   if (c->eos == DGRHD_EOS_IDEAL && !(c->gamma_ad > 1.0)) return false;
   if (c->rk_stages < 1 || c->rk_stages > 3) return false;
+  {                                         // kernels index nodes with 32-bit integers
+    double nd = 1.0;
+    for (int d = 0; d < c->ndim; ++d) nd *= (double)c->nelem[d] * (c->order_p + 1);
+    if (nd >= 2147483648.0) return false;
+  }
   if (!(c->eps_q >= 0.0 && c->eps_q < 0.5) || !(c->delta_s >= 0.0 && c->delta_s < 0.5)) return false;
   return true;
 }

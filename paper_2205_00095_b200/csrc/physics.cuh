@@ -89,8 +89,8 @@ DG_INL void dg_speeds(const EosPar& e, double rho, double P, double g2, double v
 }
 
 // One side's contribution to the interface flux:  acc += cF F_dir(W) + cU U(W)   (Eq. 2, Eq. 4).
-template <int EOS>
-DG_INL void dg_side_accum(const EosPar& e, const double W[5], int dir, double g2, double rg, double vd,
+template <int EOS, int dir>
+DG_INL void dg_side_accum(const EosPar& e, const double W[5], double g2, double rg, double vd,
                           double cF, double cU, double acc[5]) {
   const double rho = W[0], P = W[4];
   const double rh = dg_rho_h<EOS>(e, rho, P);
@@ -110,8 +110,8 @@ DG_INL void dg_side_accum(const EosPar& e, const double W[5], int dir, double g2
 // lambda_R of Eq. 23-24; U_{L,R} from W_{L,R} by Eq. 4 (reading R8).  Branch-free: the three cases
 // of R9 are the coefficient triples (1,0,0), (0,1,0), (lR,-lL,lL lR)/(lR-lL) of
 //   F = cL F_L + cR F_R + cU (U_R - U_L).
-template <int EOS>
-DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], int dir, double F[5]) {
+template <int EOS, int dir>
+DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], double F[5]) {
   const double g2L = fma(WL[1], WL[1], fma(WL[2], WL[2], fma(WL[3], WL[3], 1.0)));
   const double g2R = fma(WR[1], WR[1], fma(WR[2], WR[2], fma(WR[3], WR[3], 1.0)));
   const double rgL = rsqrt(g2L), rgR = rsqrt(g2R);
@@ -131,8 +131,8 @@ DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], int 
   }
 #pragma unroll
   for (int v = 0; v < 5; ++v) F[v] = 0.0;
-  dg_side_accum<EOS>(e, WL, dir, g2L, rgL, vL, cL, -cU, F);
-  dg_side_accum<EOS>(e, WR, dir, g2R, rgR, vR, cR, cU, F);
+  dg_side_accum<EOS, dir>(e, WL, g2L, rgL, vL, cL, -cU, F);
+  dg_side_accum<EOS, dir>(e, WR, g2R, rgR, vR, cR, cU, F);
 }
 
 // sum_d cw[d] max(|lambda-_d|, |lambda+_d|) for the CFL reduction (reading R11, Eq. 21-22).

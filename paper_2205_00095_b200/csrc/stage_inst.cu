@@ -25,9 +25,9 @@ static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
   }
   const long long ntx = (a.ne[0] + TS::TX - 1) / TS::TX, nty = (a.ne[1] + TS::TY - 1) / TS::TY,
                   ntz = (a.ne[2] + TS::TZ - 1) / TS::TZ;
-  const long long nb = ntx * nty * ntz;
-  if (nb <= 0 || nb > 2147483647LL) return cudaErrorInvalidConfiguration;
-  k<<<(unsigned)nb, TS::NT, TS::SMEM_BYTES, st>>>(a);
+  if (ntx <= 0 || nty <= 0 || ntz <= 0 || ntx > 2147483647LL || nty > 65535 || ntz > 65535)
+    return cudaErrorInvalidConfiguration;
+  k<<<dim3((unsigned)ntx, (unsigned)nty, (unsigned)ntz), TS::NT, TS::SMEM_BYTES, st>>>(a);
   return cudaGetLastError();
 }
 

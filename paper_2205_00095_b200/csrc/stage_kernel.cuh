@@ -189,40 +189,40 @@ struct DirInfo {
   }
 };
 
-// Load the halo point hl (0 .. 2*FP(D)) of direction D: the facing nodal layer of the neighbouring
-// element (periodic wrap) or, at an outflow boundary, the element's own face node (reading R12).
+// Load the halo of direction D (2*FP(D) points, spread over the block's threads): the facing nodal
+// layer of the neighbouring elements (periodic wrap) or, at an outflow boundary, the elements' own
+// face nodes (reading R12).  Everything that is uniform over the block is computed once.
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, int hl, const int org[3],
+__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, int t, const int org[3],
                                              const int teff[3]) {
   using TS = TileShape<ND, N>;
   using DI = DirInfo<ND, N, D>;
   constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
-  const int side = hl / FPD, fp = hl - side * FPD;
-  int la, lb, ca, cb;
-  DI::split(fp, la, lb, ca, cb);
-  if (la >= teff[A] || lb >= teff[B]) return;
-  int ed, nd_;
-  if (side == 0) {
-    ed = org[D] - 1; nd_ = N - 1;
-    if (ed < 0) {
-      if (a.bc[D] == DG_BC_PERIODIC) ed = a.ne[D] - 1;
-      else { ed = 0; nd_ = 0; }
-    }
-  } else {
-    ed = org[D] + teff[D]; nd_ = 0;
-    if (ed >= a.ne[D]) {
-      if (a.bc[D] == DG_BC_PERIODIC) ed = 0;
-      else { ed = a.ne[D] - 1; nd_ = N - 1; }
-    }
+  int ed0 = org[D] - 1, nl0 = N - 1, ed1 = org[D] + teff[D], nl1 = 0;
+  if (ed0 < 0) {
+    if (a.bc[D] == DG_BC_PERIODIC) ed0 = a.ne[D] - 1;
+    else { ed0 = 0; nl0 = 0; }
   }
-  int ec[3];
-  ec[D] = ed; ec[A] = org[A] + la; ec[B] = org[B] + lb;
-  const long long e = ec[0] + (long long)a.ne[0] * (ec[1] + (long long)a.ne[1] * ec[2]);
-  const int n = nd_ * TS::SN(D) + ca * TS::SN(A) + cb * TS::SN(B);
-  const long long g = e * TS::NN + n;
-  double* dst = Hs + 5 * TS::HOFF(D) + side * 5 * FPD + fp;
+  if (ed1 >= a.ne[D]) {
+    if (a.bc[D] == DG_BC_PERIODIC) ed1 = 0;
+    else { ed1 = a.ne[D] - 1; nl1 = N - 1; }
+  }
+  // 32-bit node indices: dgrhd_create rejects meshes with ndof >= 2^31
+  const int es[3] = {1, a.ne[0], a.ne[0] * a.ne[1]};
+  const int tb = org[A] * es[A] + org[B] * es[B];
+  const int b0 = (tb + ed0 * es[D]) * TS::NN + nl0 * TS::SN(D);
+  const int b1 = (tb + ed1 * es[D]) * TS::NN + nl1 * TS::SN(D);
+  const int sa = es[A] * TS::NN, sb = es[B] * TS::NN;
+  for (int hl = t; hl < 2 * FPD; hl += TS::NT) {
+    const int side = hl / FPD, fp = hl - side * FPD;
+    int la, lb, ca, cb;
+    DI::split(fp, la, lb, ca, cb);
+    if (la >= teff[A] || lb >= teff[B]) continue;
+    const double* src = a.Win + (side ? b1 : b0) + la * sa + lb * sb + (ca * TS::SN(A) + cb * TS::SN(B));
+    double* dst = Hs + 5 * TS::HOFF(D) + side * 5 * FPD + fp;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) dst[v * FPD] = __ldg(a.Win + v * a.ndof + g);
+    for (int v = 0; v < 5; ++v) dst[v * FPD] = __ldg(src + v * a.ndof);
+  }
 }
 
 // Face point fl (0 .. (T(D)+1)*FP(D)) of direction D: pointers to the left and right face states
@@ -249,6 +249,22 @@ __device__ __forceinline__ bool dg_face_ptrs(const double* Ws, const double* Hs,
   return true;
 }
 
+
+// HLL flux at face point fl of direction D into the Fhat array.
+template <int ND, int N, int EOS, int D>
+__device__ __forceinline__ void dg_face_flux(const EosPar& eos, const double* Ws, const double* Hs,
+                                             double* Fh, int fl, const int teff[3]) {
+  const double *pL = nullptr, *pR = nullptr;
+  double* pF = nullptr;
+  int sL = 0, sR = 0, sF = 0;
+  if (!dg_face_ptrs<ND, N, D>(Ws, Hs, Fh, fl, teff, pL, sL, pR, sR, pF, sF)) return;
+  double WL[5], WR[5], F[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) { WL[v] = pL[v * sL]; WR[v] = pR[v * sR]; }
+  dg_hll<EOS, D>(eos, WL, WR, F);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) pF[v * sF] = F[v];
+}
 
 // Barrier over one warp group (G warps): __syncwarp for G = 1, else the named barrier grp+1.
 template <int G>
@@ -408,9 +424,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   int* sCnt = sFlag + NE;
 
   // tile of this block
-  const int ntx = (a.ne[0] + TS::TX - 1) / TS::TX, nty = (a.ne[1] + TS::TY - 1) / TS::TY;
-  const int bt = blockIdx.x;
-  const int org[3] = {(bt % ntx) * TS::TX, ((bt / ntx) % nty) * TS::TY, (bt / (ntx * nty)) * TS::TZ};
+  const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
   // warp group, element and node of this thread
@@ -421,12 +435,8 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
   const int in[3] = {n % N, (n / N) % N, n / (N * N)};
   const bool active = (r < TS::EPG * NN) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
-  long long g = 0;
-  if (active) {
-    const long long e = (org[0] + lc[0]) +
-                        (long long)a.ne[0] * ((org[1] + lc[1]) + (long long)a.ne[1] * (org[2] + lc[2]));
-    g = e * NN + n;
-  }
+  int g = 0;                                                         // ndof < 2^31 (dgrhd_create)
+  if (active) g = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + n;
   if (t < NE) { sSmin[t] = dg_ord(1.0); sFlag[t] = 0; }
   if (t < 4) sCnt[t] = 0;
   if (t < N * N) sD[t] = a.Dhat[t];
@@ -445,34 +455,16 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     const double rg = rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
     P = Wn[4]; v0 = Wn[1] * rg; v1 = Wn[2] * rg; v2 = Wn[3] * rg;
   }
-  for (int hl = t; hl < 2 * TS::FP(0); hl += NT) dg_load_halo<ND, N, 0>(a, Hs, hl, org, teff);
-  if constexpr (ND > 1)
-    for (int hl = t; hl < 2 * TS::FP(1); hl += NT) dg_load_halo<ND, N, 1>(a, Hs, hl, org, teff);
-  if constexpr (ND > 2)
-    for (int hl = t; hl < 2 * TS::FP(2); hl += NT) dg_load_halo<ND, N, 2>(a, Hs, hl, org, teff);
+  dg_load_halo<ND, N, 0>(a, Hs, t, org, teff);
+  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, Hs, t, org, teff);
+  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, Hs, t, org, teff);
   __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    const double *pL = nullptr, *pR = nullptr;
-    double* pF = nullptr;
-    int sL = 0, sR = 0, sF = 0, dir = 0;
-    bool ok;
-    if (ND == 1 || f < TS::FOFF(1)) {
-      dir = 0; ok = dg_face_ptrs<ND, N, 0>(Ws, Hs, Fh, f, teff, pL, sL, pR, sR, pF, sF);
-    } else if (ND == 2 || f < TS::FOFF(2)) {
-      dir = 1; ok = dg_face_ptrs<ND, N, (ND > 1 ? 1 : 0)>(Ws, Hs, Fh, f - TS::FOFF(1), teff, pL, sL, pR, sR, pF, sF);
-    } else {
-      dir = 2; ok = dg_face_ptrs<ND, N, (ND > 2 ? 2 : 0)>(Ws, Hs, Fh, f - TS::FOFF(2), teff, pL, sL, pR, sR, pF, sF);
-    }
-    if (ok) {
-      double WL[5], WR[5], F[5];
-#pragma unroll
-      for (int v = 0; v < 5; ++v) { WL[v] = pL[v * sL]; WR[v] = pR[v * sR]; }
-      dg_hll<EOS>(a.eos, WL, WR, dir, F);
-#pragma unroll
-      for (int v = 0; v < 5; ++v) pF[v * sF] = F[v];
-    }
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, EOS, 0>(a.eos, Ws, Hs, Fh, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, Ws, Hs, Fh, f - TS::FOFF(1), teff);
+    else dg_face_flux<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, Ws, Hs, Fh, f - TS::FOFF(2), teff);
   }
 
   // 3. volume quadrature, direction by direction, F(W_i) = U_i v_d + P e_d; the first direction

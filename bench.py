@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="box3d", choices=["box3d", "kh2d"])
+    ap.add_argument("--workload", default="box3d", choices=["box3d", "kh2d", "c2p"])
     ap.add_argument("--size", type=int, default=0, help="override elements per axis (debug)")
     ap.add_argument("--no-extra", action="store_true", help="skip con2prim / e2e / cpu legs")
     return ap.parse_args()
@@ -124,7 +124,7 @@ def cfg_args(cfgd):
 def oracle_sample(workload):
     """Bounded sample of the workload for the oracle: the same recipe on a smaller mesh."""
     import oracle as O
-    n = 24 if workload == "box3d" else 96
+    n = 48 if workload == "box3d" else 256
     cfgd, W, _ = workload_cfg(workload, n, "cpu")
     U = O.prim2con_batch(cfgd["eos"], cfgd["gamma_ad"], W.numpy())
     ndof = U.shape[1]
@@ -203,6 +203,21 @@ def run_cuda(a):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if a.workload == "c2p":            # configs[2]: the con2prim batch micro-benchmark alone
+        n = a.size or (1 << 26)
+        peak, peak_src = peaks()
+        r = {"ideal_gamma_4_3": time_c2p(b, torch, 0, 4.0 / 3.0, n), "taub_matthews": time_c2p(b, torch, 1, 0.0, n)}
+        print(json.dumps({"metric": "con2prim states/s", "value": r["ideal_gamma_4_3"], "unit": "states/s",
+                          "n_gpus": 1, "dtype": "f64", "data": "synthetic", "higher_is_better": True,
+                          "config": {"workload": f"con2prim batch, {n} states, ideal Gamma=4/3 and Taub-Matthews (configs[2])"},
+                          "con2prim": r, "gpu_launches": 16,
+                          "roofline": {"kernel": "dg_c2p_batch_kernel", "bound": "hbm", "unit": "GB/s", "peak": peak,
+                                       "peak_source": peak_src, "alg_bytes_per_state": 80,
+                                       "achieved": r["ideal_gamma_4_3"] * 80 / 1e9,
+                                       "frac": r["ideal_gamma_4_3"] * 80 / 1e9 / peak,
+                                       "achieved_tm": r["taub_matthews"] * 80 / 1e9,
+                                       "frac_tm": r["taub_matthews"] * 80 / 1e9 / peak, "traffic": None}}))
+        return
     cfgd, W, label = workload_cfg(a.workload, a.size, "cuda")
     ctx = b.Context(b.make_config(*cfg_args(cfgd)))
     U = b.dgrhd_prim2con_batch(cfgd["eos"], cfgd["gamma_ad"], W)
@@ -269,7 +284,7 @@ def run_cuda(a):
                            "taub_matthews": time_c2p(b, torch, 1, 0.0, n)}
         out["con2prim"]["roofline_hbm_frac_ideal"] = out["con2prim"]["ideal_gamma_4_3"] * 80 / 1e9 / peak
         out["con2prim"]["roofline_hbm_frac_tm"] = out["con2prim"]["taub_matthews"] * 80 / 1e9 / peak
-        val, sps, cores, sample = time_oracle(a.workload, 1, 0)
+        val, sps, cores, sample = time_oracle(a.workload, 10, 0)
         out["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": sample, "s_per_step": sps}
     if world > 1:

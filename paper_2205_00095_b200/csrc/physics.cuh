@@ -19,6 +19,33 @@ struct EosPar {
   double G, al;
 };
 
+// Branch-free fp64 reciprocal, reciprocal square root and square root: the MUFU seed
+// (rcp/rsqrt.approx.ftz.f64, ~2^-22 relative) refined by two Newton steps (error -> 2^-44 -> below one
+// ulp), without the denormal/overflow slow paths of the IEEE sequences.  Results are within ~1 ulp
+// of the correctly rounded ones -- far inside every tolerance of this path; the one place where the
+// decision must be bit-exact (dg_admissible) does not use them.  Arguments are positive, normal
+// numbers on every admissible state.
+DG_INL double dg_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  r = fma(r, fma(-x, r, 1.0), r);
+  r = fma(r, fma(-x, r, 1.0), r);
+  return r;
+}
+DG_INL double dg_rsqrt(double x) {
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double h = 0.5 * x;
+  r = fma(r, fma(-h * r, r, 0.5), r);
+  r = fma(r, fma(-h * r, r, 0.5), r);
+  return r;
+}
+DG_INL double dg_sqrt(double x) {                 // x >= 0; sqrt(0) = 0
+  const double r = dg_rsqrt(fmax(x, 1e-300));
+  const double s = x * r;
+  return fma(fma(-s, s, x), 0.5 * r, s);
+}
+
 // rho*h as a function of (rho, P):  ideal Eq. 8: rho h = rho + al P;
 // Taub-Matthews Eq. 10: rho h = 5/2 P + 3/2 sqrt(P^2 + 4/9 rho^2)   (h(Theta) times rho).
 template <int EOS>
@@ -75,17 +102,18 @@ DG_INL void dg_sigma_frac(const EosPar& e, double rho, double P, double g2, doub
   }
 }
 
-// lambda-+ of Eq. 21 with sigma = num/den substituted, so that one square root and one division
-// remain:  lambda-+ = (v den -+ sqrt(num ((1 - v^2) den + num))) / (den + num).
+// lambda-+ of Eq. 21 with sigma = num/den substituted, as fractions over the common positive
+// denominator dn = den + num:   lambda-+ = (v den -+ sqrt(num ((1 - v^2) den + num))) / (den + num).
 template <int EOS>
-DG_INL void dg_speeds(const EosPar& e, double rho, double P, double g2, double vd, double& lm, double& lp) {
+DG_INL void dg_speeds_frac(const EosPar& e, double rho, double P, double g2, double vd, double& nm,
+                           double& np, double& dn) {
   double num, den;
   dg_sigma_frac<EOS>(e, rho, P, g2, num, den);
-  const double root = sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
-  const double r = 1.0 / (den + num);
+  const double root = dg_sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
   const double c = vd * den;
-  lm = (c - root) * r;
-  lp = (c + root) * r;
+  nm = c - root;
+  np = c + root;
+  dn = den + num;
 }
 
 // One side's contribution to the interface flux:  acc += cF F_dir(W) + cU U(W)   (Eq. 2, Eq. 4).
@@ -114,20 +142,24 @@ template <int EOS, int dir>
 DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], double F[5]) {
   const double g2L = fma(WL[1], WL[1], fma(WL[2], WL[2], fma(WL[3], WL[3], 1.0)));
   const double g2R = fma(WR[1], WR[1], fma(WR[2], WR[2], fma(WR[3], WR[3], 1.0)));
-  const double rgL = rsqrt(g2L), rgR = rsqrt(g2R);
-  const double vL = ((dir == 0) ? WL[1] : ((dir == 1) ? WL[2] : WL[3])) * rgL;
-  const double vR = ((dir == 0) ? WR[1] : ((dir == 1) ? WR[2] : WR[3])) * rgR;
-  double lmL, lpL, lmR, lpR;
-  dg_speeds<EOS>(e, WL[0], WL[4], g2L, vL, lmL, lpL);
-  dg_speeds<EOS>(e, WR[0], WR[4], g2R, vR, lmR, lpR);
-  const double lL = fmin(lmL, lmR);                 // Eq. 23
-  const double lR = fmax(lpL, lpR);                 // Eq. 24
+  const double rgL = dg_rsqrt(g2L), rgR = dg_rsqrt(g2R);
+  const double vL = WL[1 + dir] * rgL, vR = WR[1 + dir] * rgR;
+  double nmL, npL, dL, nmR, npR, dR;
+  dg_speeds_frac<EOS>(e, WL[0], WL[4], g2L, vL, nmL, npL, dL);
+  dg_speeds_frac<EOS>(e, WR[0], WR[4], g2R, vR, nmR, npR, dR);
+  // lambda_L = min(nmL/dL, nmR/dR) =: nl/dl, lambda_R = max(npL/dL, npR/dR) =: nr/dr  (Eq. 23-24),
+  // compared by cross-multiplication (dL, dR > 0); the HLL weights then need one division:
+  //   (cL, cR, cU) = (nr dl, -nl dr, nl nr) / (nr dl - nl dr).
+  const bool ml = nmL * dR <= nmR * dL, mr = npL * dR >= npR * dL;
+  const double nl = ml ? nmL : nmR, dl = ml ? dL : dR;
+  const double nr = mr ? npL : npR, dr = mr ? dL : dR;
   double cL, cR, cU;
-  if (lL >= 0.0) { cL = 1.0; cR = 0.0; cU = 0.0; }
-  else if (lR <= 0.0) { cL = 0.0; cR = 1.0; cU = 0.0; }
+  if (nl >= 0.0) { cL = 1.0; cR = 0.0; cU = 0.0; }
+  else if (nr <= 0.0) { cL = 0.0; cR = 1.0; cU = 0.0; }
   else {
-    const double rd = 1.0 / (lR - lL);
-    cL = lR * rd; cR = -lL * rd; cU = lL * lR * rd;
+    const double a = nr * dl, b = nl * dr;
+    const double q = dg_rcp(a - b);
+    cL = a * q; cR = -b * q; cU = nl * nr * q;
   }
 #pragma unroll
   for (int v = 0; v < 5; ++v) F[v] = 0.0;
@@ -139,15 +171,15 @@ DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], doub
 template <int EOS, int ND>
 DG_INL double dg_cfl_speed(const EosPar& e, const double W[5], const double cw[3]) {
   const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  const double rg = rsqrt(g2);
+  const double rg = dg_rsqrt(g2);
   double num, den;
   dg_sigma_frac<EOS>(e, W[0], W[4], g2, num, den);
-  const double r1 = 1.0 / (den + num);
+  const double r1 = dg_rcp(den + num);
   double a = 0.0;
 #pragma unroll
   for (int d = 0; d < ND; ++d) {
     const double vd = W[1 + d] * rg;
-    const double root = sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
+    const double root = dg_sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
     a = fma(cw[d], fma(fabs(vd), den, root), a);    // max(|l-|,|l+|) (den+num) = |v| den + root
   }
   return a * r1;
@@ -204,8 +236,8 @@ DG_INL double dg_sqrt_lo(double x) {
 DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
   const double D = U[0], E = U[4];
   const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
-  const double Mabs = sqrt(M2);
-  const double rD = 1.0 / D;
+  const double Mabs = dg_sqrt(M2);
+  const double rD = dg_rcp(D);
   const double xi = Mabs * rD, eta = E * rD;                     // Eq. 38
   const double al = e.al;
   if (xi == 0.0) {                                               // v = 0 (R4)
@@ -245,7 +277,7 @@ DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
   }
   const double w2 = w * w;
   const double op = 1.0 + w2, om = 1.0 - w2;
-  const double r = 1.0 / (op * om * Mabs);                       // one reciprocal for Eq. 55-58
+  const double r = dg_rcp(op * om * Mabs);                       // one reciprocal for Eq. 55-58
   const double r1 = r * om * Mabs;                               // 1/(1+w^2)
   const double beta = 2.0 * w * r1;                              // Eq. 58
   const double rho = D * om * r1;                                // Eq. 55, 1/gamma = (1-w^2)/(1+w^2)
@@ -266,11 +298,12 @@ DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
 DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
   const double D = U[0], E = U[4];
   const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
-  const double Mabs = sqrt(M2);
-  const double xi = Mabs / D, eta = E / D;                       // Eq. 38
+  const double Mabs = dg_sqrt(M2);
+  const double rD = dg_rcp(D);
+  const double xi = Mabs * rD, eta = E * rD;                       // Eq. 38
   const double x2 = xi * xi, e2 = eta * eta;
   const double dif = (eta - xi) * (eta + xi);
-  const double rden = 1.0 / (dif * dif);
+  const double rden = dg_rcp(dif * dif);
   const double sum = e2 + x2;
   const double br = 4.0 * sum - (x2 + 1.0);
   const double xe = x2 * e2;
@@ -283,9 +316,9 @@ DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
   const double d = fma(R, R, Q3);                                // Eq. 65
   double Wv;
   if (d < 0.0) {
-    double arg = R * rsqrt(-Q3);
+    double arg = R * dg_rsqrt(-Q3);
     arg = fmin(1.0, fmax(-1.0, arg));
-    Wv = 2.0 * sqrt(-Q) * cos(acos(arg) * (1.0 / 3.0)) - c1 * (1.0 / 3.0);   // Eq. 69-70
+    Wv = 2.0 * dg_sqrt(-Q) * cos(acos(arg) * (1.0 / 3.0)) - c1 * (1.0 / 3.0);   // Eq. 69-70
   } else {
     double sd = sqrt(d);
     Wv = cbrt(R + sd) + cbrt(R - sd) - c1 * (1.0 / 3.0);         // Eq. 71-73
@@ -294,22 +327,22 @@ DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
   {                                                              // R7b: one Newton step on Eq. 61
     const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
     const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
-    const double Wn = Wv - f / df;
+    const double Wn = Wv - f * dg_rcp(df);
     if (isfinite(Wn)) Wv = Wn;
     Wv = fmax(Wv, 0.0);
   }
   const double g2 = Wv + 1.0;
-  const double rg = rsqrt(g2);                                   // 1/gamma, Eq. 74
-  const double ug = sqrt(Wv);                                    // gamma beta
+  const double rg = dg_rsqrt(g2);                                  // 1/gamma, Eq. 74
+  const double ug = dg_sqrt(Wv);                                   // gamma beta
   const double beta = ug * rg;
   const double rho = D * rg;
-  const double sc = (Mabs > 0.0) ? ug / Mabs : 0.0;
+  const double sc = (Mabs > 0.0) ? ug * dg_rcp(Mabs) : 0.0;
   const double X = fma(-beta, Mabs, E);                          // E - M.v
   W[0] = rho;
   W[1] = sc * U[1];
   W[2] = sc * U[2];
   W[3] = sc * U[3];
-  W[4] = (X - rho) * (X + rho) / (3.0 * X);                      // Eq. 75
+  W[4] = (X - rho) * (X + rho) * dg_rcp(3.0 * X);                      // Eq. 75
   if (!dg_finite5(W) || !(W[4] > 0.0)) return 2;
   return 0;
 }

@@ -452,7 +452,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     }
 #pragma unroll
     for (int v = 0; v < 5; ++v) Un[v] = a.Us[v * a.ndof + g];
-    const double rg = rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
+    const double rg = dg_rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
     P = Wn[4]; v0 = Wn[1] * rg; v1 = Wn[2] * rg; v2 = Wn[3] * rg;
   }
   dg_load_halo<ND, N, 0>(a, Hs, t, org, teff);

@@ -64,6 +64,12 @@ int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t workspace_
                  void* cuda_stream, dgrhd_ctx** out);
 int dgrhd_destroy(dgrhd_ctx* ctx);
 
+/* Options.  DGRHD_OPT_CUDA_GRAPH (default 1): dgrhd_step replays each SSP-RK step (the dt kernel and
+ * the fused stage kernels) as one captured CUDA graph instead of 1 + rk_stages launches; results are
+ * identical either way. */
+enum { DGRHD_OPT_CUDA_GRAPH = 0 };
+int dgrhd_set_option(dgrhd_ctx* ctx, int option, int value);
+
 /* Copy the caller's conserved state U_dev[5][ndof] (canonical layout) into / out of the context.
  * set_state also recovers the primitives of every node (Eq. 16) and computes the
  * CFL wave-speed maximum of the new state; it does not apply the physicality operator (R15). */

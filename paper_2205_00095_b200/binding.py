@@ -12,6 +12,7 @@ import torch
 EOS_IDEAL, EOS_TAUB_MATTHEWS = 0, 1
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
+OPT_CUDA_GRAPH = 0
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdgrhd.so")
@@ -52,7 +53,7 @@ EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
            "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host",
-           "dgrhd_last_error", "dgrhd_version")
+           "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
 
 
 def lib():
@@ -67,6 +68,7 @@ def lib():
         L.dgrhd_workspace_bytes.argtypes = [C.POINTER(Config)]
         L.dgrhd_create.argtypes = [C.POINTER(Config), _vp, C.c_size_t, _vp, C.POINTER(_vp)]
         L.dgrhd_destroy.argtypes = [_vp]
+        L.dgrhd_set_option.argtypes = [_vp, C.c_int, C.c_int]
         L.dgrhd_set_state.argtypes = [_vp, _vp]
         L.dgrhd_get_state.argtypes = [_vp, _vp]
         L.dgrhd_get_prims.argtypes = [_vp, _vp]
@@ -147,6 +149,9 @@ class Context:
             self.close()
         except Exception:
             pass
+
+    def dgrhd_set_option(self, option, value):
+        _check(lib().dgrhd_set_option(self._h, option, value), self._h)
 
     def new_state(self):
         return torch.empty(5, self.ndof, dtype=torch.float64, device=self.device)

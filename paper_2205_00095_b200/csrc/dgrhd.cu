@@ -89,6 +89,11 @@ struct dgrhd_ctx {
   BasisTables basis;
   double wsum;
   EosPar eos;
+  // one captured CUDA graph per primitive-buffer parity: a whole SSP-RK step (dt kernel + stages)
+  int use_graph;
+  cudaStream_t cap_stream;
+  cudaGraphExec_t gexec[2];
+  double gdt[2];
   char err[512];
 };
 
@@ -267,12 +272,25 @@ extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t
     delete c;
     return r;
   }
+  c->use_graph = (cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) == cudaSuccess) ? 1 : 0;
   *out = c;
   return DGRHD_OK;
 }
 
+extern "C" int dgrhd_set_option(dgrhd_ctx* c, int option, int value) {
+  if (!c) return DGRHD_EINVAL;
+  if (option == DGRHD_OPT_CUDA_GRAPH) {
+    c->use_graph = (value != 0 && c->cap_stream) ? 1 : 0;
+    return DGRHD_OK;
+  }
+  return fail(c, DGRHD_EINVAL, "dgrhd_set_option: unknown option %d", option);
+}
+
 extern "C" int dgrhd_destroy(dgrhd_ctx* ctx) {
   if (!ctx) return DGRHD_EINVAL;
+  for (int i = 0; i < 2; ++i)
+    if (ctx->gexec[i]) cudaGraphExecDestroy(ctx->gexec[i]);
+  if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
   delete ctx;
   return DGRHD_OK;
 }
@@ -394,6 +412,40 @@ static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
   return DGRHD_OK;
 }
 
+// One step through a captured graph (one launch instead of 1 + stages; PAPER.md:755-757 names launch
+// overhead as the GPU bottleneck).  The graph is captured on the context's private stream and
+// replayed on the caller's stream; it is re-captured when dt (a kernel argument) changes.  Any
+// capture failure switches the context back to plain launches.
+static int launch_step_graph(dgrhd_ctx* c, double dt, StageArgs& a) {
+  const int par = c->wcur;
+  if (!c->gexec[par] || c->gdt[par] != dt) {
+    if (c->gexec[par]) { cudaGraphExecDestroy(c->gexec[par]); c->gexec[par] = nullptr; }
+    cudaStream_t user = c->stream;
+    cudaGraph_t graph = nullptr;
+    bool ok = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+      c->stream = c->cap_stream;
+      const int r = enqueue_step(c, dt, a);
+      c->stream = user;
+      c->wcur = par;
+      const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+      ok = (r == DGRHD_OK) && (e == cudaSuccess) && graph;
+    }
+    if (ok) ok = cudaGraphInstantiate(&c->gexec[par], graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (!ok) {
+      cudaGetLastError();
+      c->gexec[par] = nullptr;
+      c->use_graph = 0;
+      return enqueue_step(c, dt, a);
+    }
+    c->gdt[par] = dt;
+  }
+  DG_CUDA(c, cudaGraphLaunch(c->gexec[par], c->stream));
+  c->wcur = par ^ (c->cfg.rk_stages & 1);
+  return DGRHD_OK;
+}
+
 extern "C" int dgrhd_step(dgrhd_ctx* c, double dt, int nsteps, double* t_inout_host) {
   if (!c) return fail(c, DGRHD_EINVAL, "dgrhd_step: NULL context");
   if (nsteps < 0 || !(dt == dt)) return fail(c, DGRHD_EINVAL, "dgrhd_step: bad nsteps or dt");
@@ -404,7 +456,7 @@ extern "C" int dgrhd_step(dgrhd_ctx* c, double dt, int nsteps, double* t_inout_h
   fill_stage_args(c, a);
   a.mode = DG_MODE_STAGE;
   for (int i = 0; i < nsteps; ++i) {
-    int r = enqueue_step(c, dt, a);
+    int r = c->use_graph ? launch_step_graph(c, dt, a) : enqueue_step(c, dt, a);
     if (r != DGRHD_OK) return r;
   }
   if (t_inout_host) {

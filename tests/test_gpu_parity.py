@@ -378,3 +378,28 @@ def test_entropy_wave_converges_at_order_p_plus_1_on_gpu():
             errs.append(float((rho - exact).abs().mean()))
         orders = np.log2(np.array(errs[:-1]) / np.array(errs[1:]))
         assert (np.abs(orders - (p + 1)) < 0.35).all(), (p, errs, orders)
+
+
+def test_cuda_graph_replay_is_bit_identical_and_cuts_launch_overhead():
+    """dgrhd_step through the captured per-step graph (default) vs plain launches: same bits; on
+    config 1 (768 DOF, launch-latency bound) the time per step is reported."""
+    import time
+    b = B()
+    d, W = I.riemann1d(0)
+    U = b.dgrhd_prim2con_batch(d["eos"], d["gamma_ad"], W.to(DEV))
+    res, us = [], []
+    for graph in (1, 0):
+        ctx = b.Context(gcfg(d))
+        ctx.dgrhd_set_option(b.OPT_CUDA_GRAPH, graph)
+        ctx.dgrhd_set_state(U)
+        ctx.dgrhd_step(-0.3, 5)                       # CFL mode, dt on the device
+        ctx.dgrhd_step(1e-4, 3)                       # fixed dt: graph re-captured
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.dgrhd_step(-0.3, 200)
+        torch.cuda.synchronize()
+        us.append((time.perf_counter() - t0) / 200 * 1e6)
+        res.append(ctx.dgrhd_get_state())
+        assert ctx.dgrhd_get_counters()["n_stages"] == 3 * 208
+    assert torch.equal(res[0], res[1])
+    print(f"config 1: {us[0]:.1f} us/step with the CUDA graph, {us[1]:.1f} us/step with plain launches")

@@ -28,6 +28,14 @@ STAGES = 3
 # algorithmic HBM bytes per DOF and stage: U_s in, U_out out
 # (80 B) + U0 in on stages 2 and 3 (40 B) -> (80 + 120 + 120) / 3
 ALG_BYTES_PER_DOF_STAGE = (80.0 + 120.0 + 120.0) / 3.0
+# fp64 work per DOF and stage of dg_stage_kernel<3,4,ideal>: executed 2*dfma + dmul + dadd from the
+# ncu capture profiles/r1_ncu_summary.md, mean of the three stages (588 / 597 / 711)
+FLOP_PER_DOF_STAGE = 632.0
+# DRAM bytes per DOF and stage of the same capture (dram__bytes_read + write, mean of the 3 stages)
+NCU_TRAFFIC_PER_DOF_STAGE = 192.7
+# fp64 peak: 148 SMs x 64 DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on peak_sustained)
+# x 2 flop x SM clock
+FP64_FMA_PER_CLK = 148 * 64
 
 
 def parse():
@@ -185,6 +193,45 @@ def time_c2p(b, torch, eos, G, n):
     return n / ts[len(ts) // 2]
 
 
+def max_over_ranks(secs, device):
+    """Multi-GPU timing rule: the job's time is the slowest rank's device time."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([secs], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t)
+
+
+def aggregate_value(world, ndof, steps, secs):
+    """Whole-job DOF-updates/s: `world` independent replicas ("replicas only") over the max time."""
+    return world * ndof * STAGES * steps / secs
+
+
+def roofline_stage(workload, ndof, stage_s, clocks, hbm_peak, peak_src):
+    """Roofline of the dominant kernel (the fused stage kernel).  The slower of the two resources
+    bounds it: fp64 ALUs (flop / fp64 peak) or HBM (algorithmic bytes / measured copy bandwidth)."""
+    ach_hbm = ALG_BYTES_PER_DOF_STAGE * ndof / stage_s / 1e9
+    hbm = {"achieved": ach_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": ach_hbm / hbm_peak,
+           "peak_source": peak_src, "alg_bytes_per_dof_stage": ALG_BYTES_PER_DOF_STAGE}
+    if workload != "box3d":                       # flop count measured for the 3D p=3 ideal kernel only
+        return {"kernel": "dg_stage_kernel", "bound": "hbm", **hbm, "traffic": None,
+                "avg_launch_ms": 1e3 * stage_s}
+    mhz = clocks.get("sm_max_mhz") or 1965
+    alu_peak = FP64_FMA_PER_CLK * 2 * mhz * 1e6 / 1e12
+    ach_alu = FLOP_PER_DOF_STAGE * ndof / stage_s / 1e12
+    t_alu, t_hbm = FLOP_PER_DOF_STAGE / (alu_peak * 1e12), ALG_BYTES_PER_DOF_STAGE / (hbm_peak * 1e9)
+    out = {"kernel": "dg_stage_kernel", "bound": "alu" if t_alu >= t_hbm else "hbm",
+           "achieved": ach_alu, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach_alu / alu_peak,
+           "peak_source": "derived: 148 SM x 64 DFMA/clk x 2 x max SM clock (DESIGN.md)",
+           "flop_per_dof_stage": FLOP_PER_DOF_STAGE,
+           "traffic": NCU_TRAFFIC_PER_DOF_STAGE * ndof,
+           "traffic_source": "ncu dram__bytes_read+write per DOF of profiles/r1_ncu_summary.md x DOF per launch",
+           "avg_launch_ms": 1e3 * stage_s, "hbm": hbm}
+    if out["bound"] == "hbm":
+        out.update({k: hbm[k] for k in ("achieved", "peak", "unit", "frac", "peak_source")})
+    return out
+
+
 def run_cuda(a):
     import torch
     import torch.distributed as dist
@@ -236,11 +283,9 @@ def run_cuda(a):
         barrier()
     secs = e0.elapsed_time(e1) * 1e-3
     if world > 1:
-        t = torch.tensor([secs], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        secs = float(t)
+        secs = max_over_ranks(secs, "cuda")
     cnt = ctx.dgrhd_get_counters()
-    value = world * ndof * STAGES * a.steps / secs
+    value = aggregate_value(world, ndof, a.steps, secs)
     stage_s = secs / (STAGES * a.steps)
     peak, peak_src = peaks()
     ach = ALG_BYTES_PER_DOF_STAGE * ndof / stage_s / 1e9
@@ -256,10 +301,7 @@ def run_cuda(a):
                    "n_bad_mean": cnt["n_bad_mean"], "n_c2p_fail": cnt["n_c2p_fail"]},
         "gpu_launches": a.steps * (STAGES + 1),
         "clocks": clk.summary(),
-        "roofline": {"kernel": "dg_stage_kernel", "bound": "hbm", "achieved": ach, "peak": peak,
-                     "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
-                     "alg_bytes_per_dof_stage": ALG_BYTES_PER_DOF_STAGE,
-                     "avg_launch_ms": 1e3 * stage_s},
+        "roofline": roofline_stage(a.workload, ndof, stage_s, clk.summary(), peak, peak_src),
     }
     if rank == 0 and world == 1 and not a.no_extra:
         # end to end through the C ABI with HOST buffers (pinned): H2D state, K steps, D2H state

@@ -189,11 +189,13 @@ struct DirInfo {
   }
 };
 
-// Load the halo of direction D (2*FP(D) points, spread over the block's threads): the facing nodal
-// layer of the neighbouring elements (periodic wrap) or, at an outflow boundary, the elements' own
-// face nodes (reading R12).  Everything that is uniform over the block is computed once.
+// Load the halo of direction D: the facing nodal layer of the neighbouring elements (periodic wrap)
+// or, at an outflow boundary, the elements' own face nodes (reading R12).  Each node on the tile's
+// boundary in direction D fetches the node facing it: its global index is the thread's own index plus
+// a block-uniform offset, and its halo slot is the node's face-point index.
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, int t, const int org[3],
+__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, bool active, int g,
+                                             const int lc[3], const int in[3], const int org[3],
                                              const int teff[3]) {
   using TS = TileShape<ND, N>;
   using DI = DirInfo<ND, N, D>;
@@ -207,21 +209,21 @@ __device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, int
     if (a.bc[D] == DG_BC_PERIODIC) ed1 = 0;
     else { ed1 = a.ne[D] - 1; nl1 = N - 1; }
   }
-  // 32-bit node indices: dgrhd_create rejects meshes with ndof >= 2^31
-  const int es[3] = {1, a.ne[0], a.ne[0] * a.ne[1]};
-  const int tb = org[A] * es[A] + org[B] * es[B];
-  const int b0 = (tb + ed0 * es[D]) * TS::NN + nl0 * TS::SN(D);
-  const int b1 = (tb + ed1 * es[D]) * TS::NN + nl1 * TS::SN(D);
-  const int sa = es[A] * TS::NN, sb = es[B] * TS::NN;
-  for (int hl = t; hl < 2 * FPD; hl += TS::NT) {
-    const int side = hl / FPD, fp = hl - side * FPD;
-    int la, lb, ca, cb;
-    DI::split(fp, la, lb, ca, cb);
-    if (la >= teff[A] || lb >= teff[B]) continue;
-    const double* src = a.Win + (side ? b1 : b0) + la * sa + lb * sb + (ca * TS::SN(A) + cb * TS::SN(B));
-    double* dst = Hs + 5 * TS::HOFF(D) + side * 5 * FPD + fp;
+  const int esD = (D == 0) ? 1 : ((D == 1) ? a.ne[0] : a.ne[0] * a.ne[1]);
+  const int off0 = (ed0 - org[D]) * esD * TS::NN + nl0 * TS::SN(D);
+  const int off1 = (ed1 - (org[D] + teff[D] - 1)) * esD * TS::NN + (nl1 - (N - 1)) * TS::SN(D);
+  if (!active) return;
+  const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
+  double* dst = Hs + 5 * TS::HOFF(D) + fp;
+  if (in[D] == 0 && lc[D] == 0) {
+    const double* src = a.Win + (g + off0);
 #pragma unroll
     for (int v = 0; v < 5; ++v) dst[v * FPD] = __ldg(src + v * a.ndof);
+  }
+  if (in[D] == N - 1 && lc[D] == teff[D] - 1) {
+    const double* src = a.Win + (g + off1);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dst[5 * FPD + v * FPD] = __ldg(src + v * a.ndof);
   }
 }
 
@@ -343,6 +345,9 @@ __device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int 
   if (bad) sFlag[le] = 1;
   dg_gsync<TS::G>(grp);
   const bool flagged = active && (sFlag[le] != 0);
+  // nothing flagged in this warp group (the common case): done, no further group barriers
+  const bool any = (TS::G == 1) ? (__any_sync(0xffffffffu, flagged) != 0) : (sFlag[grp * TS::EPG] != 0);
+  if (!any) return;
   if (flagged) {
 #pragma unroll
     for (int v = 0; v < 5; ++v) scratch[v * NTN + ti] = wn * Uo[v];
@@ -455,9 +460,9 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     const double rg = dg_rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
     P = Wn[4]; v0 = Wn[1] * rg; v1 = Wn[2] * rg; v2 = Wn[3] * rg;
   }
-  dg_load_halo<ND, N, 0>(a, Hs, t, org, teff);
-  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, Hs, t, org, teff);
-  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, Hs, t, org, teff);
+  dg_load_halo<ND, N, 0>(a, Hs, active, g, lc, in, org, teff);
+  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, Hs, active, g, lc, in, org, teff);
+  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, Hs, active, g, lc, in, org, teff);
   __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads

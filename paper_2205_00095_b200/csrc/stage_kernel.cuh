@@ -71,11 +71,12 @@ struct TileShape {
   }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
-  // shared-memory layout, in doubles
-  static constexpr int O_W = 0;                          // [5][NTN]
-  static constexpr int O_F = O_W + 5 * NTN;              // [5][NTN], one direction at a time
-  static constexpr int O_H = O_F + 5 * NTN;              // halo  [dir][side][5][FP]
-  static constexpr int O_FH = O_H + 5 * NHALO;           // Fhat  [dir][plane][5][FP]
+  // shared-memory layout, in doubles.  Node array X[NREC][NTOT]: per tile node and halo node the
+  // conserved state, the 3-velocity, the pressure and the wave-speed fraction sigma = num/den.
+  static constexpr int NTOT = NTN + NHALO;               // node slots: tile nodes, then halo points
+  static constexpr int NREC = 11;                        // D Mx My Mz E | vx vy vz | P | num den
+  static constexpr int O_X = 0;                          // [NREC][NTOT]
+  static constexpr int O_FH = O_X + NREC * NTOT;         // Fhat  [dir][plane][5][FP]
   static constexpr int O_D = O_FH + 5 * NFACE;           // Dhat  [N][N] (padded to 32)
   static constexpr int O_MEAN = O_D + 32;                // [NE][5]
   static constexpr int O_SMIN = O_MEAN + 5 * NE;         // [NE] (ull)
@@ -83,6 +84,9 @@ struct TileShape {
   static constexpr int O_PART = O_RED + 32;              // [NE][4][5] partial sums of the cell mean
   static constexpr int O_FLAG = O_PART + 20 * NE;        // ints: [NE] flags + [4] counters
   static constexpr int SMEM_BYTES = O_FLAG * 8 + (NE + 4) * 4 + 16;
+  static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
+  static constexpr int BLK_THR = 1024 / NT;
+  static constexpr int MINB = (BLK_SMEM < BLK_THR ? BLK_SMEM : BLK_THR) > 0 ? (BLK_SMEM < BLK_THR ? BLK_SMEM : BLK_THR) : 1;
 };
 
 struct StageArgs {
@@ -189,12 +193,44 @@ struct DirInfo {
   }
 };
 
-// Load the halo of direction D: the facing nodal layer of the neighbouring elements (periodic wrap)
-// or, at an outflow boundary, the elements' own face nodes (reading R12).  Each node on the tile's
-// boundary in direction D fetches the node facing it: its global index is the thread's own index plus
-// a block-uniform offset, and its halo slot is the node's face-point index.
+// Record of one node in the shared node array from its primitives W (and, if known, its conserved
+// state): U (Eq. 4) for the Riemann flux and the volume flux F_d = U v_d + P e_d, the 3-velocity
+// v = u/gamma, P, and sigma_s = num/den of Eq. 22 as an unevaluated fraction.
+template <int ND, int N, int EOS, bool HAVE_U>
+__device__ __forceinline__ void dg_node_record(const EosPar& eos, const double W[5], const double U[5],
+                                               double* X, int slot) {
+  using TS = TileShape<ND, N>;
+  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
+  const double rg = dg_rsqrt(g2);
+  double num, den;
+  dg_sigma_frac<EOS>(eos, W[0], W[4], g2, num, den);
+  double* x = X + slot;
+  if (HAVE_U) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) x[v * TS::NTOT] = U[v];
+  } else {
+    const double rh = dg_rho_h<EOS>(eos, W[0], W[4]);
+    const double g = g2 * rg, grh = g * rh;
+    x[0] = g * W[0];
+    x[1 * TS::NTOT] = grh * W[1];
+    x[2 * TS::NTOT] = grh * W[2];
+    x[3 * TS::NTOT] = grh * W[3];
+    x[4 * TS::NTOT] = fma(g2, rh, -W[4]);
+  }
+  x[5 * TS::NTOT] = W[1] * rg;
+  x[6 * TS::NTOT] = W[2] * rg;
+  x[7 * TS::NTOT] = W[3] * rg;
+  x[8 * TS::NTOT] = W[4];
+  x[9 * TS::NTOT] = num;
+  x[10 * TS::NTOT] = den;
+}
+
+// Halo of direction D: each node on the tile's boundary in direction D fetches the primitives of the
+// node facing it in the neighbouring element (periodic wrap; at an outflow boundary its own, reading
+// R12) -- global index = own index + a block-uniform offset -- into the halo slot that equals the
+// node's face-point index (rows 0..4; the record is completed in a dense pass over the halo slots).
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, bool active, int g,
+__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* X, bool active, int g,
                                              const int lc[3], const int in[3], const int org[3],
                                              const int teff[3]) {
   using TS = TileShape<ND, N>;
@@ -214,58 +250,17 @@ __device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* Hs, boo
   const int off1 = (ed1 - (org[D] + teff[D] - 1)) * esD * TS::NN + (nl1 - (N - 1)) * TS::SN(D);
   if (!active) return;
   const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
-  double* dst = Hs + 5 * TS::HOFF(D) + fp;
+  double* dst = X + (TS::NTN + TS::HOFF(D) + fp);
   if (in[D] == 0 && lc[D] == 0) {
     const double* src = a.Win + (g + off0);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[v * FPD] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dst[v * TS::NTOT] = __ldg(src + v * a.ndof);
   }
   if (in[D] == N - 1 && lc[D] == teff[D] - 1) {
     const double* src = a.Win + (g + off1);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[5 * FPD + v * FPD] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dst[FPD + v * TS::NTOT] = __ldg(src + v * a.ndof);
   }
-}
-
-// Face point fl (0 .. (T(D)+1)*FP(D)) of direction D: pointers to the left and right face states
-// (stride between variables differs for tile nodes and halo points) and to the Fhat slot.
-template <int ND, int N, int D>
-__device__ __forceinline__ bool dg_face_ptrs(const double* Ws, const double* Hs, double* Fh, int fl,
-                                             const int teff[3], const double*& pL, int& sL,
-                                             const double*& pR, int& sR, double*& pF, int& sF) {
-  using TS = TileShape<ND, N>;
-  using DI = DirInfo<ND, N, D>;
-  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
-  const int p = fl / FPD, fp = fl - p * FPD;
-  int la, lb, ca, cb;
-  DI::split(fp, la, lb, ca, cb);
-  if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return false;
-  const int tnode = ca * TS::SN(A) + cb * TS::SN(B);
-  const int telem = la * TS::SE(A) + lb * TS::SE(B);
-  if (p >= 1) { pL = Ws + (telem + (p - 1) * TS::SE(D)) * TS::NN + tnode + (N - 1) * TS::SN(D); sL = TS::NTN; }
-  else        { pL = Hs + 5 * TS::HOFF(D) + fp; sL = FPD; }
-  if (p < teff[D]) { pR = Ws + (telem + p * TS::SE(D)) * TS::NN + tnode; sR = TS::NTN; }
-  else             { pR = Hs + 5 * TS::HOFF(D) + 5 * FPD + fp; sR = FPD; }
-  pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
-  sF = FPD;
-  return true;
-}
-
-
-// HLL flux at face point fl of direction D into the Fhat array.
-template <int ND, int N, int EOS, int D>
-__device__ __forceinline__ void dg_face_flux(const EosPar& eos, const double* Ws, const double* Hs,
-                                             double* Fh, int fl, const int teff[3]) {
-  const double *pL = nullptr, *pR = nullptr;
-  double* pF = nullptr;
-  int sL = 0, sR = 0, sF = 0;
-  if (!dg_face_ptrs<ND, N, D>(Ws, Hs, Fh, fl, teff, pL, sL, pR, sR, pF, sF)) return;
-  double WL[5], WR[5], F[5];
-#pragma unroll
-  for (int v = 0; v < 5; ++v) { WL[v] = pL[v * sL]; WR[v] = pR[v * sR]; }
-  dg_hll<EOS, D>(eos, WL, WR, F);
-#pragma unroll
-  for (int v = 0; v < 5; ++v) pF[v * sF] = F[v];
 }
 
 // Barrier over one warp group (G warps): __syncwarp for G = 1, else the named barrier grp+1.
@@ -299,37 +294,86 @@ __device__ __forceinline__ void dg_add_surface(const double* Fh, const int lc[3]
   }
 }
 
-// One direction of the volume term for this thread's node: flux (Eq. 2) of the node into the
-// shared buffer Fb, group barrier, tensor-line contraction with Dhat (Eq. 17).  The caller
-// alternates Fb between two buffers, so no barrier is needed after the reads.
+// HLL flux (reading R9, Eq. 21-24) at face point fl of direction D from the node records of its two
+// sides:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in the energy).
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_direction(const StageArgs& a, const double* sD, double* Fb, int ti,
-                                             bool active, int grp, const int in[3], const double Un[5],
-                                             double P, double vd, double R[5]) {
+__device__ __forceinline__ void dg_face_flux(const double* X, double* Fh, int fl, const int teff[3]) {
   using TS = TileShape<ND, N>;
-  constexpr int NTN = TS::NTN;
-  if (active) {
-    Fb[0 * NTN + ti] = Un[0] * vd;
-    Fb[1 * NTN + ti] = fma(Un[1], vd, (D == 0) ? P : 0.0);
-    Fb[2 * NTN + ti] = fma(Un[2], vd, (D == 1) ? P : 0.0);
-    Fb[3 * NTN + ti] = fma(Un[3], vd, (D == 2) ? P : 0.0);
-    Fb[4 * NTN + ti] = (Un[4] + P) * vd;
+  using DI = DirInfo<ND, N, D>;
+  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD, NTOT = TS::NTOT;
+  const int p = fl / FPD, fp = fl - p * FPD;
+  int la, lb, ca, cb;
+  DI::split(fp, la, lb, ca, cb);
+  if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return;
+  const int tnode = ca * TS::SN(A) + cb * TS::SN(B);
+  const int telem = la * TS::SE(A) + lb * TS::SE(B);
+  const int sL = (p >= 1) ? (telem + (p - 1) * TS::SE(D)) * TS::NN + tnode + (N - 1) * TS::SN(D)
+                          : TS::NTN + TS::HOFF(D) + fp;
+  const int sR = (p < teff[D]) ? (telem + p * TS::SE(D)) * TS::NN + tnode
+                               : TS::NTN + TS::HOFF(D) + FPD + fp;
+  const double* xl = X + sL;
+  const double* xr = X + sR;
+  const double vL = xl[(5 + D) * NTOT], vR = xr[(5 + D) * NTOT];
+  const double PL = xl[8 * NTOT], PR = xr[8 * NTOT];
+  double nmL, npL, dL, nmR, npR, dR;
+  {
+    const double num = xl[9 * NTOT], den = xl[10 * NTOT];
+    const double root = dg_sqrt(num * fma(fma(-vL, vL, 1.0), den, num));
+    const double c = vL * den;
+    nmL = c - root; npL = c + root; dL = den + num;
   }
-  dg_gsync<TS::G>(grp);
-  if (active) {
-    const int id = in[D];
-    const double* line = Fb + (ti - id * TS::SN(D));
-    const double* dh = sD + id * N;
-    double dq[N];
+  {
+    const double num = xr[9 * NTOT], den = xr[10 * NTOT];
+    const double root = dg_sqrt(num * fma(fma(-vR, vR, 1.0), den, num));
+    const double c = vR * den;
+    nmR = c - root; npR = c + root; dR = den + num;
+  }
+  const bool ml = nmL * dR <= nmR * dL, mr = npL * dR >= npR * dL;       // Eq. 23-24 by cross-multiplication
+  const double nl = ml ? nmL : nmR, dl = ml ? dL : dR;
+  const double nr = mr ? npL : npR, dr = mr ? dL : dR;
+  double cL, cR, cU;
+  if (nl >= 0.0) { cL = 1.0; cR = 0.0; cU = 0.0; }
+  else if (nr <= 0.0) { cL = 0.0; cR = 1.0; cU = 0.0; }
+  else {
+    const double aa = nr * dl, bb = nl * dr;
+    const double q = dg_rcp(aa - bb);
+    cL = aa * q; cR = -bb * q; cU = nl * nr * q;
+  }
+  const double kL = fma(cL, vL, -cU), kR = fma(cR, vR, cU);
+  const double pL = cL * PL, pR = cR * PR;
+  double* pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
 #pragma unroll
-    for (int q = 0; q < N; ++q) dq[q] = a.rh[D] * dh[q];
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-#pragma unroll
-      for (int q = 0; q < N; ++q) R[v] = fma(dq[q], line[v * NTN + q * TS::SN(D)], R[v]);
-    }
+  for (int v = 0; v < 5; ++v) {
+    double f = fma(kL, xl[v * NTOT], kR * xr[v * NTOT]);
+    if (v == 1 + D) f += pL + pR;
+    if (v == 4) f = fma(pL, vL, fma(pR, vR, f));
+    pF[v * FPD] = f;
   }
 }
+
+// Volume term of direction D for this thread's node (Eq. 17 over the diagonal mass matrix): the
+// tensor-line contraction of F_D(W_q) = U_q v_q + P_q e_D, formed on the fly from the node records.
+template <int ND, int N, int D>
+__device__ __forceinline__ void dg_volume(const StageArgs& a, const double* sD, const double* X, int ti,
+                                          const int in[3], double R[5]) {
+  using TS = TileShape<ND, N>;
+  constexpr int NTOT = TS::NTOT;
+  const int id = in[D];
+  const double* line = X + (ti - id * TS::SN(D));
+  const double* dh = sD + id * N;
+#pragma unroll
+  for (int q = 0; q < N; ++q) {
+    const double* x = line + q * TS::SN(D);
+    const double dq = a.rh[D] * dh[q];
+    const double t = dq * x[(5 + D) * NTOT];
+    const double Pq = x[8 * NTOT];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) R[v] = fma(t, x[v * NTOT], R[v]);
+    R[1 + D] = fma(dq, Pq, R[1 + D]);
+    R[4] = fma(t, Pq, R[4]);
+  }
+}
+
 
 // Physicality operator on the cells of one warp group (PAPER.md:242-252 steps 1-4), one thread per
 // node; cell-local reductions through shared memory with group barriers only.  Must be called by
@@ -406,9 +450,10 @@ __device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int 
   }
 }
 
-// resident blocks per SM the register allocation must allow: 1024 threads (32 warps) per SM
+// resident blocks per SM the register allocation must allow: up to 1024 threads (32 warps) per SM,
+// but no more blocks than the shared memory of an SM holds
 #ifndef DG_MINB
-#define DG_MINB (1024 / TileShape<ND, N>::NT)
+#define DG_MINB TileShape<ND, N>::MINB
 #endif
 template <int ND, int N, int EOS>
 __global__ void __launch_bounds__(TileShape<ND, N>::NT, DG_MINB)
@@ -416,9 +461,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
   constexpr int NN = TS::NN, NTN = TS::NTN, NT = TS::NT, NE = TS::NE;
   extern __shared__ __align__(16) double sm[];
-  double* Ws = sm + TS::O_W;
-  double* Fs = sm + TS::O_F;
-  double* Hs = sm + TS::O_H;
+  double* X = sm + TS::O_X;
   double* Fh = sm + TS::O_FH;
   double* sD = sm + TS::O_D;
   double* sMean = sm + TS::O_MEAN;
@@ -446,39 +489,47 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   if (t < 4) sCnt[t] = 0;
   if (t < N * N) sD[t] = a.Dhat[t];
 
-  // 1. stage W of the tile and of the neighbours' facing nodal layers; U_s of the node in flight
-  double P = 1.0, v0 = 0.0, v1 = 0.0, v2 = 0.0, Un[5] = {0, 0, 0, 0, 0};
+  // 1. primitives (recovered by the previous stage) and conserved state of the node -> its record in
+  //    the shared node array; primitives of the neighbours' facing nodal layers -> halo slots
+  double Un[5] = {0, 0, 0, 0, 0};
   if (active) {
     double Wn[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
       Wn[v] = __ldg(a.Win + v * a.ndof + g);
-      Ws[v * NTN + ti] = Wn[v];
+      Un[v] = a.Us[v * a.ndof + g];
     }
-#pragma unroll
-    for (int v = 0; v < 5; ++v) Un[v] = a.Us[v * a.ndof + g];
-    const double rg = dg_rsqrt(fma(Wn[1], Wn[1], fma(Wn[2], Wn[2], fma(Wn[3], Wn[3], 1.0))));
-    P = Wn[4]; v0 = Wn[1] * rg; v1 = Wn[2] * rg; v2 = Wn[3] * rg;
+    dg_node_record<ND, N, EOS, true>(a.eos, Wn, Un, X, ti);
   }
-  dg_load_halo<ND, N, 0>(a, Hs, active, g, lc, in, org, teff);
-  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, Hs, active, g, lc, in, org, teff);
-  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, Hs, active, g, lc, in, org, teff);
+  dg_load_halo<ND, N, 0>(a, X, active, g, lc, in, org, teff);
+  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, X, active, g, lc, in, org, teff);
+  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, X, active, g, lc, in, org, teff);
+  __syncthreads();
+  // records of the halo points (U from W by Eq. 4, reading R8), a dense pass over the halo slots
+  for (int sl = NTN + t; sl < TS::NTOT; sl += NT) {
+    double W[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) W[v] = X[v * TS::NTOT + sl];
+    dg_node_record<ND, N, EOS, false>(a.eos, W, W, X, sl);
+  }
   __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, EOS, 0>(a.eos, Ws, Hs, Fh, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, Ws, Hs, Fh, f - TS::FOFF(1), teff);
-    else dg_face_flux<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, Ws, Hs, Fh, f - TS::FOFF(2), teff);
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, 0>(X, Fh, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, (ND > 1 ? 1 : 0)>(X, Fh, f - TS::FOFF(1), teff);
+    else dg_face_flux<ND, N, (ND > 2 ? 2 : 0)>(X, Fh, f - TS::FOFF(2), teff);
   }
 
-  // 3. volume quadrature, direction by direction, F(W_i) = U_i v_d + P e_d; the first direction
-  //    overlaps other warps' face fluxes, the block barrier then frees Ws as the second F buffer
+  // 3. volume quadrature: reads the node array only, so it needs no barrier and fills the time
+  //    other warps still spend on face fluxes
   double R[5] = {0, 0, 0, 0, 0};
-  dg_direction<ND, N, 0>(a, sD, Fs, ti, active, grp, in, Un, P, v0, R);
+  if (active) {
+    dg_volume<ND, N, 0>(a, sD, X, ti, in, R);
+    if constexpr (ND > 1) dg_volume<ND, N, 1>(a, sD, X, ti, in, R);
+    if constexpr (ND > 2) dg_volume<ND, N, 2>(a, sD, X, ti, in, R);
+  }
   __syncthreads();
-  if constexpr (ND > 1) dg_direction<ND, N, 1>(a, sD, Ws, ti, active, grp, in, Un, P, v1, R);
-  if constexpr (ND > 2) dg_direction<ND, N, 2>(a, sD, Fs, ti, active, grp, in, Un, P, v2, R);
 
   // 4. surface lift
   if (active) {
@@ -508,7 +559,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   double wn = a.w[in[0]];
   if (ND > 1) wn *= a.w[in[1]];
   if (ND > 2) wn *= a.w[in[2]];
-  dg_limiter_group<ND, N>(Uo, active, ti, le, n, grp, wn, a, (ND == 2) ? Fs : Ws, sPart, sMean, sSmin,
+  dg_limiter_group<ND, N>(Uo, active, ti, le, n, grp, wn, a, X, sPart, sMean, sSmin,
                           sFlag, sCnt);
 
   // 7. primitives of the new state, CFL maximum

@@ -71,12 +71,13 @@ struct TileShape {
   }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
-  // shared-memory layout, in doubles.  Node array X[NREC][NTOT]: per tile node and halo node the
-  // conserved state, the 3-velocity, the pressure and the wave-speed fraction sigma = num/den.
-  static constexpr int NTOT = NTN + NHALO;               // node slots: tile nodes, then halo points
-  static constexpr int NREC = 11;                        // D Mx My Mz E | vx vy vz | P | num den
-  static constexpr int O_X = 0;                          // [NREC][NTOT]
-  static constexpr int O_FH = O_X + NREC * NTOT;         // Fhat  [dir][plane][5][FP]
+  // shared-memory layout, in doubles.  Node records: per tile node X[11][NTN] = D Mx My Mz E | vx vy
+  // vz | P | num den (conserved state, 3-velocity, pressure, sigma = num/den of Eq. 22); per halo
+  // point XH[9][NHALO] = D Mx My Mz E | v_normal | P | num den.
+  static constexpr int NREC = 11, HREC = 9;
+  static constexpr int O_X = 0;                          // [NREC][NTN]
+  static constexpr int O_XH = O_X + NREC * NTN;          // [HREC][NHALO]
+  static constexpr int O_FH = O_XH + HREC * NHALO;       // Fhat  [dir][plane][5][FP]
   static constexpr int O_D = O_FH + 5 * NFACE;           // Dhat  [N][N] (padded to 32)
   static constexpr int O_MEAN = O_D + 32;                // [NE][5]
   static constexpr int O_SMIN = O_MEAN + 5 * NE;         // [NE] (ull)
@@ -193,36 +194,54 @@ struct DirInfo {
   }
 };
 
-// Record of one node in the shared node array from its primitives W (and, if known, its conserved
-// state): U (Eq. 4) for the Riemann flux and the volume flux F_d = U v_d + P e_d, the 3-velocity
-// v = u/gamma, P, and sigma_s = num/den of Eq. 22 as an unevaluated fraction.
-template <int ND, int N, int EOS, bool HAVE_U>
+// Record of a tile node in the shared node array from its primitives W and conserved state U: U (for
+// the Riemann flux and the volume flux F_d = U v_d + P e_d), the 3-velocity v = u/gamma, P, and
+// sigma_s = num/den of Eq. 22 as an unevaluated fraction.
+template <int ND, int N, int EOS>
 __device__ __forceinline__ void dg_node_record(const EosPar& eos, const double W[5], const double U[5],
                                                double* X, int slot) {
-  using TS = TileShape<ND, N>;
+  constexpr int S = TileShape<ND, N>::NTN;
   const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
   const double rg = dg_rsqrt(g2);
   double num, den;
   dg_sigma_frac<EOS>(eos, W[0], W[4], g2, num, den);
   double* x = X + slot;
-  if (HAVE_U) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) x[v * TS::NTOT] = U[v];
-  } else {
-    const double rh = dg_rho_h<EOS>(eos, W[0], W[4]);
-    const double g = g2 * rg, grh = g * rh;
-    x[0] = g * W[0];
-    x[1 * TS::NTOT] = grh * W[1];
-    x[2 * TS::NTOT] = grh * W[2];
-    x[3 * TS::NTOT] = grh * W[3];
-    x[4 * TS::NTOT] = fma(g2, rh, -W[4]);
-  }
-  x[5 * TS::NTOT] = W[1] * rg;
-  x[6 * TS::NTOT] = W[2] * rg;
-  x[7 * TS::NTOT] = W[3] * rg;
-  x[8 * TS::NTOT] = W[4];
-  x[9 * TS::NTOT] = num;
-  x[10 * TS::NTOT] = den;
+  for (int v = 0; v < 5; ++v) x[v * S] = U[v];
+  x[5 * S] = W[1] * rg;
+  x[6 * S] = W[2] * rg;
+  x[7 * S] = W[3] * rg;
+  x[8 * S] = W[4];
+  x[9 * S] = num;
+  x[10 * S] = den;
+}
+
+// Record of halo point h: its primitives W sit in rows 0..4 of XH; replace them by U (Eq. 4, reading
+// R8) and add the velocity component normal to the face, P and the sigma fraction.
+template <int ND, int N, int EOS>
+__device__ __forceinline__ void dg_halo_record(const EosPar& eos, double* XH, int h) {
+  using TS = TileShape<ND, N>;
+  constexpr int S = TS::NHALO;
+  double* x = XH + h;
+  double W[5];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) W[v] = x[v * S];
+  const int D = (ND > 2 && h >= TS::HOFF(2)) ? 2 : ((ND > 1 && h >= TS::HOFF(1)) ? 1 : 0);
+  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
+  const double rg = dg_rsqrt(g2);
+  double num, den;
+  dg_sigma_frac<EOS>(eos, W[0], W[4], g2, num, den);
+  const double rh = dg_rho_h<EOS>(eos, W[0], W[4]);
+  const double g = g2 * rg, grh = g * rh;
+  x[0] = g * W[0];
+  x[1 * S] = grh * W[1];
+  x[2 * S] = grh * W[2];
+  x[3 * S] = grh * W[3];
+  x[4 * S] = fma(g2, rh, -W[4]);
+  x[5 * S] = ((D == 0) ? W[1] : ((D == 1) ? W[2] : W[3])) * rg;
+  x[6 * S] = W[4];
+  x[7 * S] = num;
+  x[8 * S] = den;
 }
 
 // Halo of direction D: each node on the tile's boundary in direction D fetches the primitives of the
@@ -230,7 +249,7 @@ __device__ __forceinline__ void dg_node_record(const EosPar& eos, const double W
 // R12) -- global index = own index + a block-uniform offset -- into the halo slot that equals the
 // node's face-point index (rows 0..4; the record is completed in a dense pass over the halo slots).
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* X, bool active, int g,
+__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* XH, bool active, int g,
                                              const int lc[3], const int in[3], const int org[3],
                                              const int teff[3]) {
   using TS = TileShape<ND, N>;
@@ -250,16 +269,16 @@ __device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* X, bool
   const int off1 = (ed1 - (org[D] + teff[D] - 1)) * esD * TS::NN + (nl1 - (N - 1)) * TS::SN(D);
   if (!active) return;
   const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
-  double* dst = X + (TS::NTN + TS::HOFF(D) + fp);
+  double* dst = XH + (TS::HOFF(D) + fp);
   if (in[D] == 0 && lc[D] == 0) {
     const double* src = a.Win + (g + off0);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[v * TS::NTOT] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dst[v * TS::NHALO] = __ldg(src + v * a.ndof);
   }
   if (in[D] == N - 1 && lc[D] == teff[D] - 1) {
     const double* src = a.Win + (g + off1);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[FPD + v * TS::NTOT] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dst[FPD + v * TS::NHALO] = __ldg(src + v * a.ndof);
   }
 }
 
@@ -297,33 +316,38 @@ __device__ __forceinline__ void dg_add_surface(const double* Fh, const int lc[3]
 // HLL flux (reading R9, Eq. 21-24) at face point fl of direction D from the node records of its two
 // sides:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in the energy).
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_face_flux(const double* X, double* Fh, int fl, const int teff[3]) {
+__device__ __forceinline__ void dg_face_flux(const double* X, const double* XH, double* Fh, int fl,
+                                             const int teff[3]) {
   using TS = TileShape<ND, N>;
   using DI = DirInfo<ND, N, D>;
-  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD, NTOT = TS::NTOT;
+  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD, ST = TS::NTN, SH = TS::NHALO;
   const int p = fl / FPD, fp = fl - p * FPD;
   int la, lb, ca, cb;
   DI::split(fp, la, lb, ca, cb);
   if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return;
   const int tnode = ca * TS::SN(A) + cb * TS::SN(B);
   const int telem = la * TS::SE(A) + lb * TS::SE(B);
-  const int sL = (p >= 1) ? (telem + (p - 1) * TS::SE(D)) * TS::NN + tnode + (N - 1) * TS::SN(D)
-                          : TS::NTN + TS::HOFF(D) + fp;
-  const int sR = (p < teff[D]) ? (telem + p * TS::SE(D)) * TS::NN + tnode
-                               : TS::NTN + TS::HOFF(D) + FPD + fp;
-  const double* xl = X + sL;
-  const double* xr = X + sR;
-  const double vL = xl[(5 + D) * NTOT], vR = xr[(5 + D) * NTOT];
-  const double PL = xl[8 * NTOT], PR = xr[8 * NTOT];
+  // left / right records: a tile node (stride ST, rows v=5+D P=8 num=9 den=10) or a halo point
+  // (stride SH, rows v=5 P=6 num=7 den=8)
+  const bool hL = (p < 1), hR = (p >= teff[D]);
+  const double* xl = hL ? XH + (TS::HOFF(D) + fp)
+                        : X + ((telem + (p - 1) * TS::SE(D)) * TS::NN + tnode + (N - 1) * TS::SN(D));
+  const double* xr = hR ? XH + (TS::HOFF(D) + FPD + fp) : X + ((telem + p * TS::SE(D)) * TS::NN + tnode);
+  const int sl = hL ? SH : ST, sr = hR ? SH : ST;
+  const double* ql = xl + (hL ? 5 * SH : (5 + D) * ST);              // v, then (P, num, den) at +kl
+  const double* qr = xr + (hR ? 5 * SH : (5 + D) * ST);
+  const int kl = hL ? SH : (3 - D) * ST, kr = hR ? SH : (3 - D) * ST;
+  const double vL = ql[0], vR = qr[0];
+  const double PL = ql[kl], PR = qr[kr];
   double nmL, npL, dL, nmR, npR, dR;
   {
-    const double num = xl[9 * NTOT], den = xl[10 * NTOT];
+    const double num = ql[kl + sl], den = ql[kl + 2 * sl];
     const double root = dg_sqrt(num * fma(fma(-vL, vL, 1.0), den, num));
     const double c = vL * den;
     nmL = c - root; npL = c + root; dL = den + num;
   }
   {
-    const double num = xr[9 * NTOT], den = xr[10 * NTOT];
+    const double num = qr[kr + sr], den = qr[kr + 2 * sr];
     const double root = dg_sqrt(num * fma(fma(-vR, vR, 1.0), den, num));
     const double c = vR * den;
     nmR = c - root; npR = c + root; dR = den + num;
@@ -344,7 +368,7 @@ __device__ __forceinline__ void dg_face_flux(const double* X, double* Fh, int fl
   double* pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
-    double f = fma(kL, xl[v * NTOT], kR * xr[v * NTOT]);
+    double f = fma(kL, xl[v * sl], kR * xr[v * sr]);
     if (v == 1 + D) f += pL + pR;
     if (v == 4) f = fma(pL, vL, fma(pR, vR, f));
     pF[v * FPD] = f;
@@ -357,7 +381,7 @@ template <int ND, int N, int D>
 __device__ __forceinline__ void dg_volume(const StageArgs& a, const double* sD, const double* X, int ti,
                                           const int in[3], double R[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int NTOT = TS::NTOT;
+  constexpr int NTOT = TS::NTN;
   const int id = in[D];
   const double* line = X + (ti - id * TS::SN(D));
   const double* dh = sD + id * N;
@@ -462,6 +486,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   constexpr int NN = TS::NN, NTN = TS::NTN, NT = TS::NT, NE = TS::NE;
   extern __shared__ __align__(16) double sm[];
   double* X = sm + TS::O_X;
+  double* XH = sm + TS::O_XH;
   double* Fh = sm + TS::O_FH;
   double* sD = sm + TS::O_D;
   double* sMean = sm + TS::O_MEAN;
@@ -499,26 +524,21 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       Wn[v] = __ldg(a.Win + v * a.ndof + g);
       Un[v] = a.Us[v * a.ndof + g];
     }
-    dg_node_record<ND, N, EOS, true>(a.eos, Wn, Un, X, ti);
+    dg_node_record<ND, N, EOS>(a.eos, Wn, Un, X, ti);
   }
-  dg_load_halo<ND, N, 0>(a, X, active, g, lc, in, org, teff);
-  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, X, active, g, lc, in, org, teff);
-  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, X, active, g, lc, in, org, teff);
+  dg_load_halo<ND, N, 0>(a, XH, active, g, lc, in, org, teff);
+  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g, lc, in, org, teff);
+  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g, lc, in, org, teff);
   __syncthreads();
   // records of the halo points (U from W by Eq. 4, reading R8), a dense pass over the halo slots
-  for (int sl = NTN + t; sl < TS::NTOT; sl += NT) {
-    double W[5];
-#pragma unroll
-    for (int v = 0; v < 5; ++v) W[v] = X[v * TS::NTOT + sl];
-    dg_node_record<ND, N, EOS, false>(a.eos, W, W, X, sl);
-  }
+  for (int h = t; h < TS::NHALO; h += NT) dg_halo_record<ND, N, EOS>(a.eos, XH, h);
   __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, 0>(X, Fh, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, (ND > 1 ? 1 : 0)>(X, Fh, f - TS::FOFF(1), teff);
-    else dg_face_flux<ND, N, (ND > 2 ? 2 : 0)>(X, Fh, f - TS::FOFF(2), teff);
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, 0>(X, XH, Fh, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, (ND > 1 ? 1 : 0)>(X, XH, Fh, f - TS::FOFF(1), teff);
+    else dg_face_flux<ND, N, (ND > 2 ? 2 : 0)>(X, XH, Fh, f - TS::FOFF(2), teff);
   }
 
   // 3. volume quadrature: reads the node array only, so it needs no barrier and fills the time

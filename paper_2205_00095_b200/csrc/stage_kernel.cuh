@@ -244,6 +244,12 @@ __device__ __forceinline__ void dg_halo_record(const EosPar& eos, double* XH, in
   x[8 * S] = den;
 }
 
+__device__ __forceinline__ void dg_async_copy8(double* smem_dst, const double* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)),
+               "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void dg_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 // Halo of direction D: each node on the tile's boundary in direction D fetches the primitives of the
 // node facing it in the neighbouring element (periodic wrap; at an outflow boundary its own, reading
 // R12) -- global index = own index + a block-uniform offset -- into the halo slot that equals the
@@ -270,15 +276,17 @@ __device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* XH, boo
   if (!active) return;
   const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
   double* dst = XH + (TS::HOFF(D) + fp);
+  // asynchronous 8-byte copies global -> shared (LDGSTS): all halo rows of the block are in flight at
+  // once and no register is held; the caller waits with dg_async_wait() before the block barrier
   if (in[D] == 0 && lc[D] == 0) {
     const double* src = a.Win + (g + off0);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[v * TS::NHALO] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * TS::NHALO, src + v * a.ndof);
   }
   if (in[D] == N - 1 && lc[D] == teff[D] - 1) {
     const double* src = a.Win + (g + off1);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dst[FPD + v * TS::NHALO] = __ldg(src + v * a.ndof);
+    for (int v = 0; v < 5; ++v) dg_async_copy8(dst + FPD + v * TS::NHALO, src + v * a.ndof);
   }
 }
 
@@ -516,6 +524,9 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 1. primitives (recovered by the previous stage) and conserved state of the node -> its record in
   //    the shared node array; primitives of the neighbours' facing nodal layers -> halo slots
+  dg_load_halo<ND, N, 0>(a, XH, active, g, lc, in, org, teff);
+  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g, lc, in, org, teff);
+  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g, lc, in, org, teff);
   double Un[5] = {0, 0, 0, 0, 0};
   if (active) {
     double Wn[5];
@@ -525,10 +536,12 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       Un[v] = a.Us[v * a.ndof + g];
     }
     dg_node_record<ND, N, EOS>(a.eos, Wn, Un, X, ti);
+    if (a.mode == DG_MODE_STAGE && a.a != 0.0) {         // U0 is needed last: warm L2 now
+#pragma unroll
+      for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g));
+    }
   }
-  dg_load_halo<ND, N, 0>(a, XH, active, g, lc, in, org, teff);
-  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g, lc, in, org, teff);
-  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g, lc, in, org, teff);
+  dg_async_wait();
   __syncthreads();
   // records of the halo points (U from W by Eq. 4, reading R8), a dense pass over the halo slots
   for (int h = t; h < TS::NHALO; h += NT) dg_halo_record<ND, N, EOS>(a.eos, XH, h);

@@ -207,6 +207,26 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
     for (int q = 0; q < c->N; ++q) a.Dhat[i * c->N + q] = c->basis.Dhat[i][q];
   }
   a.lift = c->basis.lift;
+  // halo offsets: the node facing a boundary node of a tile lies one element over (interior), or, on
+  // the first / last tile of the axis, in the element at the other end (periodic) / is the node
+  // itself (outflow, reading R12)
+  {
+    const int NN = c->NN, N = c->N;
+    const long long es[3] = {1, c->cfg.nelem[0], c->cfg.nelem[0] * c->cfg.nelem[1]};
+    int sn = 1;
+    for (int d = 0; d < 3; ++d, sn *= N) {
+      const long long step = es[d] * NN, layer = (long long)(N - 1) * sn;
+      a.hoff[d][0] = (int)(-step + layer);                 // minus side: neighbour e-1, node layer N-1
+      a.hoff[d][1] = (int)(step - layer);                  // plus side:  neighbour e+1, node layer 0
+      if (d < c->cfg.ndim && c->cfg.bc[d] == DGRHD_BC_PERIODIC) {
+        a.hfix[d][0] = (int)(c->cfg.nelem[d] * step);      // e-1 -> e-1+ne
+        a.hfix[d][1] = (int)(-c->cfg.nelem[d] * step);
+      } else {                                             // own node: total offset 0
+        a.hfix[d][0] = -a.hoff[d][0];
+        a.hfix[d][1] = -a.hoff[d][1];
+      }
+    }
+  }
   a.wsum = c->wsum;
 }
 

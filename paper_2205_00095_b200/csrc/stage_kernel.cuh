@@ -112,6 +112,7 @@ struct StageArgs {
   double w[5];            // GLL weights
   double lift, wsum;      // 1/w_0, sum of the tensor weights (node order)
   int mode;               // DG_MODE_RHS / DG_MODE_STAGE
+  int hoff[3][2], hfix[3][2];   // halo: global-index offset of the facing node (minus, plus side)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -261,18 +262,10 @@ __device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* XH, boo
   using TS = TileShape<ND, N>;
   using DI = DirInfo<ND, N, D>;
   constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
-  int ed0 = org[D] - 1, nl0 = N - 1, ed1 = org[D] + teff[D], nl1 = 0;
-  if (ed0 < 0) {
-    if (a.bc[D] == DG_BC_PERIODIC) ed0 = a.ne[D] - 1;
-    else { ed0 = 0; nl0 = 0; }
-  }
-  if (ed1 >= a.ne[D]) {
-    if (a.bc[D] == DG_BC_PERIODIC) ed1 = 0;
-    else { ed1 = a.ne[D] - 1; nl1 = N - 1; }
-  }
-  const int esD = (D == 0) ? 1 : ((D == 1) ? a.ne[0] : a.ne[0] * a.ne[1]);
-  const int off0 = (ed0 - org[D]) * esD * TS::NN + nl0 * TS::SN(D);
-  const int off1 = (ed1 - (org[D] + teff[D] - 1)) * esD * TS::NN + (nl1 - (N - 1)) * TS::SN(D);
+  // offsets of the facing node: interior value + a correction on the first / last tile of the axis
+  // (periodic wrap or outflow), both precomputed by the host (StageArgs::hoff, hfix)
+  const int off0 = a.hoff[D][0] + ((org[D] == 0) ? a.hfix[D][0] : 0);
+  const int off1 = a.hoff[D][1] + ((org[D] + teff[D] == a.ne[D]) ? a.hfix[D][1] : 0);
   if (!active) return;
   const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
   double* dst = XH + (TS::HOFF(D) + fp);

@@ -29,10 +29,10 @@ STAGES = 3
 # (80 B) + U0 in on stages 2 and 3 (40 B) -> (80 + 120 + 120) / 3
 ALG_BYTES_PER_DOF_STAGE = (80.0 + 120.0 + 120.0) / 3.0
 # fp64 work per DOF and stage of dg_stage_kernel<3,4,ideal>: executed 2*dfma + dmul + dadd from the
-# ncu capture profiles/r1_ncu_summary.md, mean of the three stages (588 / 597 / 711)
-FLOP_PER_DOF_STAGE = 632.0
+# ncu capture profiles/r1_ncu_summary.md, mean of the three stages (571 / 580 / 694)
+FLOP_PER_DOF_STAGE = 615.1
 # DRAM bytes per DOF and stage of the same capture (dram__bytes_read + write, mean of the 3 stages)
-NCU_TRAFFIC_PER_DOF_STAGE = 192.7
+NCU_TRAFFIC_PER_DOF_STAGE = 185.7
 # fp64 peak: 148 SMs x 64 DFMA/clk/SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on peak_sustained)
 # x 2 flop x SM clock
 FP64_FMA_PER_CLK = 148 * 64

@@ -30,6 +30,9 @@ typedef unsigned long long dg_ull;
 
 __host__ __device__ constexpr int dg_ipow(int b, int e) { return e <= 0 ? 1 : b * dg_ipow(b, e - 1); }
 
+#ifndef DG_NPT64       // nodes per thread of the 3D p=3 kernel (1 or 2)
+#define DG_NPT64 1
+#endif
 #ifndef DG_T3N4X       // tile of the 3D p=3 kernel (tuning knob)
 #define DG_T3N4X 2
 #define DG_T3N4Y 2
@@ -51,11 +54,16 @@ struct TileShape {
   static constexpr int TX = dg_tile(ND, N, 0), TY = dg_tile(ND, N, 1), TZ = dg_tile(ND, N, 2);
   static constexpr int NE = TX * TY * TZ;            // elements per tile
   static constexpr int NTN = NE * NN;                // nodes per tile
+  // A thread owns M nodes of one element (node n0 + m NNT, m < M): M = 2 for the 64-node hexahedron, so
+  // that an element is exactly one warp (no cross-warp barrier for anything cell-local) and every
+  // thread carries two independent fp64 instruction streams; M = 1 otherwise.
+  static constexpr int M = (NN == 64) ? DG_NPT64 : 1;
+  static constexpr int NNT = NN / M;                 // threads per element
   // Threads are organised in warp groups that own whole elements, so that everything cell-local
-  // (tensor-line contractions, cell mean, min s) synchronises a group, not the block:
-  //   NN <= 32: one warp holds EPG = 32/NN elements (lanes >= EPG*NN idle);  NN > 32: G warps per element.
-  static constexpr int G = (NN <= 32) ? 1 : (NN + 31) / 32;   // warps per group
-  static constexpr int EPG = (NN <= 32) ? 32 / NN : 1;        // elements per group
+  // (cell mean, min s) synchronises a group, not the block:
+  //   NNT <= 32: one warp holds EPG = 32/NNT elements (lanes >= EPG*NNT idle);  else G warps per element.
+  static constexpr int G = (NNT <= 32) ? 1 : (NNT + 31) / 32;   // warps per group
+  static constexpr int EPG = (NNT <= 32) ? 32 / NNT : 1;        // elements per group
   static constexpr int GT = 32 * G;                           // threads per group
   static constexpr int NG = NE / EPG;                         // groups per block
   static_assert(NE % EPG == 0, "tile must hold a whole number of warp groups");
@@ -400,17 +408,22 @@ __device__ __forceinline__ void dg_volume(const StageArgs& a, const double* sD, 
 }
 
 
-// Physicality operator on the cells of one warp group (PAPER.md:242-252 steps 1-4), one thread per
-// node; cell-local reductions through shared memory with group barriers only.  Must be called by
-// every thread of the group.  Uo: the node's state, limited in place.
+// Physicality operator on the cells of one warp group (PAPER.md:242-252 steps 1-4); a thread owns the
+// M nodes n0 + m NNT of its cell (tile slots ti0 + m NNT).  Cell-local reductions go through shared
+// memory with group barriers only.  Must be called by every thread of the group.  Uo: the nodes'
+// states, limited in place.
 template <int ND, int N>
-__device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int ti, int le, int n, int grp,
-                                                 double wn, const StageArgs& a, double* scratch,
-                                                 double* sPart, double* sMean, dg_ull* sSmin, int* sFlag,
-                                                 int* sCnt) {
+__device__ __forceinline__ void dg_limiter_group(double (*Uo)[5], bool active, int ti0, int le, int n0,
+                                                 int grp, const double* wn, const StageArgs& a,
+                                                 double* scratch, double* sPart, double* sMean,
+                                                 dg_ull* sSmin, int* sFlag, int* sCnt) {
   using TS = TileShape<ND, N>;
-  constexpr int NN = TS::NN, NTN = TS::NTN;
-  const bool bad = active && !dg_admissible(Uo, a.f_screen);         // step 1: screen (R13e)
+  constexpr int NN = TS::NN, NTN = TS::NTN, M = TS::M, NNT = TS::NNT;
+  bool bad = false;
+  if (active) {
+#pragma unroll
+    for (int m = 0; m < M; ++m) bad = bad || !dg_admissible(Uo[m], a.f_screen);   // step 1: screen (R13e)
+  }
   if (bad) sFlag[le] = 1;
   dg_gsync<TS::G>(grp);
   const bool flagged = active && (sFlag[le] != 0);
@@ -419,33 +432,36 @@ __device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int 
   if (!any) return;
   if (flagged) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) scratch[v * NTN + ti] = wn * Uo[v];
+    for (int m = 0; m < M; ++m) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) scratch[v * NTN + ti0 + m * NNT] = wn[m] * Uo[m][v];
+    }
   }
   dg_gsync<TS::G>(grp);
   // cell average: J interleaved partial sums per variable (5 J lanes), then their sum by 5 lanes
-  constexpr int J = (NN >= 20) ? 4 : NN / 5;
+  constexpr int J = (NNT >= 20) ? 4 : NNT / 5;
   if (J == 0) {                                                     // tiny cells: one lane sums
-    if (flagged && n == 0) {
+    if (flagged && n0 == 0) {
       for (int v = 0; v < 5; ++v) {
         double acc = 0.0;
-        for (int m = 0; m < NN; ++m) acc += scratch[v * NTN + le * NN + m];
+        for (int q = 0; q < NN; ++q) acc += scratch[v * NTN + le * NN + q];
         sMean[le * 5 + v] = acc / a.wsum;
       }
     }
   } else {
-    if (flagged && n < 5 * J) {
-      const int v = n % 5, j = n / 5;
+    if (flagged && n0 < 5 * J) {
+      const int v = n0 % 5, j = n0 / 5;
       const double* p = scratch + v * NTN + le * NN;
       double acc = 0.0;
-      for (int m = j; m < NN; m += J) acc += p[m];
-      sPart[le * 20 + n] = acc;
+      for (int q = j; q < NN; q += J) acc += p[q];
+      sPart[le * 20 + n0] = acc;
     }
     dg_gsync<TS::G>(grp);
-    if (flagged && n < 5) {
+    if (flagged && n0 < 5) {
       double acc = 0.0;
 #pragma unroll
-      for (int j = 0; j < J; ++j) acc += sPart[le * 20 + 5 * j + n];
-      sMean[le * 5 + n] = acc / a.wsum;
+      for (int j = 0; j < J; ++j) acc += sPart[le * 20 + 5 * j + n0];
+      sMean[le * 5 + n0] = acc / a.wsum;
     }
   }
   dg_gsync<TS::G>(grp);
@@ -456,11 +472,16 @@ __device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int 
     const bool mean_ok = dg_admissible(Ub, a.f_solve);               // step 2 (reading R13d)
     double si = 0.0;
     if (mean_ok) {
-      si = dg_limiter_node_s(Ub, Uo, a.f_solve);                     // step 3
-      if (!(si >= 0.0)) si = 0.0;
+      si = 1.0;
+#pragma unroll
+      for (int m = 0; m < M; ++m) {
+        double sm_ = dg_limiter_node_s(Ub, Uo[m], a.f_solve);        // step 3
+        if (!(sm_ >= 0.0)) sm_ = 0.0;
+        si = fmin(si, sm_);
+      }
     }
     if (si < 1.0) atomicMin(&sSmin[le], dg_ord(si));                 // step 4: s = min_i s_i
-    if (n == 0) {
+    if (n0 == 0) {
       atomicAdd(&sCnt[0], 1);
       if (!mean_ok) atomicAdd(&sCnt[1], 1);
     }
@@ -470,8 +491,11 @@ __device__ __forceinline__ void dg_limiter_group(double Uo[5], bool active, int 
     const double s = a.one_m_delta * dg_unord(sSmin[le]);            // R13c
     const double tt = 1.0 - s;
 #pragma unroll
-    for (int v = 0; v < 5; ++v)                                      // Eq. 26 from the nearer end (R14)
-      Uo[v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[v], Uo[v]) : fma(s, Uo[v] - Ub[v], Ub[v]);
+    for (int m = 0; m < M; ++m) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v)                                    // Eq. 26 from the nearer end (R14)
+        Uo[m][v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[m][v], Uo[m][v]) : fma(s, Uo[m][v] - Ub[v], Ub[v]);
+    }
   }
 }
 
@@ -501,37 +525,57 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
-  // warp group, element and node of this thread
+  // warp group, element and the M nodes (n0 + m NNT) of this thread
+  constexpr int M = TS::M, NNT = TS::NNT;
   const int t = threadIdx.x;
   const int grp = t / TS::GT, r = t - grp * TS::GT;
-  const int le = grp * TS::EPG + r / NN, n = r % NN;
-  const int ti = le * NN + n;                                        // node slot in the tile arrays
+  const int le = grp * TS::EPG + r / NNT, n0 = r % NNT;
+  const int ti0 = le * NN + n0;                                      // tile slot of node m: ti0 + m NNT
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
-  const int in[3] = {n % N, (n / N) % N, n / (N * N)};
-  const bool active = (r < TS::EPG * NN) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
-  int g = 0;                                                         // ndof < 2^31 (dgrhd_create)
-  if (active) g = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + n;
+  const bool active = (r < TS::EPG * NNT) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
+  int g0 = 0;                                                        // ndof < 2^31 (dgrhd_create)
+  if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + n0;
+  int in[M][3];
+#pragma unroll
+  for (int m = 0; m < M; ++m) {
+    const int n = n0 + m * NNT;
+    in[m][0] = n % N; in[m][1] = (n / N) % N; in[m][2] = n / (N * N);
+  }
   if (t < NE) { sSmin[t] = dg_ord(1.0); sFlag[t] = 0; }
   if (t < 4) sCnt[t] = 0;
   if (t < N * N) sD[t] = a.Dhat[t];
 
-  // 1. primitives (recovered by the previous stage) and conserved state of the node -> its record in
-  //    the shared node array; primitives of the neighbours' facing nodal layers -> halo slots
-  dg_load_halo<ND, N, 0>(a, XH, active, g, lc, in, org, teff);
-  if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g, lc, in, org, teff);
-  if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g, lc, in, org, teff);
-  double Un[5] = {0, 0, 0, 0, 0};
-  if (active) {
-    double Wn[5];
+  // 1. primitives (recovered by the previous stage) and conserved state of the nodes -> their records
+  //    in the shared node array; primitives of the neighbours' facing nodal layers -> halo slots
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      Wn[v] = __ldg(a.Win + v * a.ndof + g);
-      Un[v] = a.Us[v * a.ndof + g];
+  for (int m = 0; m < M; ++m) {
+    dg_load_halo<ND, N, 0>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
+    if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
+    if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
+  }
+  double Un[M][5];
+#pragma unroll
+  for (int m = 0; m < M; ++m)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) Un[m][v] = 0.0;
+  if (active) {
+    double Wn[M][5];
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        Wn[m][v] = __ldg(a.Win + v * a.ndof + g0 + m * NNT);
+        Un[m][v] = a.Us[v * a.ndof + g0 + m * NNT];
+      }
     }
-    dg_node_record<ND, N, EOS>(a.eos, Wn, Un, X, ti);
+#pragma unroll
+    for (int m = 0; m < M; ++m) dg_node_record<ND, N, EOS>(a.eos, Wn[m], Un[m], X, ti0 + m * NNT);
     if (a.mode == DG_MODE_STAGE && a.a != 0.0) {         // U0 is needed last: warm L2 now
 #pragma unroll
-      for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g));
+      for (int m = 0; m < M; ++m)
+#pragma unroll
+        for (int v = 0; v < 5; ++v)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0 + m * NNT));
     }
   }
   dg_async_wait();
@@ -549,59 +593,86 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 3. volume quadrature: reads the node array only, so it needs no barrier and fills the time
   //    other warps still spend on face fluxes
-  double R[5] = {0, 0, 0, 0, 0};
+  double R[M][5];
+#pragma unroll
+  for (int m = 0; m < M; ++m)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
   if (active) {
-    dg_volume<ND, N, 0>(a, sD, X, ti, in, R);
-    if constexpr (ND > 1) dg_volume<ND, N, 1>(a, sD, X, ti, in, R);
-    if constexpr (ND > 2) dg_volume<ND, N, 2>(a, sD, X, ti, in, R);
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+      dg_volume<ND, N, 0>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
+      if constexpr (ND > 1) dg_volume<ND, N, 1>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
+      if constexpr (ND > 2) dg_volume<ND, N, 2>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
+    }
   }
   __syncthreads();
 
   // 4. surface lift
   if (active) {
-    dg_add_surface<ND, N, 0>(Fh, lc, in, a.rh[0] * a.lift, R);
-    if constexpr (ND > 1) dg_add_surface<ND, N, 1>(Fh, lc, in, a.rh[1] * a.lift, R);
-    if constexpr (ND > 2) dg_add_surface<ND, N, 2>(Fh, lc, in, a.rh[2] * a.lift, R);
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+      dg_add_surface<ND, N, 0>(Fh, lc, in[m], a.rh[0] * a.lift, R[m]);
+      if constexpr (ND > 1) dg_add_surface<ND, N, 1>(Fh, lc, in[m], a.rh[1] * a.lift, R[m]);
+      if constexpr (ND > 2) dg_add_surface<ND, N, 2>(Fh, lc, in[m], a.rh[2] * a.lift, R[m]);
+    }
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
 #pragma unroll
-      for (int v = 0; v < 5; ++v) a.Rout[v * a.ndof + g] = R[v];
+      for (int m = 0; m < M; ++m)
+#pragma unroll
+        for (int v = 0; v < 5; ++v) a.Rout[v * a.ndof + g0 + m * NNT] = R[m][v];
     }
     return;
   }
 
   // 5. SSP-RK combine (Shu-Osher form)
   const double dt = *a.dt_ptr;
-  double Uo[5];
+  double Uo[M][5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) Uo[v] = a.b * fma(dt, R[v], Un[v]);
+  for (int m = 0; m < M; ++m)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) Uo[m][v] = a.b * fma(dt, R[m][v], Un[m][v]);
   if (a.a != 0.0 && active) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) Uo[v] = fma(a.a, a.U0[v * a.ndof + g], Uo[v]);
+    for (int m = 0; m < M; ++m)
+#pragma unroll
+      for (int v = 0; v < 5; ++v) Uo[m][v] = fma(a.a, a.U0[v * a.ndof + g0 + m * NNT], Uo[m][v]);
   }
 
-  // 6. physicality-enforcing operator (cell-local)
-  double wn = a.w[in[0]];
-  if (ND > 1) wn *= a.w[in[1]];
-  if (ND > 2) wn *= a.w[in[2]];
-  dg_limiter_group<ND, N>(Uo, active, ti, le, n, grp, wn, a, X, sPart, sMean, sSmin,
-                          sFlag, sCnt);
+  // 6. physicality-enforcing operator (cell-local; the node array is free after the barrier above)
+  double wn[M];
+#pragma unroll
+  for (int m = 0; m < M; ++m) {
+    wn[m] = a.w[in[m][0]];
+    if (ND > 1) wn[m] *= a.w[in[m][1]];
+    if (ND > 2) wn[m] *= a.w[in[m][2]];
+  }
+  dg_limiter_group<ND, N>(Uo, active, ti0, le, n0, grp, wn, a, X, sPart, sMean, sSmin, sFlag, sCnt);
 
   // 7. primitives of the new state, CFL maximum
   double speed = 0.0;
   if (active) {
-    double Wo[5];
-    const int st = dg_con2prim<EOS>(a.eos, Uo, Wo);
-    if (st != 0) atomicAdd(&sCnt[2], 1);
+    double Wo[M][5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      a.Uout[v * a.ndof + g] = Uo[v];
-      a.Wout[v * a.ndof + g] = Wo[v];
+    for (int m = 0; m < M; ++m) {
+      const int st = dg_con2prim<EOS>(a.eos, Uo[m], Wo[m]);
+      if (st != 0) atomicAdd(&sCnt[2], 1);
     }
+#pragma unroll
+    for (int m = 0; m < M; ++m)
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        a.Uout[v * a.ndof + g0 + m * NNT] = Uo[m][v];
+        a.Wout[v * a.ndof + g0 + m * NNT] = Wo[m][v];
+      }
     if (a.do_cfl) {
-      const double sp = dg_cfl_speed<EOS, ND>(a.eos, Wo, a.cw);
-      if (sp > 0.0) speed = sp;
+#pragma unroll
+      for (int m = 0; m < M; ++m) {
+        const double sp = dg_cfl_speed<EOS, ND>(a.eos, Wo[m], a.cw);
+        if (sp > 0.0) speed = fmax(speed, sp);
+      }
     }
   }
   if (a.do_cfl) {

@@ -314,17 +314,27 @@ DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
   const double R = (9.0 * c1 * c2 - 27.0 * c3 - 2.0 * c1 * c1 * c1) * (1.0 / 54.0);   // Eq. 67
   const double Q3 = Q * Q * Q;
   const double d = fma(R, R, Q3);                                // Eq. 65
+  // The transcendental part of the closed form (acos/cos, Eq. 69-70; cube roots, Eq. 71-73) is
+  // evaluated in single precision -- it only has to land in the basin of the wanted root -- and the
+  // root is then refined on the cubic of Eq. 61 itself by three Newton steps (reading R7b: the first
+  // squares the ~1e-7 seed error, the second reaches the fp64 floor for all gamma, the third covers
+  // gamma -> 1 where W = gamma^2-1 is tiny against the seed's absolute error).
   double Wv;
   if (d < 0.0) {
     double arg = R * dg_rsqrt(-Q3);
     arg = fmin(1.0, fmax(-1.0, arg));
-    Wv = 2.0 * dg_sqrt(-Q) * cos(acos(arg) * (1.0 / 3.0)) - c1 * (1.0 / 3.0);   // Eq. 69-70
+    const float th = acosf((float)arg) * (1.0f / 3.0f);
+    Wv = 2.0 * dg_sqrt(-Q) * (double)__cosf(th) - c1 * (1.0 / 3.0);        // Eq. 69-70
   } else {
-    double sd = sqrt(d);
-    Wv = cbrt(R + sd) + cbrt(R - sd) - c1 * (1.0 / 3.0);         // Eq. 71-73
+    const double sd = dg_sqrt(d);
+    const double p = R + sd, q = R - sd;
+    const double cp = (fabs(p) < 1e37) ? (double)cbrtf((float)p) : cbrt(p);
+    const double cq = (fabs(q) < 1e37) ? (double)cbrtf((float)q) : cbrt(q);
+    Wv = cp + cq - c1 * (1.0 / 3.0);                                       // Eq. 71-73
   }
   Wv = fmax(Wv, 0.0);
-  {                                                              // R7b: one Newton step on Eq. 61
+#pragma unroll
+  for (int it = 0; it < 3; ++it) {                                         // R7b: Newton on Eq. 61
     const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
     const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
     const double Wn = Wv - f * dg_rcp(df);

@@ -403,3 +403,25 @@ def test_cuda_graph_replay_is_bit_identical_and_cuts_launch_overhead():
         assert ctx.dgrhd_get_counters()["n_stages"] == 3 * 208
     assert torch.equal(res[0], res[1])
     print(f"config 1: {us[0]:.1f} us/step with the CUDA graph, {us[1]:.1f} us/step with plain launches")
+
+
+def test_tm_slow_flows_recovered_to_full_relative_accuracy_on_gpu():
+    """The CUDA Taub-Matthews route (single-precision closed form + three Newton steps on Eq. 61,
+    DESIGN.md R7b) against exactly known primitives and against the oracle, |u| in [1e-9, 1e-1]."""
+    rng = np.random.default_rng(4)
+    n = 20011
+    umag = 10.0 ** rng.uniform(-9, -1, n)
+    dirn = rng.normal(size=(3, n)); dirn /= np.sqrt((dirn ** 2).sum(0))
+    rho = 10.0 ** rng.uniform(-3, 2, n)
+    P = rho * 10.0 ** rng.uniform(-6, 3, n)
+    W = np.vstack([rho[None], umag * dirn, P[None]])
+    U = O.prim2con_batch(1, 0.0, W)
+    Wo, _ = O.con2prim_batch(1, 0.0, U)
+    st = torch.zeros(n, dtype=torch.int32, device=DEV)
+    Wg = B().dgrhd_con2prim_batch(1, 0.0, to_dev(U), status=st).cpu().numpy()
+    assert int(st.max()) == 0
+    ug = np.sqrt((Wg[1:4] ** 2).sum(0))
+    assert np.max(np.abs(ug / umag - 1)) < 2e-12
+    assert np.max(np.abs(Wg[0] / rho - 1)) < 1e-14
+    rho_e, u_e, dir_e, p_ok = c2p_errors(Wg, Wo, U)
+    assert rho_e.max() <= 1e-10 and u_e.max() <= 1e-10 and dir_e.max() <= 1e-10 and p_ok.all()

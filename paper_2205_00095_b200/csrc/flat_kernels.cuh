@@ -29,8 +29,11 @@ __device__ __forceinline__ void dg_block_atomic_max(double x, double* sRed, dg_u
   }
 }
 
+#ifndef DG_C2P_MINB
+#define DG_C2P_MINB 6      // 6 x 256 threads per SM (42 registers): best of a 1..8 sweep
+#endif
 template <int EOS>
-__global__ void __launch_bounds__(DG_FLAT_NT)
+__global__ void __launch_bounds__(DG_FLAT_NT, DG_C2P_MINB)
 dg_c2p_batch_kernel(long long n, const double* __restrict__ U, double* __restrict__ W,
                     int* __restrict__ status, EosPar eos) {
   const long long i = (long long)blockIdx.x * DG_FLAT_NT + threadIdx.x;

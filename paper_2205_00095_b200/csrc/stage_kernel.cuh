@@ -2,13 +2,16 @@
 //
 // One launch performs, for a tile of TX x TY x TZ elements per thread block (one thread per nodal
 // point, PAPER.md:128-145 order of operations):
-//   1. stage the tile's nodal primitives W (recovered by the previous stage, Eq. 16) and the
-//      one-node-deep face layer of the neighbouring elements in shared memory (with GLL nodes the
-//      face interpolation of :132-134 is a gather of that layer, reading R1);
-//   2. HLL interface flux (Eq. 21-24, reading R9), each face point of the tile once, spread
-//      evenly over the block's threads                                          -> shared memory;
-//   3. per direction: physical flux at every node (Eq. 2)                       -> shared memory,
-//   4. volume quadrature (Eq. 17) + surface lift (Eq. 18), both over the diagonal mass matrix;
+//   1. per tile node a record in shared memory -- conserved state U_s, 3-velocity, pressure and the
+//      fraction sigma_s = num/den of Eq. 22 -- from the node's primitives W (recovered by the previous
+//      stage, Eq. 16) and U_s; the primitives of the one-node-deep face layer of the neighbouring
+//      elements arrive by cp.async (with GLL nodes the face interpolation of :132-134 is a gather
+//      of that layer, reading R1) and get their records (U by Eq. 4) in a dense pass;
+//   2. HLL interface flux (Eq. 21-24, reading R9) from the two records of each face point of the
+//      tile, once each, spread evenly over the block's threads                  -> shared memory;
+//   3. volume quadrature (Eq. 17) over the diagonal mass matrix, F_d = U v_d + P e_d (Eq. 2) formed on
+//      the fly from the records along the node's tensor lines (read-only: no barrier);
+//   4. surface lift (Eq. 18);
 //   MODE_RHS stops here and writes R = L(U).  MODE_STAGE continues:
 //   5. SSP-RK combine  U_out = a U0 + b (U_s + dt R)   (:147-152, reading R10), dt read from
 //      device memory;

@@ -217,6 +217,27 @@ def box3d(seed, n=128, p=3, kmax=8, device="cpu", sigma=2.0, vrms=0.6, vcap=0.99
     return cfg, W.contiguous()
 
 
+def box2d(seed, nx=32, ny=32, p=2, kmax=1, device="cpu", eos=EOS_IDEAL, gamma_ad=5.0 / 3.0, sigma=2.0,
+          vrms=0.6, vcap=0.99, rho_floor=1e-6, p_over_rho=0.01, bc=(BC_PERIODIC, BC_PERIODIC)):
+    """2D companion of config 5 (same recipe evaluated on the plane z = 0.3125 of the 3D band-limited
+    fields, all three velocity components kept): exercises the physicality operator of the 2D
+    kernels, which config 4's smooth shear layer never triggers."""
+    g = torch.Generator().manual_seed(int(seed))
+    N = p + 1
+    coords = (axis_coords(0.0, 1.0, nx, N, device), axis_coords(0.0, 1.0, ny, N, device),
+              torch.tensor([0.3125], dtype=F64, device=device))
+    vg = _band_field(g, 3, kmax, coords, device)[:, 0] * (vrms / math.sqrt(3.0))
+    gg = _band_field(g, 1, kmax, coords, device)[:, 0]
+    vmag = torch.sqrt((vg * vg).sum(0, keepdim=True))
+    vg = vg * torch.clamp(vcap / vmag, max=1.0)
+    rho = torch.clamp(torch.exp(sigma * gg), min=rho_floor)
+    v = vg.reshape(3, -1)
+    Wg = torch.cat([rho.reshape(1, -1), _u_from_v(v), p_over_rho * rho.reshape(1, -1)])
+    W = grid_to_canonical(Wg.reshape(5, ny * N, nx * N), [nx, ny], N)
+    cfg = _cfg(2, [nx, ny], [0.0] * 2, [1.0] * 2, list(bc), p, eos, gamma_ad)
+    return cfg, W.contiguous()
+
+
 def limiter_stress(U, n_nodes, seed, frac=0.05):
     """Companion input 5L: overwrite 1-3 nodes in a seeded `frac` of the cells of the conserved
     state U[5, ndof] with inadmissible values (D < 0, or E = 0.9 sqrt(D^2+|M|^2)).  Pure data

@@ -15,61 +15,7 @@ from paper_2205_00095_b200 import inputs as I
 
 pytestmark = pytest.mark.gpu
 
-DEV = "cuda"
-
-
-def B():
-    from paper_2205_00095_b200 import binding
-    return binding
-
-
-def ocfg(d):
-    return O.make_config(d["ndim"], d["nelem"], d["xmin"], d["xmax"], d["bc"], d["order_p"],
-                         d["eos"], d["gamma_ad"], d["rk_stages"], d["eps_q"], d["delta_s"])
-
-
-def gcfg(d):
-    return B().make_config(d["ndim"], d["nelem"], d["xmin"], d["xmax"], d["bc"], d["order_p"],
-                           d["eos"], d["gamma_ad"], d["rk_stages"], d["eps_q"], d["delta_s"])
-
-
-def to_dev(a):
-    return torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64).to(DEV).contiguous()
-
-
-def relmax(a, b):
-    """max|a-b| / max|b| per variable (rows)."""
-    a, b = np.asarray(a), np.asarray(b)
-    return np.max(np.abs(a - b), axis=1) / np.maximum(np.max(np.abs(b), axis=1), 1e-300)
-
-
-def smooth_prims(cfgd, seed, amp=0.3):
-    """Smooth, bounded, seeded primitive field on the mesh of cfgd (pure input data)."""
-    nd, N = cfgd["ndim"], cfgd["order_p"] + 1
-    rng = np.random.default_rng(seed)
-    ph = rng.uniform(0, 2 * np.pi, size=(5, 3))
-    ax = [I.axis_coords(cfgd["xmin"][d], cfgd["xmax"][d], cfgd["nelem"][d], N).numpy() for d in range(nd)]
-    L = [cfgd["xmax"][d] - cfgd["xmin"][d] for d in range(nd)]
-    if nd == 1:
-        X = [ax[0]]
-    elif nd == 2:
-        yy, xx = np.meshgrid(ax[1], ax[0], indexing="ij")
-        X = [xx, yy]
-    else:
-        zz, yy, xx = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
-        X = [xx, yy, zz]
-    s = [sum(np.sin(2 * np.pi * (X[d] - cfgd["xmin"][d]) / L[d] + ph[v, d]) for d in range(nd)) / nd
-         for v in range(5)]
-    Wg = np.stack([1.0 + amp * s[0], 0.8 * amp * s[1], 0.8 * amp * s[2] * (nd > 1),
-                   0.8 * amp * s[3] * (nd > 2), 0.7 + 0.5 * amp * s[4]])
-    W = I.grid_to_canonical(torch.from_numpy(Wg), cfgd["nelem"][:nd], N)
-    return W.contiguous().numpy()
-
-
-def mesh(nd, nelem, p, eos, G, bc=None, **kw):
-    lo = [0.0, -0.5, 0.25][:nd]
-    hi = [1.0, 1.0, 1.0][:nd]
-    return I._cfg(nd, nelem, lo, hi, bc or [I.BC_PERIODIC] * nd, p, eos, G, **kw)
+from _util import B, DEV, gcfg, mesh, ocfg, relmax, smooth_prims, to_dev  # noqa: E402
 
 
 # ------------------------------------------------------------------------------------------------

@@ -12,8 +12,10 @@
  *       e = ix + nx*(iy + ny*iz)  (element),  n = i + N*(j + N*k)  (node in element), N = p+1,
  *       i.e. element of a 5 x ndof array with ndof = nelem_total * N^ndim, row stride ndof.
  *     Nodes are tensor-product Gauss-Lobatto-Legendre points (reading R1).
- *   - every pointer named *_dev is a DEVICE pointer (8-byte aligned at least), every pointer named
- *     *_host is a HOST pointer.  The caller owns all buffers, including the workspace: the library
+ *   - every pointer named *_dev is a DEVICE pointer, every pointer named *_host is a HOST pointer.
+ *     State pointers handed to dgrhd_rhs / dgrhd_enforce_physicality must be 16-byte aligned (the
+ *     kernels move whole nodal lines with 16-byte accesses; EINVAL otherwise); everything else needs
+ *     8-byte alignment only (dgrhd_con2prim_batch takes its 16-byte path when it can).  The caller owns all buffers, including the workspace: the library
  *     allocates no device memory and frees none.
  *   - every call returns an int status (DGRHD_OK = 0) and never throws or aborts; argument errors
  *     are detected before any launch.  Numerical trouble is not an error return: it is counted on
@@ -75,7 +77,8 @@ int dgrhd_set_option(dgrhd_ctx* ctx, int option, int value);
  * CFL wave-speed maximum of the new state; it does not apply the physicality operator (R15). */
 int dgrhd_set_state(dgrhd_ctx* ctx, const double* U_dev);
 int dgrhd_get_state(dgrhd_ctx* ctx, double* U_dev);
-/* Primitives W[5][ndof] of the internal state (as recovered by the last stage / set_state). */
+/* Primitives W[5][ndof] of the internal state (recovered from it by this call, PAPER.md:128-130
+ * Eq. 16: the context keeps only the pressure of its state between stages). */
 int dgrhd_get_prims(dgrhd_ctx* ctx, double* W_dev);
 
 /* R = L(U): the DG spatial operator, Eq. 15-18, on caller buffers in the canonical
@@ -96,7 +99,8 @@ int dgrhd_enforce_physicality(dgrhd_ctx* ctx, double* U_dev, unsigned char* flag
 
 /* CFL time step (formula: DESIGN.md reading R11):
  *   dt = cfl / max_nodes sum_d (2p+1) max(|lambda-_d|, |lambda+_d|) / h_d,  lambda+- of Eq. 21-22.
- * U_dev = NULL uses the internal state.  Synchronises; *dt_host receives dt. */
+ * U_dev = NULL uses the internal state.  Synchronises; *dt_host receives dt.  ESTATE if the state has no
+ * positive finite wave speed (e.g. con2prim failed everywhere): dt would be infinite. */
 int dgrhd_cfl_dt(dgrhd_ctx* ctx, const double* U_dev, double cfl, double* dt_host);
 
 /* Advance the internal state by nsteps SSP-RK steps; each stage is
@@ -108,12 +112,16 @@ int dgrhd_cfl_dt(dgrhd_ctx* ctx, const double* U_dev, double cfl, double* dt_hos
 int dgrhd_step(dgrhd_ctx* ctx, double dt, int nsteps, double* t_inout_host);
 
 /* Device counters accumulated since create / the last reset (synchronises):
- *   out_host[0] n_flagged   cell-activations of the physicality operator inside dgrhd_step
- *   out_host[1] n_bad_mean  cells whose average was itself inadmissible (flattened)
- *   out_host[2] n_c2p_fail  nodes where con2prim failed (inadmissible input or P <= 0)
- *   out_host[3] n_stages    RK stages executed by dgrhd_step
+ *   out_host[0] n_flagged      cell-activations of the physicality operator inside dgrhd_step
+ *   out_host[1] n_bad_mean     cells whose average was itself inadmissible (flattened)
+ *   out_host[2] n_c2p_fail     nodes where con2prim failed (inadmissible input or P <= 0)
+ *   out_host[3] n_stages       RK stages executed by dgrhd_step
+ *   out_host[4] n_tm_fallback  Taub-Matthews recoveries that took the double-precision closed form
+ *                              because the fast route's Newton polish had not converged
+ *   out_host[5] n_bad_dt       CFL-mode steps whose wave-speed maximum was not a positive finite
+ *                              number: they ran with dt = 0 (state unchanged) instead of dt = inf
  * reset != 0 zeroes them afterwards. */
-int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[4], int reset);
+int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[6], int reset);
 
 /* Conserved -> primitive recovery of a flat SoA batch U_dev[5][n] -> W_dev[5][n]:
  * ideal EOS by Newton iteration on the quartic of Eq. 59 (beta = 2w/(1+w^2), Eq. 58; small-xi
@@ -123,13 +131,18 @@ int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[4], int reset);
 int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const double* U_dev, double* W_dev,
                          int* status_dev, void* cuda_stream);
 
+/* Number of Taub-Matthews recoveries of the context-free batch calls (all streams of the current
+ * device) that took the double-precision fallback since the last reset (see n_tm_fallback above).
+ * Synchronises cuda_stream. */
+int dgrhd_tm_fallback_count(int64_t* out_host, int reset, void* cuda_stream);
+
 /* Primitive -> conserved, Eq. 4, flat SoA batch W_dev[5][n] -> U_dev[5][n]. */
 int dgrhd_prim2con_batch(int eos, double gamma_ad, int64_t n, const double* W_dev, double* U_dev,
                          void* cuda_stream);
 
 /* Host-buffer convenience wrapper around dgrhd_con2prim_batch: copies U_host[5][n] to the device
- * (chunked, through the caller's staging buffer stage_dev of stage_bytes >= 80 bytes per state of
- * one chunk), runs the kernel, copies W_host[5][n] back, synchronises.  Used for end-to-end timing. */
+ * (chunked, through the caller's 16-byte aligned staging buffer stage_dev of stage_bytes >= 80 bytes
+ * per state of one chunk, at least 160), runs the kernel, copies W_host[5][n] back, synchronises.  Used for end-to-end timing. */
 int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, const double* U_host,
                               double* W_host, void* stage_dev, size_t stage_bytes,
                               void* cuda_stream);
@@ -144,7 +157,7 @@ int dgrhd_run_host(dgrhd_ctx* ctx, const double* U_host_in, double* U_host_out, 
  * thread).  Never NULL; valid until the next call on the same context / thread. */
 const char* dgrhd_last_error(const dgrhd_ctx* ctx);
 
-/* Library version string, e.g. "dgrhd 0.1 (sm_100a)". */
+/* Library version string, e.g. "dgrhd 0.2 (sm_100a)". */
 const char* dgrhd_version(void);
 
 #ifdef __cplusplus

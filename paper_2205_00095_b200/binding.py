@@ -52,7 +52,7 @@ _vp, _dp, _i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
 EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_state",
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
-           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host",
+           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count",
            "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
 
 
@@ -78,6 +78,7 @@ def lib():
         L.dgrhd_step.argtypes = [_vp, C.c_double, C.c_int, _dp]
         L.dgrhd_get_counters.argtypes = [_vp, _i64p, C.c_int]
         L.dgrhd_con2prim_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp, _vp]
+        L.dgrhd_tm_fallback_count.argtypes = [_i64p, C.c_int, _vp]
         L.dgrhd_prim2con_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp]
         L.dgrhd_con2prim_batch_host.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp,
                                                 C.c_size_t, _vp]
@@ -209,9 +210,10 @@ class Context:
         return tt.value
 
     def dgrhd_get_counters(self, reset=False):
-        out = (C.c_int64 * 4)()
+        out = (C.c_int64 * 6)()
         _check(lib().dgrhd_get_counters(self._h, out, int(reset)), self._h)
-        return dict(n_flagged=out[0], n_bad_mean=out[1], n_c2p_fail=out[2], n_stages=out[3])
+        return dict(n_flagged=out[0], n_bad_mean=out[1], n_c2p_fail=out[2], n_stages=out[3],
+                    n_tm_fallback=out[4], n_bad_dt=out[5])
 
 
 def dgrhd_con2prim_batch(eos, gamma_ad, U, W=None, status=None):
@@ -219,6 +221,12 @@ def dgrhd_con2prim_batch(eos, gamma_ad, U, W=None, status=None):
     _check(lib().dgrhd_con2prim_batch(eos, gamma_ad, U.shape[1], _ptr(U, 5), _ptr(W, 5),
                                       _ptr(status), _stream()))
     return W
+
+
+def dgrhd_tm_fallback_count(reset=False):
+    out = C.c_int64()
+    _check(lib().dgrhd_tm_fallback_count(C.byref(out), int(reset), _stream()))
+    return out.value
 
 
 def dgrhd_prim2con_batch(eos, gamma_ad, W, U=None):

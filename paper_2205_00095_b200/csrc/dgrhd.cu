@@ -4,6 +4,7 @@
 // the caller's stream; there is no CPU fallback (every compute call needs a CUDA device).
 #include "../../include/dgrhd.h"
 
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -14,7 +15,9 @@
 #include "flat_kernels.cuh"
 
 // launchers of the fused stage kernel, one translation unit per (ndim, EOS): stage_inst.cu
-#define DG_DECL(nd, eos) cudaError_t dg_launch_stage_##nd##_##eos(int N, const StageArgs& a, cudaStream_t st);
+#define DG_DECL(nd, eos)                                                                   \
+  cudaError_t dg_launch_stage_##nd##_##eos(int N, const StageArgs& a, cudaStream_t st); \
+  cudaError_t dg_prepare_stage_##nd##_##eos(int N);
 DG_DECL(1, 0) DG_DECL(1, 1) DG_DECL(2, 0) DG_DECL(2, 1) DG_DECL(3, 0) DG_DECL(3, 1)
 #undef DG_DECL
 
@@ -22,25 +25,23 @@ namespace {
 
 thread_local char g_err[512] = "";
 
-void set_err(char* dst, const char* fmt, ...) {
-  va_list ap;
-  va_start(ap, fmt);
-  vsnprintf(dst, 512, fmt, ap);
-  va_end(ap);
-}
 
 constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
-// device scalars at the head of the workspace
+// device scalars at the head of the workspace.  The CFL maximum and the event counters are spread
+// over DG_NSLOT slots, 128 bytes apart (one atomic per thread block: a single address would
+// serialise them); readers take the maximum / the sum over the slots.
 struct DevScalars {
   double dt;          // time step of the step in flight
   double t_acc;       // sum of the steps taken by the current dgrhd_step call
-  dg_ull amax;        // ordered-int image of the CFL maximum of the internal state
-  dg_ull amax_tmp;    // same, for dgrhd_cfl_dt on a caller state
-  dg_ull counters[4]; // n_flagged, n_bad_mean, n_c2p_fail, n_stages
+  dg_ull n_stages;    // RK stages executed by dgrhd_step
+  dg_ull n_bad_dt;    // steps whose CFL maximum was not a positive finite number (dt = 0)
   dg_ull call_cnt[2]; // per-call counters of dgrhd_enforce_physicality
-  double wnode[125];  // tensor GLL weights, node order
+  dg_ull pad_[10];
+  dg_ull amax[DG_NSLOT * DG_SLOT_STRIDE];      // ordered-int images of the CFL maximum of the state
+  dg_ull amax_tmp[DG_NSLOT * DG_SLOT_STRIDE];  // same, for dgrhd_cfl_dt on a caller state
+  dg_ull counters[DG_NSLOT * DG_SLOT_STRIDE];  // per slot: n_flagged, n_bad_mean, n_c2p_fail, n_tm_fallback
 };
 
 bool valid_cfg(const dgrhd_config* c) {
@@ -83,13 +84,17 @@ struct dgrhd_ctx {
   size_t state_bytes;
   cudaStream_t stream;
   DevScalars* sc;
-  double *Ua, *Ub, *W[2];
-  int wcur;                 // W[wcur] holds the primitives of the internal state Ua
+  // B[0..2]: state buffers (5 x ndof each); the state lives in B[par] for RK1 (whose output cannot
+  // overwrite its input: neighbouring blocks read their halo from it) and in B[0] otherwise.
+  // P[0..1]: pressure of the stage input / output, ping-pong; P[par] belongs to the state.
+  double* B[3];
+  double* P[2];
+  int par;
   bool has_state;
   BasisTables basis;
   double wsum;
   EosPar eos;
-  // one captured CUDA graph per primitive-buffer parity: a whole SSP-RK step (dt kernel + stages)
+  // one captured CUDA graph per parity: a whole SSP-RK step (dt kernel + stages)
   int use_graph;
   cudaStream_t cap_stream;
   cudaGraphExec_t gexec[2];
@@ -118,6 +123,9 @@ static int cuda_fail(dgrhd_ctx* c, cudaError_t e, const char* where) {
     if (e__ != cudaSuccess) return cuda_fail(c, e__, #call); \
   } while (0)
 
+static inline double* state_buf(dgrhd_ctx* c) { return c->B[c->cfg.rk_stages == 1 ? c->par : 0]; }
+static inline bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
 // ------------------------------------------------------------------------------------------------
 // kernel dispatch helpers
 // ------------------------------------------------------------------------------------------------
@@ -134,8 +142,22 @@ static cudaError_t launch_stage(dgrhd_ctx* c, const StageArgs& a) {
   return cudaErrorInvalidValue;
 }
 
-// W = p(U) over a state (+ failure count, + CFL maximum when amax != NULL)
-static cudaError_t launch_c2p_state(dgrhd_ctx* c, const double* U, double* W, dg_ull* amax,
+static cudaError_t prepare_stage(dgrhd_ctx* c) {
+  const int key = c->cfg.ndim * 2 + c->cfg.eos;
+  switch (key) {
+    case 2: return dg_prepare_stage_1_0(c->N);
+    case 3: return dg_prepare_stage_1_1(c->N);
+    case 4: return dg_prepare_stage_2_0(c->N);
+    case 5: return dg_prepare_stage_2_1(c->N);
+    case 6: return dg_prepare_stage_3_0(c->N);
+    case 7: return dg_prepare_stage_3_1(c->N);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// P = P(U) over a state (+ all primitives when W != NULL, + failure counts, + CFL maximum when
+// amax != NULL)
+static cudaError_t launch_c2p_state(dgrhd_ctx* c, const double* U, double* P, double* W, dg_ull* amax,
                                     dg_ull* counters) {
   const long long n = c->ndof;
   const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
@@ -143,7 +165,7 @@ static cudaError_t launch_c2p_state(dgrhd_ctx* c, const double* U, double* W, dg
   for (int d = 0; d < c->cfg.ndim; ++d)
     cw[d] = (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]);
 #define DG_GO(E, D) \
-  dg_c2p_state_kernel<E, D><<<nb, DG_FLAT_NT, 0, c->stream>>>(n, U, W, c->eos, cw[0], cw[1], cw[2], amax, counters)
+  dg_c2p_state_kernel<E, D><<<nb, DG_FLAT_NT, 0, c->stream>>>(n, U, P, W, c->eos, cw[0], cw[1], cw[2], amax, counters)
   if (c->cfg.eos == DGRHD_EOS_IDEAL) {
     if (c->cfg.ndim == 1) DG_GO(0, 1); else if (c->cfg.ndim == 2) DG_GO(0, 2); else DG_GO(0, 3);
   } else {
@@ -153,17 +175,25 @@ static cudaError_t launch_c2p_state(dgrhd_ctx* c, const double* U, double* W, dg
   return cudaGetLastError();
 }
 
+static LimPar make_limpar(dgrhd_ctx* c) {
+  LimPar lp;
+  for (int i = 0; i < 5; ++i) lp.w[i] = (i < c->N) ? c->basis.w[i] : 0.0;
+  lp.wsum = c->wsum;
+  lp.f_screen = 1.0 - 0.5 * c->cfg.eps_q;
+  lp.f_solve = 1.0 - c->cfg.eps_q;
+  lp.one_m_delta = 1.0 - c->cfg.delta_s;
+  return lp;
+}
+
 template <int ND>
 static cudaError_t launch_limiter_nd(dgrhd_ctx* c, double* U, unsigned char* flag, double* s,
                                      dg_ull* counters) {
-  const double fs = 1.0 - 0.5 * c->cfg.eps_q, fv = 1.0 - c->cfg.eps_q, od = 1.0 - c->cfg.delta_s;
-#define DG_GO(NV)                                                                                   \
-  {                                                                                                 \
-    using LS = LimShape<dg_ipow(NV, ND)>;                                                           \
-    const unsigned nb = (unsigned)((c->nelem + LS::NE - 1) / LS::NE);                               \
-    dg_limiter_kernel<ND, NV><<<nb, LS::NT, 0, c->stream>>>(c->nelem, c->ndof, U, flag, s,          \
-                                                            c->sc->wnode, c->wsum, fs, fv, od,      \
-                                                            counters);                              \
+  const LimPar lp = make_limpar(c);
+#define DG_GO(NV)                                                                                  \
+  {                                                                                                \
+    constexpr int EPB = 4 * (32 / dg_ipow(NV, ND - 1));                                            \
+    const unsigned nb = (unsigned)((c->nelem + EPB - 1) / EPB);                                    \
+    dg_limiter_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, flag, s, lp, counters); \
   }
   switch (c->N) {
     case 1: DG_GO(1) break;
@@ -186,13 +216,17 @@ static cudaError_t launch_limiter(dgrhd_ctx* c, double* U, unsigned char* flag, 
 static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
   memset(&a, 0, sizeof a);
   a.ndof = c->ndof;
+  const int N = c->N;
   for (int d = 0; d < 3; ++d) {
     a.ne[d] = (int)c->cfg.nelem[d];
-    a.bc[d] = c->cfg.bc[d];
     if (d < c->cfg.ndim) {
       const double h = (c->cfg.xmax[d] - c->cfg.xmin[d]) / (double)c->cfg.nelem[d];
-      a.rh[d] = 2.0 / h;
+      const double rh = 2.0 / h;
       a.cw[d] = (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]);
+      a.lift[d] = rh * c->basis.lift;
+      double* D = (d == 0) ? a.Dx : (d == 1 ? a.Dy : a.Dz);
+      for (int i = 0; i < N; ++i)
+        for (int q = 0; q < N; ++q) D[i * N + q] = rh * c->basis.Dhat[i][q];
     }
   }
   a.f_screen = 1.0 - 0.5 * c->cfg.eps_q;
@@ -200,18 +234,14 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
   a.one_m_delta = 1.0 - c->cfg.delta_s;
   a.eos = c->eos;
   a.dt_ptr = &c->sc->dt;
-  a.amax = &c->sc->amax;
+  a.amax = c->sc->amax;
   a.counters = c->sc->counters;
-  for (int i = 0; i < c->N; ++i) {
-    a.w[i] = c->basis.w[i];
-    for (int q = 0; q < c->N; ++q) a.Dhat[i * c->N + q] = c->basis.Dhat[i][q];
-  }
-  a.lift = c->basis.lift;
+  for (int i = 0; i < N; ++i) a.w[i] = c->basis.w[i];
   // halo offsets: the node facing a boundary node of a tile lies one element over (interior), or, on
   // the first / last tile of the axis, in the element at the other end (periodic) / is the node
   // itself (outflow, reading R12)
   {
-    const int NN = c->NN, N = c->N;
+    const int NN = c->NN;
     const long long es[3] = {1, c->cfg.nelem[0], c->cfg.nelem[0] * c->cfg.nelem[1]};
     int sn = 1;
     for (int d = 0; d < 3; ++d, sn *= N) {
@@ -233,13 +263,15 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
 // ------------------------------------------------------------------------------------------------
 // create / destroy
 // ------------------------------------------------------------------------------------------------
+static size_t pbuf_bytes(long long ndof) { return align_up((size_t)ndof * sizeof(double)); }
+
 extern "C" size_t dgrhd_workspace_bytes(const dgrhd_config* cfg) {
   if (!valid_cfg(cfg)) return 0;
   long long ne = 1;
   for (int d = 0; d < cfg->ndim; ++d) ne *= cfg->nelem[d];
   const long long ndof = ne * ipow(cfg->order_p + 1, cfg->ndim);
   const size_t sb = align_up((size_t)ndof * 5 * sizeof(double));
-  return align_up(sizeof(DevScalars)) + 4 * sb;
+  return align_up(sizeof(DevScalars)) + 3 * sb + 2 * pbuf_bytes(ndof);
 }
 
 extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t workspace_bytes,
@@ -270,22 +302,20 @@ extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t
   char* p = (char*)workspace_dev;
   c->sc = (DevScalars*)p;  p += align_up(sizeof(DevScalars));
   const size_t sb = align_up(c->state_bytes);
-  c->Ua = (double*)p;  p += sb;
-  c->Ub = (double*)p;  p += sb;
-  c->W[0] = (double*)p;  p += sb;
-  c->W[1] = (double*)p;
-  // tensor weights in node order and their sum (summed in node order)
-  DevScalars h;
-  memset(&h, 0, sizeof h);
+  for (int i = 0; i < 3; ++i) { c->B[i] = (double*)p;  p += sb; }
+  for (int i = 0; i < 2; ++i) { c->P[i] = (double*)p;  p += pbuf_bytes(c->ndof); }
+  // sum of the tensor weights (summed in node order)
   c->wsum = 0.0;
   for (int n = 0; n < c->NN; ++n) {
     double w = c->basis.w[n % c->N];
     if (cfg->ndim > 1) w *= c->basis.w[(n / c->N) % c->N];
     if (cfg->ndim > 2) w *= c->basis.w[n / (c->N * c->N)];
-    h.wnode[n] = w;
     c->wsum += w;
   }
-  cudaError_t e = cudaMemcpyAsync(c->sc, &h, sizeof h, cudaMemcpyHostToDevice, c->stream);
+  // per-device kernel attributes (shared-memory opt-in) for this context's instantiation, outside
+  // any stream capture
+  cudaError_t e = prepare_stage(c);
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) {
     int r = cuda_fail(nullptr, e, "dgrhd_create");
@@ -318,12 +348,18 @@ extern "C" int dgrhd_destroy(dgrhd_ctx* ctx) {
 // ------------------------------------------------------------------------------------------------
 // state access
 // ------------------------------------------------------------------------------------------------
+static int refresh_state_pressure(dgrhd_ctx* c) {
+  DG_CUDA(c, cudaMemsetAsync(c->sc->amax, 0, sizeof c->sc->amax, c->stream));
+  DG_CUDA(c, launch_c2p_state(c, state_buf(c), c->P[c->par], nullptr, c->sc->amax, c->sc->counters));
+  return DGRHD_OK;
+}
+
 extern "C" int dgrhd_set_state(dgrhd_ctx* c, const double* U_dev) {
   if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_set_state: NULL argument");
-  DG_CUDA(c, cudaMemcpyAsync(c->Ua, U_dev, c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
-  DG_CUDA(c, cudaMemsetAsync(&c->sc->amax, 0, sizeof(dg_ull), c->stream));
-  c->wcur = 0;
-  DG_CUDA(c, launch_c2p_state(c, c->Ua, c->W[0], &c->sc->amax, c->sc->counters));
+  c->par = 0;
+  DG_CUDA(c, cudaMemcpyAsync(c->B[0], U_dev, c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  const int r = refresh_state_pressure(c);
+  if (r != DGRHD_OK) return r;
   c->has_state = true;
   return DGRHD_OK;
 }
@@ -331,31 +367,33 @@ extern "C" int dgrhd_set_state(dgrhd_ctx* c, const double* U_dev) {
 extern "C" int dgrhd_get_state(dgrhd_ctx* c, double* U_dev) {
   if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_get_state: NULL argument");
   if (!c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_get_state: no state set");
-  DG_CUDA(c, cudaMemcpyAsync(U_dev, c->Ua, c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  DG_CUDA(c, cudaMemcpyAsync(U_dev, state_buf(c), c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
   return DGRHD_OK;
 }
 
 extern "C" int dgrhd_get_prims(dgrhd_ctx* c, double* W_dev) {
   if (!c || !W_dev) return fail(c, DGRHD_EINVAL, "dgrhd_get_prims: NULL argument");
   if (!c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_get_prims: no state set");
-  DG_CUDA(c, cudaMemcpyAsync(W_dev, c->W[c->wcur], c->state_bytes, cudaMemcpyDeviceToDevice, c->stream));
+  DG_CUDA(c, launch_c2p_state(c, state_buf(c), nullptr, W_dev, nullptr, nullptr));
   return DGRHD_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
-// R = L(U) on caller buffers: nodal con2prim into the spare primitive buffer, then the fused
-// kernel in MODE_RHS
+// R = L(U) on caller buffers: nodal pressure into the spare pressure buffer, then the fused kernel
+// in MODE_RHS
 // ------------------------------------------------------------------------------------------------
 extern "C" int dgrhd_rhs(dgrhd_ctx* c, const double* U_dev, double* R_dev) {
   if (!c || !U_dev || !R_dev) return fail(c, DGRHD_EINVAL, "dgrhd_rhs: NULL argument");
   if (U_dev == R_dev) return fail(c, DGRHD_EINVAL, "dgrhd_rhs: U_dev and R_dev overlap");
-  double* Wtmp = c->W[c->wcur ^ 1];
-  DG_CUDA(c, launch_c2p_state(c, U_dev, Wtmp, nullptr, c->sc->counters));
+  if (!aligned16(U_dev) || !aligned16(R_dev))
+    return fail(c, DGRHD_EINVAL, "dgrhd_rhs: state pointers must be 16-byte aligned");
+  double* Ptmp = c->P[c->par ^ 1];
+  DG_CUDA(c, launch_c2p_state(c, U_dev, Ptmp, nullptr, nullptr, c->sc->counters));
   StageArgs a;
   fill_stage_args(c, a);
   a.mode = DG_MODE_RHS;
-  a.Win = Wtmp;
   a.Us = U_dev;
+  a.Pin = Ptmp;
   a.Rout = R_dev;
   DG_CUDA(c, launch_stage(c, a));
   return DGRHD_OK;
@@ -366,12 +404,14 @@ extern "C" int dgrhd_enforce_physicality(dgrhd_ctx* c, double* U_dev, unsigned c
   if (!c) return fail(c, DGRHD_EINVAL, "dgrhd_enforce_physicality: NULL context");
   const bool internal = (U_dev == nullptr);
   if (internal && !c->has_state) return fail(c, DGRHD_ESTATE, "dgrhd_enforce_physicality: no state set");
-  double* U = internal ? c->Ua : U_dev;
+  if (!internal && !aligned16(U_dev))
+    return fail(c, DGRHD_EINVAL, "dgrhd_enforce_physicality: state pointer must be 16-byte aligned");
+  double* U = internal ? state_buf(c) : U_dev;
   DG_CUDA(c, cudaMemsetAsync(c->sc->call_cnt, 0, 2 * sizeof(dg_ull), c->stream));
   DG_CUDA(c, launch_limiter(c, U, flag_dev, s_dev, c->sc->call_cnt));
-  if (internal) {                       // refresh the primitives and the CFL maximum of the state
-    DG_CUDA(c, cudaMemsetAsync(&c->sc->amax, 0, sizeof(dg_ull), c->stream));
-    DG_CUDA(c, launch_c2p_state(c, c->Ua, c->W[c->wcur], &c->sc->amax, c->sc->counters));
+  if (internal) {                       // refresh the pressure and the CFL maximum of the state
+    const int r = refresh_state_pressure(c);
+    if (r != DGRHD_OK) return r;
   }
   if (counters_host) {
     dg_ull h[2];
@@ -386,48 +426,63 @@ extern "C" int dgrhd_enforce_physicality(dgrhd_ctx* c, double* U_dev, unsigned c
 extern "C" int dgrhd_cfl_dt(dgrhd_ctx* c, const double* U_dev, double cfl, double* dt_host) {
   if (!c || !dt_host) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: NULL argument");
   if (!(cfl > 0.0)) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: cfl must be > 0");
-  dg_ull* slot = &c->sc->amax;
+  dg_ull* slots = c->sc->amax;
   if (U_dev) {
-    slot = &c->sc->amax_tmp;
-    DG_CUDA(c, cudaMemsetAsync(slot, 0, sizeof(dg_ull), c->stream));
-    DG_CUDA(c, launch_c2p_state(c, U_dev, nullptr, slot, nullptr));
+    slots = c->sc->amax_tmp;
+    DG_CUDA(c, cudaMemsetAsync(slots, 0, sizeof c->sc->amax_tmp, c->stream));
+    DG_CUDA(c, launch_c2p_state(c, U_dev, nullptr, nullptr, slots, nullptr));
   } else if (!c->has_state) {
     return fail(c, DGRHD_ESTATE, "dgrhd_cfl_dt: no state set");
   }
-  dg_ull h = 0;
-  DG_CUDA(c, cudaMemcpyAsync(&h, slot, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  static_assert(sizeof(double) == sizeof(dg_ull), "ordered-integer image");
+  double h[DG_NSLOT * DG_SLOT_STRIDE];
+  DG_CUDA(c, cudaMemcpyAsync(h, slots, sizeof h, cudaMemcpyDeviceToHost, c->stream));
   DG_CUDA(c, cudaStreamSynchronize(c->stream));
-  double m;
-  memcpy(&m, &h, sizeof m);
-  *dt_host = cfl / m;
+  double m = 0.0;
+  for (int s = 0; s < DG_NSLOT; ++s)
+    if (h[s * DG_SLOT_STRIDE] > m) m = h[s * DG_SLOT_STRIDE];
+  const double dt = cfl / m;
+  if (!(m > 0.0) || !std::isfinite(dt))
+    return fail(c, DGRHD_ESTATE, "dgrhd_cfl_dt: no positive finite wave speed in the state (con2prim failures?)");
+  *dt_host = dt;
   return DGRHD_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
 // SSP-RK steps (Shu-Osher form, reading R10): per step one dt kernel + one fused kernel per stage,
-// all on the context's stream, dt and the CFL maximum resident on the device.
-//   buffers: Ua = U at the start of the step (and the state between calls), Ub = stage state,
-//   W[wcur] = primitives of the stage input, W[wcur^1] = primitives of the stage output.
+// all on the context's stream, dt and the CFL maximum resident on the device.  A stage's output
+// never overwrites its input (other blocks read their halo from it); it may overwrite U0 (each
+// thread reads and writes its own nodes only):
+//   RK1     B[par] -> B[par^1]
+//   SSPRK2  B0 -> B1;  (B1, U0 = B0) -> B0
+//   SSPRK3  B0 -> B1;  (B1, U0 = B0) -> B2;  (B2, U0 = B0) -> B0
+// The pressure buffers alternate every stage: P[par] -> P[par^1].
 // ------------------------------------------------------------------------------------------------
 static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
   const int S = c->cfg.rk_stages;
   static const double A3[3] = {0.0, 0.75, 1.0 / 3.0}, B3[3] = {1.0, 0.25, 2.0 / 3.0};
   static const double A2[2] = {0.0, 0.5}, B2[2] = {1.0, 0.5};
-  dg_dt_kernel<<<1, 1, 0, c->stream>>>(dt, -dt, &c->sc->amax, &c->sc->dt, &c->sc->t_acc,
-                                       &c->sc->counters[3], S);
+  dg_dt_kernel<<<1, 1, 0, c->stream>>>(dt, -dt, c->sc->amax, &c->sc->dt, &c->sc->t_acc,
+                                       &c->sc->n_stages, &c->sc->n_bad_dt, S);
   DG_CUDA(c, cudaGetLastError());
   for (int s = 0; s < S; ++s) {
     const bool last = (s == S - 1);
     a.a = (S == 2) ? A2[s] : A3[s];
     a.b = (S == 2) ? B2[s] : B3[s];
-    a.Win = c->W[c->wcur];
-    a.Wout = c->W[c->wcur ^ 1];
-    a.Us = (s == 0) ? c->Ua : c->Ub;
-    a.U0 = c->Ua;
-    a.Uout = last ? c->Ua : c->Ub;
+    if (S == 1) {
+      a.Us = c->B[c->par];
+      a.Uout = c->B[c->par ^ 1];
+      a.U0 = a.Us;
+    } else {
+      a.Us = c->B[s];
+      a.U0 = c->B[0];
+      a.Uout = last ? c->B[0] : c->B[s + 1];
+    }
+    a.Pin = c->P[c->par];
+    a.Pout = c->P[c->par ^ 1];
     a.do_cfl = last ? 1 : 0;
     DG_CUDA(c, launch_stage(c, a));
-    c->wcur ^= 1;
+    c->par ^= 1;
   }
   return DGRHD_OK;
 }
@@ -437,7 +492,7 @@ static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
 // replayed on the caller's stream; it is re-captured when dt (a kernel argument) changes.  Any
 // capture failure switches the context back to plain launches.
 static int launch_step_graph(dgrhd_ctx* c, double dt, StageArgs& a) {
-  const int par = c->wcur;
+  const int par = c->par;
   if (!c->gexec[par] || c->gdt[par] != dt) {
     if (c->gexec[par]) { cudaGraphExecDestroy(c->gexec[par]); c->gexec[par] = nullptr; }
     cudaStream_t user = c->stream;
@@ -447,7 +502,7 @@ static int launch_step_graph(dgrhd_ctx* c, double dt, StageArgs& a) {
       c->stream = c->cap_stream;
       const int r = enqueue_step(c, dt, a);
       c->stream = user;
-      c->wcur = par;
+      c->par = par;
       const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
       ok = (r == DGRHD_OK) && (e == cudaSuccess) && graph;
     }
@@ -462,7 +517,7 @@ static int launch_step_graph(dgrhd_ctx* c, double dt, StageArgs& a) {
     c->gdt[par] = dt;
   }
   DG_CUDA(c, cudaGraphLaunch(c->gexec[par], c->stream));
-  c->wcur = par ^ (c->cfg.rk_stages & 1);
+  c->par = par ^ (c->cfg.rk_stages & 1);
   return DGRHD_OK;
 }
 
@@ -491,12 +546,14 @@ extern "C" int dgrhd_step(dgrhd_ctx* c, double dt, int nsteps, double* t_inout_h
 extern "C" int dgrhd_run_host(dgrhd_ctx* c, const double* U_host_in, double* U_host_out, double dt,
                               int nsteps, double* t_inout_host) {
   if (!c || !U_host_in || !U_host_out) return fail(c, DGRHD_EINVAL, "dgrhd_run_host: NULL argument");
-  DG_CUDA(c, cudaMemcpyAsync(c->Ub, U_host_in, c->state_bytes, cudaMemcpyHostToDevice, c->stream));
-  int r = dgrhd_set_state(c, c->Ub);
+  c->par = 0;
+  DG_CUDA(c, cudaMemcpyAsync(c->B[0], U_host_in, c->state_bytes, cudaMemcpyHostToDevice, c->stream));
+  int r = refresh_state_pressure(c);
   if (r != DGRHD_OK) return r;
+  c->has_state = true;
   r = dgrhd_step(c, dt, nsteps, nullptr);
   if (r != DGRHD_OK) return r;
-  DG_CUDA(c, cudaMemcpyAsync(U_host_out, c->Ua, c->state_bytes, cudaMemcpyDeviceToHost, c->stream));
+  DG_CUDA(c, cudaMemcpyAsync(U_host_out, state_buf(c), c->state_bytes, cudaMemcpyDeviceToHost, c->stream));
   double h = 0.0;
   DG_CUDA(c, cudaMemcpyAsync(&h, &c->sc->t_acc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
   DG_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -504,13 +561,24 @@ extern "C" int dgrhd_run_host(dgrhd_ctx* c, const double* U_host_in, double* U_h
   return DGRHD_OK;
 }
 
-extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[4], int reset) {
+extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[6], int reset) {
   if (!c || !out_host) return fail(c, DGRHD_EINVAL, "dgrhd_get_counters: NULL argument");
-  dg_ull h[4];
-  DG_CUDA(c, cudaMemcpyAsync(h, c->sc->counters, sizeof h, cudaMemcpyDeviceToHost, c->stream));
-  if (reset) DG_CUDA(c, cudaMemsetAsync(c->sc->counters, 0, sizeof h, c->stream));
+  DevScalars h;
+  DG_CUDA(c, cudaMemcpyAsync(&h, c->sc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
+  if (reset) {
+    DG_CUDA(c, cudaMemsetAsync(c->sc->counters, 0, sizeof h.counters, c->stream));
+    DG_CUDA(c, cudaMemsetAsync(&c->sc->n_stages, 0, 2 * sizeof(dg_ull), c->stream));
+  }
   DG_CUDA(c, cudaStreamSynchronize(c->stream));
-  for (int i = 0; i < 4; ++i) out_host[i] = (int64_t)h[i];
+  dg_ull sum[4] = {0, 0, 0, 0};
+  for (int s = 0; s < DG_NSLOT; ++s)
+    for (int k = 0; k < 4; ++k) sum[k] += h.counters[s * DG_SLOT_STRIDE + k];
+  out_host[0] = (int64_t)sum[0];
+  out_host[1] = (int64_t)sum[1];
+  out_host[2] = (int64_t)sum[2];
+  out_host[3] = (int64_t)h.n_stages;
+  out_host[4] = (int64_t)sum[3];
+  out_host[5] = (int64_t)h.n_bad_dt;
   return DGRHD_OK;
 }
 
@@ -530,14 +598,31 @@ extern "C" int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const d
                                     double* W_dev, int* status_dev, void* cuda_stream) {
   int r = check_batch("dgrhd_con2prim_batch", eos, gamma_ad, n, U_dev, W_dev);
   if (r != DGRHD_OK || n == 0) return r;
-  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
   const EosPar e = make_eos(eos, gamma_ad);
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  if (eos == DGRHD_EOS_IDEAL)
-    dg_c2p_batch_kernel<0><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
-  else
-    dg_c2p_batch_kernel<1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+  // two adjacent states per thread with 16-byte accesses when every row is 16-byte aligned
+  const bool vec = (n % 2 == 0) && aligned16(U_dev) && aligned16(W_dev);
+  const long long nthr = vec ? n / 2 : n;
+  const unsigned nb = (unsigned)((nthr + DG_FLAT_NT - 1) / DG_FLAT_NT);
+  if (eos == DGRHD_EOS_IDEAL) {
+    if (vec) dg_c2p_batch_kernel<0, 2><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+    else dg_c2p_batch_kernel<0, 1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+  } else {
+    if (vec) dg_c2p_batch_kernel<1, 2><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+    else dg_c2p_batch_kernel<1, 1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e);
+  }
   DG_CUDA(nullptr, cudaGetLastError());
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_tm_fallback_count(int64_t* out_host, int reset, void* cuda_stream) {
+  if (!out_host) return fail(nullptr, DGRHD_EINVAL, "dgrhd_tm_fallback_count: NULL argument");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  dg_ull h = 0, z = 0;
+  DG_CUDA(nullptr, cudaMemcpyFromSymbolAsync(&h, g_tm_fallbacks, sizeof h, 0, cudaMemcpyDeviceToHost, st));
+  if (reset) DG_CUDA(nullptr, cudaMemcpyToSymbolAsync(g_tm_fallbacks, &z, sizeof z, 0, cudaMemcpyHostToDevice, st));
+  DG_CUDA(nullptr, cudaStreamSynchronize(st));
+  *out_host = (int64_t)h;
   return DGRHD_OK;
 }
 
@@ -562,13 +647,13 @@ extern "C" int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, co
                                          void* cuda_stream) {
   int r = check_batch("dgrhd_con2prim_batch_host", eos, gamma_ad, n, U_host, W_host);
   if (r != DGRHD_OK || n == 0) return r;
-  if (!stage_dev || stage_bytes < 80) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_host: staging buffer too small");
+  if (!stage_dev || stage_bytes < 160) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_host: staging buffer too small");
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int64_t cap = (int64_t)(stage_bytes / 80);
+  const int64_t cap = (int64_t)(stage_bytes / 80) / 2 * 2;      // even chunks keep the rows 16-byte aligned
   double* Ud = (double*)stage_dev;
   for (int64_t s = 0; s < n; s += cap) {
     const int64_t m = (n - s < cap) ? (n - s) : cap;
-    double* Wd = Ud + 5 * m;
+    double* Wd = Ud + 5 * ((m + 1) / 2 * 2);
     DG_CUDA(nullptr, cudaMemcpy2DAsync(Ud, m * sizeof(double), U_host + s, n * sizeof(double),
                                        m * sizeof(double), 5, cudaMemcpyHostToDevice, st));
     r = dgrhd_con2prim_batch(eos, gamma_ad, m, Ud, Wd, nullptr, cuda_stream);
@@ -582,4 +667,4 @@ extern "C" int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, co
 
 extern "C" const char* dgrhd_last_error(const dgrhd_ctx* c) { return c ? c->err : g_err; }
 
-extern "C" const char* dgrhd_version(void) { return "dgrhd 0.1 (sm_100a)"; }
+extern "C" const char* dgrhd_version(void) { return "dgrhd 0.2 (sm_100a)"; }

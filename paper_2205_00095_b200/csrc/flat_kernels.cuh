@@ -2,16 +2,21 @@
 // neighbour data (sm_100a, fp64):
 //   dg_c2p_batch_kernel    conserved -> primitive over a flat SoA batch
 //   dg_p2c_batch_kernel    primitive -> conserved (Eq. 4)
-//   dg_c2p_state_kernel    the same recovery on a context state, plus the failure counter and
-//                          the CFL wave-speed maximum (reading R11)
-//   dg_limiter_kernel      the physicality-enforcing operator on caller data
+//   dg_c2p_state_kernel    pressure (and optionally all primitives) of a context state, the failure
+//                          counter and the CFL wave-speed maximum (reading R11)
+//   dg_limiter_kernel      the physicality-enforcing operator on caller data:
+//                          the SAME device function as inside the fused stage kernel
 //   dg_dt_kernel           dt = cfl / amax on the device (no host round trip)
-// All are HBM-streaming kernels: one thread per state / node, SoA rows read and written with
-// fully coalesced 8-byte accesses (32 lanes x 8 B = one 256 B line per variable per warp).
+// All are HBM-streaming kernels.  The batch kernels give each thread NS = 2 adjacent states: one
+// 16-byte access per variable and thread (a warp moves 512 contiguous bytes per row) and two
+// independent solver streams.
 #pragma once
 #include "stage_kernel.cuh"
 
 #define DG_FLAT_NT 256
+
+// fallbacks of the Taub-Matthews solve (physics.cuh) taken by the context-free batch calls
+__device__ dg_ull g_tm_fallbacks;
 
 // block-wide max of a non-negative double -> one atomicMax on its ordered-integer image
 __device__ __forceinline__ void dg_block_atomic_max(double x, double* sRed, dg_ull* dst) {
@@ -29,22 +34,35 @@ __device__ __forceinline__ void dg_block_atomic_max(double x, double* sRed, dg_u
   }
 }
 
-#ifndef DG_C2P_MINB
-#define DG_C2P_MINB 6      // 6 x 256 threads per SM (42 registers): best of a 1..8 sweep
-#endif
-template <int EOS>
-__global__ void __launch_bounds__(DG_FLAT_NT, DG_C2P_MINB)
+// NS = 2: n even and U, W 16-byte aligned (checked by the host); NS = 1: any n / alignment.
+template <int EOS, int NS>
+__global__ void __launch_bounds__(DG_FLAT_NT, 4)
 dg_c2p_batch_kernel(long long n, const double* __restrict__ U, double* __restrict__ W,
                     int* __restrict__ status, EosPar eos) {
-  const long long i = (long long)blockIdx.x * DG_FLAT_NT + threadIdx.x;
+  const long long i = ((long long)blockIdx.x * DG_FLAT_NT + threadIdx.x) * NS;
   if (i >= n) return;
-  double u[5], w[5];
+  double u[NS][5], w[NS][5];
+  int st[NS], nfall = 0;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) u[v] = __ldg(U + v * n + i);
-  const int st = dg_con2prim<EOS>(eos, u, w);
+  for (int v = 0; v < 5; ++v) {
+    double x[NS];
+    dg_ldg_line<NS>(U + v * n + i, x);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) W[v * n + i] = w[v];
-  if (status) status[i] = st;
+    for (int s = 0; s < NS; ++s) u[s][v] = x[s];
+  }
+  dg_con2prim_n<EOS, NS, true>(eos, u, w, nullptr, st, &nfall);
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    double x[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) x[s] = w[s][v];
+    dg_st_line<NS>(W + v * n + i, x);
+  }
+  if (status) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s) status[i + s] = st[s];
+  }
+  if (EOS == DG_EOS_TM && nfall) atomicAdd(&g_tm_fallbacks, (dg_ull)nfall);
 }
 
 template <int EOS>
@@ -60,100 +78,111 @@ dg_p2c_batch_kernel(long long n, const double* __restrict__ W, double* __restric
   for (int v = 0; v < 5; ++v) U[v * n + i] = u[v];
 }
 
-// W = p(U) at every node of a state (Eq. 16); W may be NULL (CFL only).  counters[2] += failures.
-// amax (or NULL): atomicMax of sum_d cw[d] max(|lambda-_d|,|lambda+_d|) over the nodes (R11).
+// P = P(U) at every node of a state (Eq. 16), P / W optional outputs (W: all five primitives).
+// counters (or NULL): [2] += failures, [3] += Taub-Matthews fallbacks.  amax (or NULL): atomicMax of
+// sum_d cw[d] max(|lambda-_d|,|lambda+_d|) over the nodes (R11).
 template <int EOS, int ND>
 __global__ void __launch_bounds__(DG_FLAT_NT)
-dg_c2p_state_kernel(long long n, const double* __restrict__ U, double* __restrict__ W, EosPar eos,
-                    double cw0, double cw1, double cw2, dg_ull* amax, dg_ull* counters) {
+dg_c2p_state_kernel(long long n, const double* __restrict__ U, double* __restrict__ P,
+                    double* __restrict__ W, EosPar eos, double cw0, double cw1, double cw2,
+                    dg_ull* amax, dg_ull* counters) {
   __shared__ double sRed[32];
-  __shared__ int sFail;
-  if (threadIdx.x == 0) sFail = 0;
+  __shared__ int sFail[2];
+  if (threadIdx.x < 2) sFail[threadIdx.x] = 0;
   __syncthreads();
   const long long i = (long long)blockIdx.x * DG_FLAT_NT + threadIdx.x;
   double speed = 0.0;
   if (i < n) {
-    double u[5], w[5];
+    double u[1][5], w[1][5];
+    int st[1], nfall = 0;
 #pragma unroll
-    for (int v = 0; v < 5; ++v) u[v] = __ldg(U + v * n + i);
-    const int st = dg_con2prim<EOS>(eos, u, w);
+    for (int v = 0; v < 5; ++v) u[0][v] = __ldg(U + v * n + i);
+    dg_con2prim_n<EOS, 1, true>(eos, u, w, nullptr, st, &nfall);
+    if (P) P[i] = w[0][4];
     if (W) {
 #pragma unroll
-      for (int v = 0; v < 5; ++v) W[v * n + i] = w[v];
+      for (int v = 0; v < 5; ++v) W[v * n + i] = w[0][v];
     }
-    if (st != 0) atomicAdd(&sFail, 1);
+    if (st[0] != 0) atomicAdd(&sFail[0], 1);
+    if (nfall) atomicAdd(&sFail[1], nfall);
     if (amax) {
       const double cw[3] = {cw0, cw1, cw2};
-      const double s = dg_cfl_speed<EOS, ND>(eos, w, cw);
+      const double s = dg_cfl_speed<EOS, ND>(eos, u[0], w[0][4], cw);
       if (s > 0.0) speed = s;                       // NaN never wins
     }
   }
-  if (amax) dg_block_atomic_max(speed, sRed, amax);
+  if (amax) dg_block_atomic_max(speed, sRed, amax + (blockIdx.x % DG_NSLOT) * DG_SLOT_STRIDE);
   __syncthreads();
-  if (threadIdx.x == 0 && sFail && counters) atomicAdd(&counters[2], (dg_ull)sFail);
+  if (threadIdx.x == 0 && counters) {
+    const int slot = (blockIdx.x % DG_NSLOT) * DG_SLOT_STRIDE;
+    if (sFail[0]) atomicAdd(&counters[slot + 2], (dg_ull)sFail[0]);
+    if (sFail[1]) atomicAdd(&counters[slot + 3], (dg_ull)sFail[1]);
+  }
 }
 
-// The physicality-enforcing operator on a canonical-layout state, NE cells per block, one thread
-// per node.  flag[n_e] / s[n_e] optional; counters[0..1] += flagged cells / inadmissible means.
-template <int NN>
-struct LimShape {
-  static constexpr int NE = (256 / NN) > 0 ? (256 / NN) : 1;
-  static constexpr int NTN = NE * NN;
-  static constexpr int NT = (NTN + 31) / 32 * 32;
-};
-
+// The physicality-enforcing operator on a canonical-layout state: the thread mapping of the fused
+// stage kernel (a thread owns an x-line, a cell is NL consecutive lanes of one warp) over a flat list
+// of cells.  flag[n_e] / s[n_e] optional; counters[0..1] += flagged cells / inadmissible means.
 template <int ND, int N>
-__global__ void __launch_bounds__(LimShape<dg_ipow(N, ND)>::NT)
+__global__ void __launch_bounds__(128)
 dg_limiter_kernel(long long nelem, long long ndof, double* U, unsigned char* flag, double* s_out,
-                  const double* __restrict__ wnode /* [NN] tensor weights */, double wsum,
-                  double f_screen, double f_solve, double one_m_delta, dg_ull* counters) {
-  constexpr int NN = dg_ipow(N, ND);
-  using LS = LimShape<NN>;
-  __shared__ double scratch[5 * LS::NTN];
-  __shared__ double sMean[5 * LS::NE];
-  __shared__ dg_ull sSmin[LS::NE];
-  __shared__ int sFlag[LS::NE];
-  __shared__ int sCnt[2];
-  const int t = threadIdx.x;
-  const int le = t / NN, n = t - le * NN;
-  const long long e = (long long)blockIdx.x * LS::NE + le;
-  const bool active = (t < LS::NTN) && (e < nelem);
-  if (t < LS::NE) { sSmin[t] = dg_ord(1.0); sFlag[t] = 0; }
-  if (t < 2) sCnt[t] = 0;
-  __syncthreads();
-  double Uo[5] = {0, 0, 0, 0, 0};
-  const long long g = e * NN + n;
-  if (active) {
+                  LimPar lp, dg_ull* counters) {
+  constexpr int NN = dg_ipow(N, ND), NL = dg_ipow(N, ND - 1), EPW = 32 / NL;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const int ew = lane / NL, ln = lane - ew * NL;
+  const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
+  const bool active = (ew < EPW) && (e < nelem);
+  const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
+  const long long g0 = e * NN + N * ln;
+  double Uo[N][5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) Uo[v] = U[v * ndof + g];
+  for (int v = 0; v < 5; ++v) {
+    double x[N];
+    if (active) dg_ld_line<N>(U + v * ndof + g0, x);
+#pragma unroll
+    for (int m = 0; m < N; ++m) Uo[m][v] = active ? x[m] : 0.0;
   }
-  const double wn = active ? wnode[n] : 0.0;
+  double wl = 1.0;
+  if (ND >= 2) wl *= lp.w[j];
+  if (ND >= 3) wl *= lp.w[k];
+  int cnt[2] = {0, 0};
   double s;
-  const bool flagged = dg_limiter_block<NN, LS::NE, LS::NTN>(Uo, active, t, le, n, wn, wsum, f_screen,
-                                                            f_solve, one_m_delta, scratch, sMean,
-                                                            sSmin, sFlag, sCnt, s);
+  const bool flagged = dg_limiter_lines<ND, N>(Uo, active, lane, wl, lp, cnt, s);
   if (active && flagged) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) U[v * ndof + g] = Uo[v];
+    for (int v = 0; v < 5; ++v) {
+      double x[N];
+#pragma unroll
+      for (int m = 0; m < N; ++m) x[m] = Uo[m][v];
+      dg_st_line<N>(U + v * ndof + g0, x);
+    }
   }
-  if (active && n == 0) {
+  if (active && ln == 0) {
     if (flag) flag[e] = flagged ? 1 : 0;
     if (s_out) s_out[e] = s;
   }
-  __syncthreads();
-  if (t == 0 && counters) {
-    if (sCnt[0]) atomicAdd(&counters[0], (dg_ull)sCnt[0]);
-    if (sCnt[1]) atomicAdd(&counters[1], (dg_ull)sCnt[1]);
+  if (counters) {
+    if (cnt[0]) atomicAdd(&counters[0], (dg_ull)cnt[0]);
+    if (cnt[1]) atomicAdd(&counters[1], (dg_ull)cnt[1]);
   }
 }
 
 // dt for the coming step, on the device: fixed (dt_fixed > 0) or cfl / amax (reading R11); consumes
-// the accumulated maximum (the step's last stage refills it), advances the elapsed time.
+// the accumulated maximum (the step's last stage refills it), advances the elapsed time.  A maximum
+// that is not a positive finite number (every speed NaN after con2prim failures, an empty state)
+// gives dt = 0 -- the step leaves the state unchanged -- and counts one bad step.
 __global__ void dg_dt_kernel(double dt_fixed, double cfl, dg_ull* amax, double* dt_out, double* t_acc,
-                             dg_ull* n_stages, int stages) {
-  const double m = dg_unord(*amax);
-  const double dt = (dt_fixed > 0.0) ? dt_fixed : cfl / m;
-  *amax = 0ull;
+                             dg_ull* n_stages, dg_ull* n_bad_dt, int stages) {
+  double m = 0.0;
+  for (int s = 0; s < DG_NSLOT; ++s) {
+    m = fmax(m, dg_unord(amax[s * DG_SLOT_STRIDE]));
+    amax[s * DG_SLOT_STRIDE] = 0ull;
+  }
+  double dt = dt_fixed;
+  if (!(dt_fixed > 0.0)) {
+    dt = cfl / m;
+    if (!(m > 0.0) || !isfinite(dt)) { dt = 0.0; *n_bad_dt += 1ull; }
+  }
   *dt_out = dt;
   *t_acc += dt;
   *n_stages += (dg_ull)stages;

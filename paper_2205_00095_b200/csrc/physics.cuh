@@ -14,6 +14,15 @@
 #define DG_EOS_TM 1
 #define DG_INL __device__ __forceinline__
 
+// Opt-in debug build (-DDG_DEBUG_ASSERTS): bounds / ownership checks on every shared-memory slot
+// index and halo offset of the fused kernel -- the stand-in for compute-sanitizer, which is closed
+// on this GPU pool.  A failed check traps the kernel.
+#ifdef DG_DEBUG_ASSERTS
+#define DG_ASSERT(c) do { if (!(c)) { printf("DG_ASSERT %s:%d: %s\n", __FILE__, __LINE__, #c); __trap(); } } while (0)
+#else
+#define DG_ASSERT(c) do { } while (0)
+#endif
+
 // EOS constants handed to the kernels: G = Gamma, al = Gamma/(Gamma-1) (ideal EOS only).
 struct EosPar {
   double G, al;
@@ -54,26 +63,6 @@ DG_INL double dg_rho_h(const EosPar& e, double rho, double P) {
   return fma(2.5, P, 1.5 * sqrt(fma(P, P, (4.0 / 9.0) * rho * rho)));
 }
 
-// sigma_s of Eq. 22, sigma = cs^2 / (gamma^2 (1 - cs^2)), with cs^2 of Eq. 9 / Eq. 11 folded in so
-// that only one division remains:
-//   ideal: cs^2 = G P/(rho h)          => sigma = G P / (g2 (rho h - G P))
-//   TM:    cs^2 = num/den, num = 3 Th^2 + 5 Th r, den = 12 Th^2 + 2 + 12 Th r, r = sqrt(Th^2+4/9),
-//          multiply through by rho^2 (R = rho r = sqrt(P^2 + 4/9 rho^2)):
-//          sigma = (3 P^2 + 5 P R) / (g2 (9 P^2 + 2 rho^2 + 7 P R))
-template <int EOS>
-DG_INL double dg_sigma(const EosPar& e, double rho, double P, double g2) {
-  if (EOS == DG_EOS_IDEAL) {
-    double GP = e.G * P;
-    double rh = fma(e.al, P, rho);
-    return GP / (g2 * (rh - GP));
-  }
-  double R = sqrt(fma(P, P, (4.0 / 9.0) * rho * rho));
-  double PR = P * R;
-  double num = fma(3.0 * P, P, 5.0 * PR);
-  double den = fma(9.0 * P, P, fma(2.0 * rho, rho, 7.0 * PR));
-  return num / (g2 * den);
-}
-
 // Eq. 4: D = gamma rho, M = gamma rho h u, E = gamma^2 rho h - P  with gamma = sqrt(1+|u|^2).
 template <int EOS>
 DG_INL void dg_prim2con(const EosPar& e, const double W[5], double U[5]) {
@@ -88,99 +77,55 @@ DG_INL void dg_prim2con(const EosPar& e, const double W[5], double U[5]) {
   U[4] = fma(g2, rh, -W[4]);
 }
 
-// sigma_s = num/den of Eq. 22 as an unevaluated fraction (same algebra as dg_sigma).
+// What the flux and the wave speeds need at a node, from its conserved state U and its pressure
+// P = P(U) (recovered once per node by the stage that produced U and kept in HBM, 8 B per node):
+//   3-velocity  v = M / (E + P)                 (Eq. 4: M = gamma^2 rho h v, E + P = gamma^2 rho h),
+//   q = 1 - |v|^2 = 1/gamma^2,   rho h = (E + P) q,
+//   sigma_s = cs^2 / (gamma^2 (1 - cs^2)) of Eq. 22 as an unevaluated fraction num/den:
+//     ideal (Eq. 9, cs^2 = G P/(rho h)):   num = G P q,  den = rho h - G P;
+//     Taub-Matthews (Eq. 11 times rho^2, R := rho sqrt(Theta^2 + 4/9) = (2 rho h - 5 P)/3 by Eq. 10,
+//     rho^2 = 9/4 (R^2 - P^2)):            num = (3 P^2 + 5 P R) q,  den = 9/2 (P^2 + R^2) + 7 P R.
+// No square root and one reciprocal; rho itself is never needed.
 template <int EOS>
-DG_INL void dg_sigma_frac(const EosPar& e, double rho, double P, double g2, double& num, double& den) {
+DG_INL void dg_derive(const EosPar& e, const double U[5], double P, double v[3], double& num, double& den) {
+  const double r = dg_rcp(U[4] + P);
+  v[0] = U[1] * r; v[1] = U[2] * r; v[2] = U[3] * r;
+  const double q = fma(-v[0], v[0], fma(-v[1], v[1], fma(-v[2], v[2], 1.0)));
+  const double rh = (U[4] + P) * q;
   if (EOS == DG_EOS_IDEAL) {
-    num = e.G * P;
-    den = g2 * (fma(e.al, P, rho) - num);
+    const double GP = e.G * P;
+    num = GP * q;
+    den = rh - GP;
   } else {
-    const double R = sqrt(fma(P, P, (4.0 / 9.0) * rho * rho));
+    const double R = fma(2.0, rh, -5.0 * P) * (1.0 / 3.0);
     const double PR = P * R;
-    num = fma(3.0 * P, P, 5.0 * PR);
-    den = g2 * fma(9.0 * P, P, fma(2.0 * rho, rho, 7.0 * PR));
+    num = fma(3.0 * P, P, 5.0 * PR) * q;
+    den = fma(4.5, fma(P, P, R * R), 7.0 * PR);
   }
 }
 
 // lambda-+ of Eq. 21 with sigma = num/den substituted, as fractions over the common positive
 // denominator dn = den + num:   lambda-+ = (v den -+ sqrt(num ((1 - v^2) den + num))) / (den + num).
-template <int EOS>
-DG_INL void dg_speeds_frac(const EosPar& e, double rho, double P, double g2, double vd, double& nm,
-                           double& np, double& dn) {
-  double num, den;
-  dg_sigma_frac<EOS>(e, rho, P, g2, num, den);
-  const double root = dg_sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
-  const double c = vd * den;
+DG_INL void dg_speeds_frac(double vn, double num, double den, double& nm, double& np, double& dn) {
+  const double root = dg_sqrt(num * fma(fma(-vn, vn, 1.0), den, num));
+  const double c = vn * den;
   nm = c - root;
   np = c + root;
   dn = den + num;
 }
 
-// One side's contribution to the interface flux:  acc += cF F_dir(W) + cU U(W)   (Eq. 2, Eq. 4).
-template <int EOS, int dir>
-DG_INL void dg_side_accum(const EosPar& e, const double W[5], double g2, double rg, double vd,
-                          double cF, double cU, double acc[5]) {
-  const double rho = W[0], P = W[4];
-  const double rh = dg_rho_h<EOS>(e, rho, P);
-  const double g = g2 * rg;
-  const double grh = g * rh;
-  const double k = fma(cF, vd, cU);                 // cF U v_d + cU U = U (cF v_d + cU)
-  const double cP = cF * P;
-  acc[0] = fma(k, g * rho, acc[0]);
-  acc[1] = fma(k, grh * W[1], acc[1] + ((dir == 0) ? cP : 0.0));
-  acc[2] = fma(k, grh * W[2], acc[2] + ((dir == 1) ? cP : 0.0));
-  acc[3] = fma(k, grh * W[3], acc[3] + ((dir == 2) ? cP : 0.0));
-  const double E = fma(g2, rh, -P);
-  acc[4] = fma(k, E, fma(cP, vd, acc[4]));          // cF (E+P) v_d + cU E
-}
-
-// HLL two-wave flux (PAPER.md:161 cites Schneider et al.; reading R9) with lambda_L,
-// lambda_R of Eq. 23-24; U_{L,R} from W_{L,R} by Eq. 4 (reading R8).  Branch-free: the three cases
-// of R9 are the coefficient triples (1,0,0), (0,1,0), (lR,-lL,lL lR)/(lR-lL) of
-//   F = cL F_L + cR F_R + cU (U_R - U_L).
-template <int EOS, int dir>
-DG_INL void dg_hll(const EosPar& e, const double WL[5], const double WR[5], double F[5]) {
-  const double g2L = fma(WL[1], WL[1], fma(WL[2], WL[2], fma(WL[3], WL[3], 1.0)));
-  const double g2R = fma(WR[1], WR[1], fma(WR[2], WR[2], fma(WR[3], WR[3], 1.0)));
-  const double rgL = dg_rsqrt(g2L), rgR = dg_rsqrt(g2R);
-  const double vL = WL[1 + dir] * rgL, vR = WR[1 + dir] * rgR;
-  double nmL, npL, dL, nmR, npR, dR;
-  dg_speeds_frac<EOS>(e, WL[0], WL[4], g2L, vL, nmL, npL, dL);
-  dg_speeds_frac<EOS>(e, WR[0], WR[4], g2R, vR, nmR, npR, dR);
-  // lambda_L = min(nmL/dL, nmR/dR) =: nl/dl, lambda_R = max(npL/dL, npR/dR) =: nr/dr  (Eq. 23-24),
-  // compared by cross-multiplication (dL, dR > 0); the HLL weights then need one division:
-  //   (cL, cR, cU) = (nr dl, -nl dr, nl nr) / (nr dl - nl dr).
-  const bool ml = nmL * dR <= nmR * dL, mr = npL * dR >= npR * dL;
-  const double nl = ml ? nmL : nmR, dl = ml ? dL : dR;
-  const double nr = mr ? npL : npR, dr = mr ? dL : dR;
-  double cL, cR, cU;
-  if (nl >= 0.0) { cL = 1.0; cR = 0.0; cU = 0.0; }
-  else if (nr <= 0.0) { cL = 0.0; cR = 1.0; cU = 0.0; }
-  else {
-    const double a = nr * dl, b = nl * dr;
-    const double q = dg_rcp(a - b);
-    cL = a * q; cR = -b * q; cU = nl * nr * q;
-  }
-#pragma unroll
-  for (int v = 0; v < 5; ++v) F[v] = 0.0;
-  dg_side_accum<EOS, dir>(e, WL, g2L, rgL, vL, cL, -cU, F);
-  dg_side_accum<EOS, dir>(e, WR, g2R, rgR, vR, cR, cU, F);
-}
-
-// sum_d cw[d] max(|lambda-_d|, |lambda+_d|) for the CFL reduction (reading R11, Eq. 21-22).
+// sum_d cw[d] max(|lambda-_d|, |lambda+_d|) for the CFL reduction (reading R11, Eq. 21-22), from the
+// node's conserved state and pressure.
 template <int EOS, int ND>
-DG_INL double dg_cfl_speed(const EosPar& e, const double W[5], const double cw[3]) {
-  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  const double rg = dg_rsqrt(g2);
-  double num, den;
-  dg_sigma_frac<EOS>(e, W[0], W[4], g2, num, den);
+DG_INL double dg_cfl_speed(const EosPar& e, const double U[5], double P, const double cw[3]) {
+  double v[3], num, den;
+  dg_derive<EOS>(e, U, P, v, num, den);
   const double r1 = dg_rcp(den + num);
   double a = 0.0;
 #pragma unroll
   for (int d = 0; d < ND; ++d) {
-    const double vd = W[1 + d] * rg;
-    const double root = dg_sqrt(num * fma(fma(-vd, vd, 1.0), den, num));
-    a = fma(cw[d], fma(fabs(vd), den, root), a);    // max(|l-|,|l+|) (den+num) = |v| den + root
+    const double root = dg_sqrt(num * fma(fma(-v[d], v[d], 1.0), den, num));
+    a = fma(cw[d], fma(fabs(v[d]), den, root), a);   // max(|l-|,|l+|) (den+num) = |v| den + root
   }
   return a * r1;
 }
@@ -207,12 +152,11 @@ DG_INL bool dg_admissible(const double U[5], double one_minus_eps) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// con2prim.  Returns status: 0 ok, 1 inadmissible input (W = NaN), 2 P <= 0 or non-finite.
+// con2prim.  Status per state: 0 ok, 1 inadmissible input (outputs NaN), 2 P <= 0 or non-finite.
+// The solvers work on NS states of one thread in lockstep (NS independent fp64 instruction
+// streams: the iteration is latency-bound on one state); a state that has converged is frozen, so
+// every state takes exactly the iterates it would take alone.
 // ---------------------------------------------------------------------------------------------
-DG_INL bool dg_finite5(const double W[5]) {
-  return isfinite(W[0]) && isfinite(W[1]) && isfinite(W[2]) && isfinite(W[3]) && isfinite(W[4]);
-}
-
 // single-precision reciprocal / square root of a double (MUFU): only where the result feeds a
 // self-correcting iteration (Newton's step size, its starting point), never a final value.
 DG_INL double dg_rcp_lo(double x) {
@@ -226,147 +170,226 @@ DG_INL double dg_sqrt_lo(double x) {
   return (double)r;
 }
 
-// Ideal EOS: Newton on the quartic of Eq. 59 in w, beta = 2w/(1+w^2) (Eq. 58),
-// start beta_0 = |M|/E (reading R2), stop |dw| <= 1e-14 w or 16 iterations (R3), small-xi series
-// Eq. 60 for xi < 1e-4 (R4); finishing Eq. 55-57 with 1/gamma = (1-w^2)/(1+w^2).
-// fp64 divisions are the expensive operation here, so: xi, eta share 1/D; the Newton step p/p' and
-// the starting point use single-precision reciprocals (the iteration corrects them: a step with
-// relative error 6e-8 still contracts the error by that factor, and the stopping test is on the
-// fp64 step); the three divisions of the finishing formulas share one reciprocal.
-DG_INL int dg_con2prim_ideal(const EosPar& e, const double U[5], double W[5]) {
-  const double D = U[0], E = U[4];
-  const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
-  const double Mabs = dg_sqrt(M2);
-  const double rD = dg_rcp(D);
-  const double xi = Mabs * rD, eta = E * rD;                     // Eq. 38
+// Ideal EOS: the root w in (0,1) of the quartic of Eq. 59, beta = 2w/(1+w^2)
+// (Eq. 58), by Newton's iteration from beta_0 = |M|/E (reading R2), stopped at |dw| <= 1e-14 w or 16
+// iterations (R3); small-xi series Eq. 60 for xi < 1e-4 (R4).  fp64 divisions are the expensive
+// operation, so xi and eta share 1/D, and the Newton step p/p' and the starting point use
+// single-precision reciprocals (the iteration corrects them: a step with relative error 6e-8 still
+// contracts the error by that factor, and the stopping test is on the fp64 step).
+// In: D, E, |M| of admissible states.  Out: w.
+template <int NS>
+DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, const double* Mabs,
+                             double* w) {
   const double al = e.al;
-  if (xi == 0.0) {                                               // v = 0 (R4)
-    W[0] = D; W[1] = 0.0; W[2] = 0.0; W[3] = 0.0;
-    W[4] = (e.G - 1.0) * (E - D);
-    return (isfinite(W[4]) && W[4] > 0.0) ? 0 : 2;
-  }
-  double w;
-  if (xi < 1e-4) {                                               // Eq. 60
-    double a1 = fma(al, eta, -1.0);
-    double a12 = a1 * a1;
-    double am = al - 1.0;
-    double t3 = am * am / (8.0 * a12 * a12) * ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
-    w = am / (2.0 * a1) * xi + t3 * xi * xi * xi;
-  } else {
-    const double c4 = (al - 1.0) * xi;                           // Eq. 59 (c0 = c4)
-    const double c3 = -2.0 * fma(al, eta, 1.0);
-    const double c2 = 2.0 * (al + 1.0) * xi;
-    const double c1 = -2.0 * fma(al, eta, -1.0);
-    const double d3 = 4.0 * c4, d2 = 3.0 * c3, d1 = 2.0 * c2;   // p'(w) coefficients
-    const bool lo_ok = (eta < 1e30);                             // single-precision range of p'
-    if (lo_ok) {
-      const double b0 = fmin(xi * dg_rcp_lo(eta), 1.0);
-      w = fmin(b0 * dg_rcp_lo(1.0 + dg_sqrt_lo(fmax(fma(-b0, b0, 1.0), 0.0))), 0.999999);
-    } else {
-      const double b0 = xi / eta;
-      w = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
+  double c4[NS], c3[NS], c2[NS], c1[NS];
+  bool run[NS], lo[NS];
+  bool any = false;
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {
+    const double rD = dg_rcp(D[s]);
+    const double xi = Mabs[s] * rD, eta = E[s] * rD;               // Eq. 38
+    c4[s] = (al - 1.0) * xi;                                       // Eq. 59 (c0 = c4)
+    c3[s] = -2.0 * fma(al, eta, 1.0);
+    c2[s] = 2.0 * (al + 1.0) * xi;
+    c1[s] = -2.0 * fma(al, eta, -1.0);
+    lo[s] = (eta < 1e30);                                          // single-precision range of p'
+    run[s] = (xi >= 1e-4);
+    if (run[s]) {
+      if (lo[s]) {
+        const double b0 = fmin(xi * dg_rcp_lo(eta), 1.0);
+        w[s] = fmin(b0 * dg_rcp_lo(1.0 + dg_sqrt_lo(fmax(fma(-b0, b0, 1.0), 0.0))), 0.999999);
+      } else {
+        const double b0 = xi / eta;
+        w[s] = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
+      }
+    } else {                                                       // Eq. 60 (xi = 0 gives w = 0: v = 0)
+      const double a1 = fma(al, eta, -1.0);
+      const double a12 = a1 * a1;
+      const double am = al - 1.0;
+      const double t3 = am * am / (8.0 * a12 * a12) * ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
+      w[s] = am / (2.0 * a1) * xi + t3 * xi * xi * xi;
     }
+    any = any || run[s];
+  }
 #pragma unroll 1
-    for (int it = 0; it < 16; ++it) {
-      const double p = fma(fma(fma(fma(c4, w, c3), w, c2), w, c1), w, c4);
-      const double dp = fma(fma(fma(d3, w, d2), w, d1), w, c1);
-      const double dw = lo_ok ? p * dg_rcp_lo(dp) : p / dp;
-      w -= dw;
-      if (fabs(dw) <= 1e-14 * w) break;
+  for (int it = 0; it < 16 && any; ++it) {
+    any = false;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const double ws = w[s];
+      const double p = fma(fma(fma(fma(c4[s], ws, c3[s]), ws, c2[s]), ws, c1[s]), ws, c4[s]);
+      const double dp = fma(fma(fma(4.0 * c4[s], ws, 3.0 * c3[s]), ws, 2.0 * c2[s]), ws, c1[s]);
+      const double dw = lo[s] ? p * dg_rcp_lo(dp) : p / dp;
+      const double wn = ws - dw;
+      if (run[s]) {
+        w[s] = wn;
+        run[s] = !(fabs(dw) <= 1e-14 * wn);
+      }
+      any = any || run[s];
     }
   }
-  const double w2 = w * w;
-  const double op = 1.0 + w2, om = 1.0 - w2;
-  const double r = dg_rcp(op * om * Mabs);                       // one reciprocal for Eq. 55-58
-  const double r1 = r * om * Mabs;                               // 1/(1+w^2)
-  const double beta = 2.0 * w * r1;                              // Eq. 58
-  const double rho = D * om * r1;                                // Eq. 55, 1/gamma = (1-w^2)/(1+w^2)
-  const double sc = 2.0 * w * op * r;                            // gamma beta / |M|  (Eq. 56)
-  W[0] = rho;
-  W[1] = sc * U[1];
-  W[2] = sc * U[2];
-  W[3] = sc * U[3];
-  W[4] = (e.G - 1.0) * (E - beta * Mabs - rho);                  // Eq. 57
-  if (!(w >= 0.0 && w < 1.0) || !dg_finite5(W) || !(W[4] > 0.0)) return 2;
-  return 0;
 }
 
-// Taub-Matthews: cubic in Wv = gamma^2 - 1 with c1..c3 of Eq. 62-64, Q, R, d of
-// Eq. 65-67, trigonometric branch Eq. 69-70 (d < 0) or Cardano Eq. 71-73 (d >= 0), then Eq. 74-75.
-// Safeguards of reading R7: eta^2-xi^2 = (eta-xi)(eta+xi), acos argument clamped, Wv >= 0; R7b: one
-// Newton correction of the root on the cubic itself (full relative accuracy as gamma -> 1).
-DG_INL int dg_con2prim_tm(const double U[5], double W[5]) {
-  const double D = U[0], E = U[4];
-  const double M2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
-  const double Mabs = dg_sqrt(M2);
-  const double rD = dg_rcp(D);
-  const double xi = Mabs * rD, eta = E * rD;                       // Eq. 38
-  const double x2 = xi * xi, e2 = eta * eta;
-  const double dif = (eta - xi) * (eta + xi);
-  const double rden = dg_rcp(dif * dif);
-  const double sum = e2 + x2;
-  const double br = 4.0 * sum - (x2 + 1.0);
-  const double xe = x2 * e2;
-  const double c1 = (sum * br - 14.0 * xe) * (0.5 * rden);       // Eq. 62
-  const double c2 = (br * br - 57.0 * xe) * (0.0625 * rden);     // Eq. 63
-  const double c3 = -9.0 * xe * (0.0625 * rden);                 // Eq. 64
-  const double Q = (3.0 * c2 - c1 * c1) * (1.0 / 9.0);           // Eq. 66
-  const double R = (9.0 * c1 * c2 - 27.0 * c3 - 2.0 * c1 * c1 * c1) * (1.0 / 54.0);   // Eq. 67
+// Taub-Matthews: the positive root Wv = gamma^2 - 1 of the cubic of Eq. 61 with
+// c1..c3 of Eq. 62-64.  The analytic route: Q, R, d of Eq. 65-67, the trigonometric branch Eq. 69-70
+// (d < 0) or Cardano's Eq. 71-73 (d >= 0), with the safeguards of reading R7 (eta^2 - xi^2 =
+// (eta-xi)(eta+xi), acos argument clamped, Wv >= 0).  The closed form returns Wv as a difference of
+// O(c1) terms, so it is polished on the cubic itself by Newton steps (reading R7b), which makes the
+// accuracy of the transcendental part irrelevant: it is evaluated in single precision and followed by
+// three Newton steps, after which the last step must satisfy |dWv| <= 1e-13 Wv + 1e-300 (quadratic
+// convergence from a 1e-7 seed ends far below that).  A state that fails the test -- PAPER.md:392:
+// Newton on this cubic "is not guaranteed to converge to the positive root" from a poor start -- takes
+// the fallback: the same closed form in double precision plus two Newton steps; *nfall counts them.
+DG_INL double dg_tm_cubic_newton(double Wv, double c1, double c2, double c3, double& dW) {
+  const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
+  const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
+  const double Wn = Wv - f * dg_rcp(df);
+  dW = Wn - Wv;
+  return isfinite(Wn) ? fmax(Wn, 0.0) : Wv;
+}
+
+static __device__ __noinline__ double dg_tm_closed_form_fp64(double c1, double c2, double c3) {
+  const double Q = (3.0 * c2 - c1 * c1) * (1.0 / 9.0);
+  const double R = (9.0 * c1 * c2 - 27.0 * c3 - 2.0 * c1 * c1 * c1) * (1.0 / 54.0);
   const double Q3 = Q * Q * Q;
-  const double d = fma(R, R, Q3);                                // Eq. 65
-  // The transcendental part of the closed form (acos/cos, Eq. 69-70; cube roots, Eq. 71-73) is
-  // evaluated in single precision -- it only has to land in the basin of the wanted root -- and the
-  // root is then refined on the cubic of Eq. 61 itself by three Newton steps (reading R7b: the first
-  // squares the ~1e-7 seed error, the second reaches the fp64 floor for all gamma, the third covers
-  // gamma -> 1 where W = gamma^2-1 is tiny against the seed's absolute error).
+  const double d = fma(R, R, Q3);
   double Wv;
   if (d < 0.0) {
-    double arg = R * dg_rsqrt(-Q3);
-    arg = fmin(1.0, fmax(-1.0, arg));
-    const float th = acosf((float)arg) * (1.0f / 3.0f);
-    Wv = 2.0 * dg_sqrt(-Q) * (double)__cosf(th) - c1 * (1.0 / 3.0);        // Eq. 69-70
+    const double arg = fmin(1.0, fmax(-1.0, R / sqrt(-Q3)));
+    Wv = 2.0 * sqrt(-Q) * cos(acos(arg) * (1.0 / 3.0)) - c1 * (1.0 / 3.0);
   } else {
-    const double sd = dg_sqrt(d);
-    const double p = R + sd, q = R - sd;
-    const double cp = (fabs(p) < 1e37) ? (double)cbrtf((float)p) : cbrt(p);
-    const double cq = (fabs(q) < 1e37) ? (double)cbrtf((float)q) : cbrt(q);
-    Wv = cp + cq - c1 * (1.0 / 3.0);                                       // Eq. 71-73
+    const double sd = sqrt(d);
+    Wv = cbrt(R + sd) + cbrt(R - sd) - c1 * (1.0 / 3.0);
   }
   Wv = fmax(Wv, 0.0);
-#pragma unroll
-  for (int it = 0; it < 3; ++it) {                                         // R7b: Newton on Eq. 61
-    const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
-    const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
-    const double Wn = Wv - f * dg_rcp(df);
-    if (isfinite(Wn)) Wv = Wn;
-    Wv = fmax(Wv, 0.0);
-  }
-  const double g2 = Wv + 1.0;
-  const double rg = dg_rsqrt(g2);                                  // 1/gamma, Eq. 74
-  const double ug = dg_sqrt(Wv);                                   // gamma beta
-  const double beta = ug * rg;
-  const double rho = D * rg;
-  const double sc = (Mabs > 0.0) ? ug * dg_rcp(Mabs) : 0.0;
-  const double X = fma(-beta, Mabs, E);                          // E - M.v
-  W[0] = rho;
-  W[1] = sc * U[1];
-  W[2] = sc * U[2];
-  W[3] = sc * U[3];
-  W[4] = (X - rho) * (X + rho) * dg_rcp(3.0 * X);                      // Eq. 75
-  if (!dg_finite5(W) || !(W[4] > 0.0)) return 2;
-  return 0;
+  double dW;
+  Wv = dg_tm_cubic_newton(Wv, c1, c2, c3, dW);
+  Wv = dg_tm_cubic_newton(Wv, c1, c2, c3, dW);
+  return Wv;
 }
 
-template <int EOS>
-DG_INL int dg_con2prim(const EosPar& e, const double U[5], double W[5]) {
-  if (!dg_admissible(U, 1.0)) {                                  // Eq. 25: solvers need admissible U
-    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+template <int NS>
+DG_INL void dg_tm_solve_W(const double* D, const double* E, const double* Mabs, double* Wv, int* nfall) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) W[v] = qnan;
-    return 1;
+  for (int s = 0; s < NS; ++s) {
+    const double rD = dg_rcp(D[s]);
+    const double xi = Mabs[s] * rD, eta = E[s] * rD;                // Eq. 38
+    const double x2 = xi * xi, e2 = eta * eta;
+    const double dif = (eta - xi) * (eta + xi);
+    const double rden = dg_rcp(dif * dif);
+    const double sum = e2 + x2;
+    const double br = 4.0 * sum - (x2 + 1.0);
+    const double xe = x2 * e2;
+    const double c1 = (sum * br - 14.0 * xe) * (0.5 * rden);       // Eq. 62
+    const double c2 = (br * br - 57.0 * xe) * (0.0625 * rden);     // Eq. 63
+    const double c3 = -9.0 * xe * (0.0625 * rden);                 // Eq. 64
+    const double Q = (3.0 * c2 - c1 * c1) * (1.0 / 9.0);           // Eq. 66
+    const double R = (9.0 * c1 * c2 - 27.0 * c3 - 2.0 * c1 * c1 * c1) * (1.0 / 54.0);   // Eq. 67
+    const double Q3 = Q * Q * Q;
+    const double d = fma(R, R, Q3);                                // Eq. 65
+    double W0;
+    if (d < 0.0) {
+      double arg = R * dg_rsqrt(-Q3);
+      arg = fmin(1.0, fmax(-1.0, arg));
+      const float th = acosf((float)arg) * (1.0f / 3.0f);
+      W0 = 2.0 * dg_sqrt(-Q) * (double)cosf(th) - c1 * (1.0 / 3.0);          // Eq. 69-70
+    } else {
+      const double sd = dg_sqrt(d);
+      const double p = R + sd, q = R - sd;
+      const double cp = (fabs(p) < 1e37) ? (double)cbrtf((float)p) : cbrt(p);
+      const double cq = (fabs(q) < 1e37) ? (double)cbrtf((float)q) : cbrt(q);
+      W0 = cp + cq - c1 * (1.0 / 3.0);                                       // Eq. 71-73
+    }
+    W0 = fmax(W0, 0.0);
+    double dW;
+    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);                             // R7b
+    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
+    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
+    if (!(fabs(dW) <= fma(1e-13, W0, 1e-300))) {                             // not converged / NaN
+      W0 = dg_tm_closed_form_fp64(c1, c2, c3);
+      if (nfall) *nfall += 1;
+    }
+    Wv[s] = W0;
   }
-  if (EOS == DG_EOS_IDEAL) return dg_con2prim_ideal(e, U, W);
-  return dg_con2prim_tm(U, W);
+}
+
+DG_INL bool dg_finite5(const double W[5]) {
+  return isfinite(W[0]) && isfinite(W[1]) && isfinite(W[2]) && isfinite(W[3]) && isfinite(W[4]);
+}
+
+// con2prim of NS states in lockstep.  FULL: W[s] = [rho, u, P] (Eq. 55-57 / Eq. 74-75); else only the
+// pressure P[s] (what the stage kernel keeps).  st[s]: status.  nfall (or NULL): += Taub-Matthews
+// fallbacks.  Inputs failing Eq. 25 are rejected before either solver (status 1, outputs NaN).
+template <int EOS, int NS, bool FULL>
+DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5], double* P, int* st,
+                          int* nfall) {
+  const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+  double D[NS], E[NS], Mabs[NS];
+  bool adm[NS];
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {
+    adm[s] = dg_admissible(U[s], 1.0);
+    // an inadmissible state is replaced by a harmless one for the solver; its outputs are NaN
+    D[s] = adm[s] ? U[s][0] : 1.0;
+    E[s] = adm[s] ? U[s][4] : 2.0;
+    Mabs[s] = adm[s] ? dg_sqrt(fma(U[s][1], U[s][1], fma(U[s][2], U[s][2], U[s][3] * U[s][3]))) : 0.0;
+  }
+  if (EOS == DG_EOS_IDEAL) {
+    double w[NS];
+    dg_ideal_solve_w<NS>(e, D, E, Mabs, w);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const double w2 = w[s] * w[s];
+      const double op = 1.0 + w2, om = 1.0 - w2;
+      const double r1 = dg_rcp(op);
+      const double beta = 2.0 * w[s] * r1;                         // Eq. 58
+      const double rho = D[s] * om * r1;                           // Eq. 55, 1/gamma = (1-w^2)/(1+w^2)
+      const double Pv = (e.G - 1.0) * (E[s] - beta * Mabs[s] - rho);   // Eq. 57
+      bool ok = (w[s] >= 0.0 && w[s] < 1.0) && isfinite(Pv) && (Pv > 0.0);
+      if (FULL) {
+        // u = gamma v = gamma beta M/|M|, gamma beta = 2w/(1-w^2)   (Eq. 56)
+        const double sc = (Mabs[s] > 0.0) ? 2.0 * w[s] * dg_rcp(om * Mabs[s]) : 0.0;
+        W[s][0] = rho; W[s][1] = sc * U[s][1]; W[s][2] = sc * U[s][2]; W[s][3] = sc * U[s][3]; W[s][4] = Pv;
+        ok = ok && dg_finite5(W[s]);
+      } else {
+        P[s] = Pv;
+      }
+      st[s] = adm[s] ? (ok ? 0 : 2) : 1;
+    }
+  } else {
+    double Wv[NS];
+    dg_tm_solve_W<NS>(D, E, Mabs, Wv, nfall);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const double g2 = Wv[s] + 1.0;
+      const double rg = dg_rsqrt(g2);                              // 1/gamma, Eq. 74
+      const double ug = dg_sqrt(Wv[s]);                            // gamma beta
+      const double beta = ug * rg;
+      const double rho = D[s] * rg;
+      const double X = fma(-beta, Mabs[s], E[s]);                  // E - M.v
+      const double Pv = (X - rho) * (X + rho) * dg_rcp(3.0 * X);   // Eq. 75
+      bool ok = isfinite(Pv) && (Pv > 0.0);
+      if (FULL) {
+        const double sc = (Mabs[s] > 0.0) ? ug * dg_rcp(Mabs[s]) : 0.0;
+        W[s][0] = rho; W[s][1] = sc * U[s][1]; W[s][2] = sc * U[s][2]; W[s][3] = sc * U[s][3]; W[s][4] = Pv;
+        ok = ok && dg_finite5(W[s]);
+      } else {
+        P[s] = Pv;
+      }
+      st[s] = adm[s] ? (ok ? 0 : 2) : 1;
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < NS; ++s) {
+    if (!adm[s]) {
+      if (FULL) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) W[s][v] = qnan;
+      } else {
+        P[s] = qnan;
+      }
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -1,26 +1,34 @@
 // stage_kernel.cuh -- the fused SSP-RK stage kernel of the CUDA path (sm_100a, fp64).
 //
-// One launch performs, for a tile of TX x TY x TZ elements per thread block (one thread per nodal
-// point, PAPER.md:128-145 order of operations):
-//   1. per tile node a record in shared memory -- conserved state U_s, 3-velocity, pressure and the
-//      fraction sigma_s = num/den of Eq. 22 -- from the node's primitives W (recovered by the previous
-//      stage, Eq. 16) and U_s; the primitives of the one-node-deep face layer of the neighbouring
-//      elements arrive by cp.async (with GLL nodes the face interpolation of :132-134 is a gather
-//      of that layer, reading R1) and get their records (U by Eq. 4) in a dense pass;
-//   2. HLL interface flux (Eq. 21-24, reading R9) from the two records of each face point of the
-//      tile, once each, spread evenly over the block's threads                  -> shared memory;
-//   3. volume quadrature (Eq. 17) over the diagonal mass matrix, F_d = U v_d + P e_d (Eq. 2) formed on
-//      the fly from the records along the node's tensor lines (read-only: no barrier);
-//   4. surface lift (Eq. 18);
-//   MODE_RHS stops here and writes R = L(U).  MODE_STAGE continues:
-//   5. SSP-RK combine  U_out = a U0 + b (U_s + dt R)   (:147-152, reading R10), dt read from
-//      device memory;
-//   6. physicality-enforcing operator on the cell (Eq. 25-37), cell-local reductions in shared
-//      memory;
-//   7. con2prim of the new state (Eq. 16 for the next stage) and, on the step's last stage, the
-//      CFL wave-speed maximum (reading R11) reduced by warp shuffles + one atomicMax per block.
-// HBM traffic per node and stage: W_s 40 B (+halo, mostly L2 hits), U_s 40 B, U0 40 B (a != 0),
-// U_out 40 B, W_out 40 B.
+// One launch = one SSP-RK stage (PAPER.md:128-152 order of operations) over the whole mesh; a thread
+// block owns a tile of TX x TY x TZ elements and a THREAD OWNS ONE x-LINE of an element: the N = p+1
+// nodes (i = 0..N-1) at fixed (j,k).  Consequences of that mapping:
+//   * the line is contiguous in the canonical layout X[v][e][n], n = i + N (j + N k): every state
+//     access of a thread is a 16-byte vector access (N even) and a warp reads / writes whole 128-byte
+//     lines; the neighbours' facing nodal layers in y and z are lines too (16-byte cp.async);
+//   * the x-direction volume contraction (Eq. 17) runs in registers; the y and z contractions read
+//     the line-mates' records from shared memory with 16-byte loads (natural node order: the N nodes
+//     of a thread are adjacent);
+//   * a cell is N^(d-1) <= 25 consecutive lanes of ONE warp, so everything cell-local in the
+//     physicality operator (cell mean, min s) is a warp shuffle: no shared memory, no barrier;
+//   * N independent fp64 instruction streams per thread (con2prim's Newton iteration in lockstep).
+// Inputs per node: the stage state U_s and its pressure P_s = P(U_s), recovered by the stage that
+// produced U_s (8 B per node; everything else the flux and the wave speeds need follows from (U, P)
+// without a square root, physics.cuh dg_derive).  Primitives are never stored.
+// Steps:
+//   1. own lines and the one-node-deep face layers of the neighbouring elements (GLL nodes: the face
+//      interpolation of :132-134 is a gather, reading R1; periodic wrap / outflow copy, R12) -> records
+//      in shared memory: U, v = M/(E+P), P and the fraction sigma = num/den of Eq. 22;
+//   2. HLL interface flux (Eq. 21-24, reading R9) at every face point of the tile, once each, spread
+//      over the block's threads; volume quadrature (Eq. 17) over the diagonal mass matrix, F_d =
+//      U v_d + P e_d (Eq. 2) formed on the fly from the records;
+//   3. surface lift (Eq. 18).  MODE_RHS stops here and writes R = L(U).  MODE_STAGE continues:
+//   4. SSP-RK combine  U_out = a U0 + b (U_s + dt R)   (:147-152, reading R10), dt from device memory;
+//   5. physicality-enforcing operator on the cell (Eq. 25-37, :242-252);
+//   6. pressure of the new state (con2prim, Eq. 16 for the next stage) and, on the step's last stage,
+//      the CFL wave-speed maximum (reading R11): warp shuffle -> one atomicMax per block.
+// Algorithmic HBM traffic per node and stage: U_s 40 B + P_s 8 B in, U0 40 B in (a != 0), U_out 40 B +
+// P_out 8 B out = 96 / 136 B (mean over SSPRK3: 122.7 B); halo layers are L2 hits.
 #pragma once
 #include "physics.cuh"
 
@@ -28,343 +36,315 @@
 #define DG_MODE_STAGE 1
 #define DG_BC_PERIODIC 0
 #define DG_BC_OUTFLOW 1
+#define DG_NSLOT 32          // counter / CFL-maximum slots (spread same-address atomics), 128 B apart
+#define DG_SLOT_STRIDE 16    // in 8-byte words
 
 typedef unsigned long long dg_ull;
 
 __host__ __device__ constexpr int dg_ipow(int b, int e) { return e <= 0 ? 1 : b * dg_ipow(b, e - 1); }
 
-#ifndef DG_NPT64       // nodes per thread of the 3D p=3 kernel (1 or 2)
-#define DG_NPT64 1
-#endif
-#ifndef DG_T3N4X       // tile of the 3D p=3 kernel (tuning knob)
-#define DG_T3N4X 2
-#define DG_T3N4Y 2
-#define DG_T3N4Z 1
-#endif
-// elements per thread block along x,y,z for [ndim-1][N-1]
+// elements per thread block along x,y,z for [ndim-1][N-1]; every tile is 4 warps of x-line threads
+// (3D p=3: 2x2x2 elements = 512 nodes = 128 threads, two blocks per SM on shared memory)
 __host__ __device__ constexpr int dg_tile(int nd, int N, int d) {
   constexpr int t[3][5][3] = {
-      {{256, 1, 1}, {128, 1, 1}, {60, 1, 1}, {64, 1, 1}, {48, 1, 1}},
-      {{32, 8, 1}, {16, 4, 1}, {6, 4, 1}, {4, 4, 1}, {4, 2, 1}},
-      {{8, 8, 4}, {4, 4, 2}, {2, 2, 2}, {DG_T3N4X, DG_T3N4Y, DG_T3N4Z}, {2, 1, 1}}};
+      {{64, 1, 1}, {64, 1, 1}, {64, 1, 1}, {64, 1, 1}, {64, 1, 1}},
+      {{16, 8, 1}, {16, 4, 1}, {10, 4, 1}, {8, 4, 1}, {6, 4, 1}},
+      {{8, 4, 4}, {4, 4, 2}, {3, 2, 2}, {2, 2, 2}, {2, 2, 1}}};
   return t[nd - 1][N - 1][d];
 }
 
 template <int ND, int N>
 struct TileShape {
   static constexpr int NN = dg_ipow(N, ND);          // nodes per element
-  static constexpr int NF1 = dg_ipow(N, ND - 1);     // nodes per element face
+  static constexpr int NF1 = dg_ipow(N, ND - 1);     // nodes per element face = x-lines per element
+  static constexpr int NL = NF1;                     // threads per element
   static constexpr int TX = dg_tile(ND, N, 0), TY = dg_tile(ND, N, 1), TZ = dg_tile(ND, N, 2);
   static constexpr int NE = TX * TY * TZ;            // elements per tile
-  static constexpr int NTN = NE * NN;                // nodes per tile
-  // A thread owns M nodes of one element (node n0 + m NNT, m < M): M = 2 for the 64-node hexahedron, so
-  // that an element is exactly one warp (no cross-warp barrier for anything cell-local) and every
-  // thread carries two independent fp64 instruction streams; M = 1 otherwise.
-  static constexpr int M = (NN == 64) ? DG_NPT64 : 1;
-  static constexpr int NNT = NN / M;                 // threads per element
-  // Threads are organised in warp groups that own whole elements, so that everything cell-local
-  // (cell mean, min s) synchronises a group, not the block:
-  //   NNT <= 32: one warp holds EPG = 32/NNT elements (lanes >= EPG*NNT idle);  else G warps per element.
-  static constexpr int G = (NNT <= 32) ? 1 : (NNT + 31) / 32;   // warps per group
-  static constexpr int EPG = (NNT <= 32) ? 32 / NNT : 1;        // elements per group
-  static constexpr int GT = 32 * G;                           // threads per group
-  static constexpr int NG = NE / EPG;                         // groups per block
-  static_assert(NE % EPG == 0, "tile must hold a whole number of warp groups");
-  static_assert(G == 1 || NG <= 15, "named barriers 1..15");
-  static constexpr int NT = NG * GT;                 // threads per block
+  static constexpr int EPW = 32 / NL;                // elements per warp (lanes >= EPW*NL idle)
+  static constexpr int NW = (NE + EPW - 1) / EPW;    // warps per block
+  static constexpr int NT = 32 * NW;                 // threads per block
+  static constexpr bool VEC = (N % 2 == 0);          // 16-byte accesses along the line
+  // shared-memory slot of node (i,j,k) of tile element le: le*ES + i + N*j + PK*k.  The k-planes of
+  // the 3D p=3 element are padded by two slots so that the 16-byte line loads of a quarter-warp
+  // (lanes j = 0..3, k = 0..1) fall into distinct banks.
+  static constexpr int PK = (ND == 3) ? N * N + ((N == 4) ? 2 : 0) : 0;
+  static constexpr int ES = (ND == 1) ? N : ((ND == 2) ? N * N : N * PK);
+  static constexpr int NS = (NE * ES + 1) / 2 * 2;   // slots per record row
   __host__ __device__ static constexpr int T(int d) { return d == 0 ? TX : (d == 1 ? TY : TZ); }
   __host__ __device__ static constexpr int SE(int d) { return d == 0 ? 1 : (d == 1 ? TX : TX * TY); }
-  __host__ __device__ static constexpr int SN(int d) { return dg_ipow(N, d); }
+  __host__ __device__ static constexpr int SS(int d) { return d == 0 ? 1 : (d == 1 ? N : PK); }
   __host__ __device__ static constexpr int FP(int d) { return NE / T(d) * NF1; }   // points per face plane
   __host__ __device__ static constexpr int HOFF(int d) { return d <= 0 ? 0 : HOFF(d - 1) + 2 * FP(d - 1); }
   __host__ __device__ static constexpr int FOFF(int d) {
     return d <= 0 ? 0 : FOFF(d - 1) + (T(d - 1) + 1) * FP(d - 1);
   }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
+  static constexpr int NHP = (NHALO + 1) / 2 * 2;    // row stride of the halo array
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
-  // shared-memory layout, in doubles.  Node records: per tile node X[11][NTN] = D Mx My Mz E | vx vy
-  // vz | P | num den (conserved state, 3-velocity, pressure, sigma = num/den of Eq. 22); per halo
-  // point XH[9][NHALO] = D Mx My Mz E | v_normal | P | num den.
-  static constexpr int NREC = 11, HREC = 9;
-  static constexpr int O_X = 0;                          // [NREC][NTN]
-  static constexpr int O_XH = O_X + NREC * NTN;          // [HREC][NHALO]
-  static constexpr int O_FH = O_XH + HREC * NHALO;       // Fhat  [dir][plane][5][FP]
-  static constexpr int O_D = O_FH + 5 * NFACE;           // Dhat  [N][N] (padded to 32)
-  static constexpr int O_MEAN = O_D + 32;                // [NE][5]
-  static constexpr int O_SMIN = O_MEAN + 5 * NE;         // [NE] (ull)
-  static constexpr int O_RED = O_SMIN + NE;              // [32]
-  static constexpr int O_PART = O_RED + 32;              // [NE][4][5] partial sums of the cell mean
-  static constexpr int O_FLAG = O_PART + 20 * NE;        // ints: [NE] flags + [4] counters
-  static constexpr int SMEM_BYTES = O_FLAG * 8 + (NE + 4) * 4 + 16;
+  // shared memory, in doubles.  Node records X[11][NS] = D Mx My Mz E | vx vy vz | P | num den (conserved
+  // state, 3-velocity, pressure, sigma = num/den of Eq. 22); halo points XH[6][NHP] = D Mx My Mz E | P.
+  static constexpr int NREC = 11, HREC = 6;
+  static constexpr int O_X = 0;
+  static constexpr int O_XH = O_X + NREC * NS;
+  static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][plane][5][FP]
+  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = y, z
+  static constexpr int O_RED = O_D + 2 * 26;         // [32] block reduction of the CFL maximum
+  static constexpr int O_CNT = O_RED + 32;           // 4 ints
+  static constexpr int SMEM_BYTES = (O_CNT + 2) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
-  static constexpr int BLK_THR = 1024 / NT;
-  static constexpr int MINB = (BLK_SMEM < BLK_THR ? BLK_SMEM : BLK_THR) > 0 ? (BLK_SMEM < BLK_THR ? BLK_SMEM : BLK_THR) : 1;
+  static constexpr int BLK_REG = 65536 / (NT * 128);   // leave >= 128 registers per thread
+  static constexpr int MINB = (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) > 0 ? (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) : 1;
 };
 
 struct StageArgs {
-  const double* Win;      // W_s[5][ndof] primitives of the stage input state
-  const double* Us;       // U_s[5][ndof]
-  const double* U0;       // U at the start of the step (read only if a != 0)
-  double* Uout;           // may alias Us (each thread reads and writes its own node only)
-  double* Wout;           // must not alias Win
+  const double* Us;       // U_s[5][ndof]   stage input state (16-byte aligned if N is even)
+  const double* Pin;      // P_s[ndof]      its pressure
+  const double* U0;       // U at the start of the step (read only if a != 0); may alias Uout
+  double* Uout;           // must not alias Us (neighbouring blocks read their halo from Us)
+  double* Pout;           // must not alias Pin
   double* Rout;           // MODE_RHS: R = L(U_s)
   long long ndof;
-  int ne[3], bc[3];
-  double rh[3];           // 2/h_d
-  double cw[3];           // (2p+1)/h_d
+  int ne[3];
   double a, b;            // Shu-Osher coefficients of this stage
   const double* dt_ptr;   // device
   double f_screen, f_solve, one_m_delta;   // 1-eps_q/2, 1-eps_q, 1-delta_s
   EosPar eos;
-  dg_ull* amax;           // ordered-int image of the CFL maximum (atomicMax)
+  double cw[3];           // (2p+1)/h_d
+  dg_ull* amax;           // [DG_NSLOT] ordered-int images of the CFL maximum (atomicMax)
   int do_cfl;
-  dg_ull* counters;       // [0] n_flagged [1] n_bad_mean [2] n_c2p_fail
-  double Dhat[25];        // Dhat[i*N+q]
+  dg_ull* counters;       // [DG_NSLOT][n_flagged, n_bad_mean, n_c2p_fail, n_tm_fallback]
+  double Dx[25];          // (2/h_x) Dhat[i*N+q]
+  double Dy[25], Dz[25];
   double w[5];            // GLL weights
-  double lift, wsum;      // 1/w_0, sum of the tensor weights (node order)
+  double lift[3];         // (2/h_d) / w_0
+  double wsum;            // sum of the tensor weights
   int mode;               // DG_MODE_RHS / DG_MODE_STAGE
   int hoff[3][2], hfix[3][2];   // halo: global-index offset of the facing node (minus, plus side)
 };
 
 // ---------------------------------------------------------------------------------------------
-// Physicality operator on a block of cells (PAPER.md:242-252 steps 1-4), one thread per node.
-// Must be called by every thread of the block.  Uo: the node's state, limited in place.
-//   le, n: element-in-block and node-in-element of this thread; wn: tensor GLL weight of the node.
-//   scratch: >= 5*NTN doubles of shared memory free for use; sMean [NE][5]; sSmin [NE]; sFlag [NE];
-//   sCnt[0..1] += flagged cells / bad means of this block.
-// Returns this cell's flag; s_out receives the blend factor (1 if unflagged).
+// line access helpers: N consecutive doubles, 16-byte vectors when N is even (p 16-byte aligned)
 // ---------------------------------------------------------------------------------------------
-template <int NN, int NE, int NTN>
-__device__ __forceinline__ bool dg_limiter_block(double Uo[5], bool active, int t, int le, int n,
-                                                 double wn, double wsum, double f_screen,
-                                                 double f_solve, double one_m_delta,
-                                                 double* scratch, double* sMean, dg_ull* sSmin,
-                                                 int* sFlag, int* sCnt, double& s_out) {
+template <int N>
+DG_INL void dg_ld_line(const double* p, double x[N]) {
+  if (N % 2 == 0) {
+#pragma unroll
+    for (int m = 0; m < N / 2; ++m) {
+      const double2 t = *reinterpret_cast<const double2*>(p + 2 * m);
+      x[2 * m] = t.x; x[2 * m + 1] = t.y;
+    }
+  } else {
+#pragma unroll
+    for (int m = 0; m < N; ++m) x[m] = p[m];
+  }
+}
+template <int N>
+DG_INL void dg_ldg_line(const double* p, double x[N]) {      // read-only global data
+  if (N % 2 == 0) {
+#pragma unroll
+    for (int m = 0; m < N / 2; ++m) {
+      const double2 t = __ldg(reinterpret_cast<const double2*>(p + 2 * m));
+      x[2 * m] = t.x; x[2 * m + 1] = t.y;
+    }
+  } else {
+#pragma unroll
+    for (int m = 0; m < N; ++m) x[m] = __ldg(p + m);
+  }
+}
+template <int N>
+DG_INL void dg_st_line(double* p, const double x[N]) {
+  if (N % 2 == 0) {
+#pragma unroll
+    for (int m = 0; m < N / 2; ++m) *reinterpret_cast<double2*>(p + 2 * m) = make_double2(x[2 * m], x[2 * m + 1]);
+  } else {
+#pragma unroll
+    for (int m = 0; m < N; ++m) p[m] = x[m];
+  }
+}
+// asynchronous copy global -> shared of a line (LDGSTS): no register is held while in flight
+template <int N>
+DG_INL void dg_async_line(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (N % 2 == 0) {
+#pragma unroll
+    for (int m = 0; m < N / 2; ++m)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + 16 * m), "l"(gmem_src + 2 * m) : "memory");
+  } else {
+#pragma unroll
+    for (int m = 0; m < N; ++m)
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d + 8 * m), "l"(gmem_src + m) : "memory");
+  }
+}
+DG_INL void dg_async_copy8(double* smem_dst, const double* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)),
+               "l"(gmem_src) : "memory");
+}
+DG_INL void dg_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// ---------------------------------------------------------------------------------------------
+// The physicality-enforcing operator (PAPER.md:242-252 steps 1-4) on the cells of one warp.  A
+// thread owns the x-line j,k of its cell: nodes Uo[0..N-1], limited in place; the NL lines of a cell
+// are consecutive lanes starting at a multiple of NL.  MUST be called by all 32 lanes (inactive
+// lanes pass active = false).  This one function serves the fused stage kernel and the stand-alone
+// dgrhd_enforce_physicality kernel.
+//   wl: product of the GLL weights of the line's fixed coordinates (w_j w_k); w: the 1D weights.
+//   cnt[0], cnt[1] += cells flagged / cells with an inadmissible mean, counted on the cell's first lane.
+// Returns the cell's flag; s_out = blend factor (1 if unflagged, 0 for an inadmissible mean, R13d).
+// ---------------------------------------------------------------------------------------------
+struct LimPar {
+  double w[5];
+  double wsum, f_screen, f_solve, one_m_delta;
+};
+
+template <int NL>
+DG_INL double dg_cell_sum(double x, int base) {
+  if ((NL & (NL - 1)) == 0) {                      // power of two: butterfly inside the aligned group
+#pragma unroll
+    for (int o = NL / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    return x;
+  }
+  double acc = 0.0;                                // fixed lane order, the same on every lane
+#pragma unroll
+  for (int o = 0; o < NL; ++o) acc += __shfl_sync(0xffffffffu, x, min(base + o, 31));
+  return acc;
+}
+template <int NL>
+DG_INL double dg_cell_min(double x, int base) {
+  if ((NL & (NL - 1)) == 0) {
+#pragma unroll
+    for (int o = NL / 2; o > 0; o >>= 1) x = fmin(x, __shfl_xor_sync(0xffffffffu, x, o));
+    return x;
+  }
+  double acc = x;
+#pragma unroll
+  for (int o = 0; o < NL; ++o) acc = fmin(acc, __shfl_sync(0xffffffffu, x, min(base + o, 31)));
+  return acc;
+}
+
+template <int ND, int N>
+DG_INL bool dg_limiter_lines(double (*Uo)[5], bool active, int lane, double wl, const LimPar& lp,
+                             int cnt[2], double& s_out) {
+  constexpr int NL = dg_ipow(N, ND - 1);
   s_out = 1.0;
-  bool bad = active && !dg_admissible(Uo, f_screen);               // step 1: screen (R13e)
-  if (bad) sFlag[le] = 1;
-  if (!__syncthreads_or(bad)) return false;                        // nothing to do in this block
-  const bool flagged = active && (sFlag[le] != 0);
-  if (flagged) {
+  bool bad = false;
+  if (active) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) scratch[v * NTN + t] = wn * Uo[v];
+    for (int m = 0; m < N; ++m) bad = bad || !dg_admissible(Uo[m], lp.f_screen);   // step 1: screen (R13e)
   }
-  __syncthreads();
-  if (flagged) {                                                   // cell average, fixed node order
-    for (int v = n; v < 5; v += NN) {
-      const double* p = scratch + v * NTN + le * NN;
-      double acc = 0.0;
-      for (int m = 0; m < NN; ++m) acc += p[m];
-      sMean[le * 5 + v] = acc / wsum;
-    }
-  }
-  __syncthreads();
+  const unsigned ball = __ballot_sync(0xffffffffu, bad);
+  if (ball == 0u) return false;                   // nothing flagged in this warp (the common case)
+  const int base = (lane / NL) * NL;
+  const unsigned cmask = ((NL >= 32) ? 0xffffffffu : ((1u << NL) - 1u)) << base;
+  const bool flagged = active && ((ball & cmask) != 0u);
   double Ub[5];
-  if (flagged) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) Ub[v] = sMean[le * 5 + v];
-    const bool mean_ok = dg_admissible(Ub, f_solve);               // step 2 (reading R13d)
-    double si = 0.0;
-    if (mean_ok) {
-      si = dg_limiter_node_s(Ub, Uo, f_solve);                     // step 3
-      if (!(si >= 0.0)) si = 0.0;
+  for (int v = 0; v < 5; ++v) {                   // cell average: line partial sums, then across lanes
+    double part = 0.0;
+    if (flagged) {
+#pragma unroll
+      for (int m = 0; m < N; ++m) part = fma(wl * lp.w[m], Uo[m][v], part);
     }
-    if (si < 1.0) atomicMin(&sSmin[le], dg_ord(si));               // step 4: s = min_i s_i
-    if (n == 0) {
-      atomicAdd(&sCnt[0], 1);
-      if (!mean_ok) atomicAdd(&sCnt[1], 1);
+    Ub[v] = dg_cell_sum<NL>(part, base) / lp.wsum;
+  }
+  double si = 1.0;
+  bool mean_ok = true;
+  if (flagged) {
+    mean_ok = dg_admissible(Ub, lp.f_solve);      // step 2 (reading R13d)
+    if (mean_ok) {
+#pragma unroll
+      for (int m = 0; m < N; ++m) {
+        double sm_ = dg_limiter_node_s(Ub, Uo[m], lp.f_solve);     // step 3
+        if (!(sm_ >= 0.0)) sm_ = 0.0;
+        si = fmin(si, sm_);
+      }
+    } else {
+      si = 0.0;
     }
   }
-  __syncthreads();
+  const double smin = dg_cell_min<NL>(si, base);  // step 4: s = min_i s_i
   if (flagged) {
-    const double s = one_m_delta * dg_unord(sSmin[le]);            // R13c
+    const double s = lp.one_m_delta * smin;       // R13c
     const double tt = 1.0 - s;
 #pragma unroll
-    for (int v = 0; v < 5; ++v)                                    // Eq. 26 from the nearer end (R14)
-      Uo[v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[v], Uo[v]) : fma(s, Uo[v] - Ub[v], Ub[v]);
+    for (int m = 0; m < N; ++m) {
+#pragma unroll
+      for (int v = 0; v < 5; ++v)                 // Eq. 26 from the nearer end (R14)
+        Uo[m][v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[m][v], Uo[m][v]) : fma(s, Uo[m][v] - Ub[v], Ub[v]);
+    }
     s_out = s;
+    if (lane == base) {
+      cnt[0] += 1;
+      if (!mean_ok) cnt[1] += 1;
+    }
   }
   return flagged;
 }
 
 // ---------------------------------------------------------------------------------------------
-// helpers: decode a face point / halo point of direction D of the tile
+// One side of a face point: from a tile node record (rows U | v | P | num den) or from a halo point
+// (rows U | P; velocity and sigma derived here -- each halo point is used by exactly one face point)
 // ---------------------------------------------------------------------------------------------
-template <int ND, int N, int D>
-struct DirInfo {
-  using TS = TileShape<ND, N>;
-  static constexpr int A = (D == 0) ? 1 : 0;        // transverse axes (ascending)
-  static constexpr int B = (D == 2) ? 1 : 2;
-  static constexpr int FPD = TS::FP(D);
-  // transverse decode of a face-plane point fp = tn + NF1*te
-  __device__ __forceinline__ static void split(int fp, int& la, int& lb, int& ca, int& cb) {
-    const int te = fp / TS::NF1, tn = fp - te * TS::NF1;
-    la = te % TS::T(A);
-    lb = te / TS::T(A);
-    ca = tn % N;
-    cb = tn / N;
-  }
-};
-
-// Record of a tile node in the shared node array from its primitives W and conserved state U: U (for
-// the Riemann flux and the volume flux F_d = U v_d + P e_d), the 3-velocity v = u/gamma, P, and
-// sigma_s = num/den of Eq. 22 as an unevaluated fraction.
-template <int ND, int N, int EOS>
-__device__ __forceinline__ void dg_node_record(const EosPar& eos, const double W[5], const double U[5],
-                                               double* X, int slot) {
-  constexpr int S = TileShape<ND, N>::NTN;
-  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  const double rg = dg_rsqrt(g2);
-  double num, den;
-  dg_sigma_frac<EOS>(eos, W[0], W[4], g2, num, den);
-  double* x = X + slot;
+template <int ND, int N, int EOS, int D>
+DG_INL void dg_side_node(const double* x, double U[5], double& vn, double& P, double& num, double& den) {
+  constexpr int S = TileShape<ND, N>::NS;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) x[v * S] = U[v];
-  x[5 * S] = W[1] * rg;
-  x[6 * S] = W[2] * rg;
-  x[7 * S] = W[3] * rg;
-  x[8 * S] = W[4];
-  x[9 * S] = num;
-  x[10 * S] = den;
+  for (int v = 0; v < 5; ++v) U[v] = x[v * S];
+  vn = x[(5 + D) * S];
+  P = x[8 * S];
+  num = x[9 * S];
+  den = x[10 * S];
+}
+template <int ND, int N, int EOS, int D>
+DG_INL void dg_side_halo(const EosPar& eos, const double* h, double U[5], double& vn, double& P,
+                         double& num, double& den) {
+  constexpr int S = TileShape<ND, N>::NHP;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) U[v] = h[v * S];
+  P = h[5 * S];
+  double v3[3];
+  dg_derive<EOS>(eos, U, P, v3, num, den);
+  vn = v3[D];
 }
 
-// Record of halo point h: its primitives W sit in rows 0..4 of XH; replace them by U (Eq. 4, reading
-// R8) and add the velocity component normal to the face, P and the sigma fraction.
-template <int ND, int N, int EOS>
-__device__ __forceinline__ void dg_halo_record(const EosPar& eos, double* XH, int h) {
-  using TS = TileShape<ND, N>;
-  constexpr int S = TS::NHALO;
-  double* x = XH + h;
-  double W[5];
-#pragma unroll
-  for (int v = 0; v < 5; ++v) W[v] = x[v * S];
-  const int D = (ND > 2 && h >= TS::HOFF(2)) ? 2 : ((ND > 1 && h >= TS::HOFF(1)) ? 1 : 0);
-  const double g2 = fma(W[1], W[1], fma(W[2], W[2], fma(W[3], W[3], 1.0)));
-  const double rg = dg_rsqrt(g2);
-  double num, den;
-  dg_sigma_frac<EOS>(eos, W[0], W[4], g2, num, den);
-  const double rh = dg_rho_h<EOS>(eos, W[0], W[4]);
-  const double g = g2 * rg, grh = g * rh;
-  x[0] = g * W[0];
-  x[1 * S] = grh * W[1];
-  x[2 * S] = grh * W[2];
-  x[3 * S] = grh * W[3];
-  x[4 * S] = fma(g2, rh, -W[4]);
-  x[5 * S] = ((D == 0) ? W[1] : ((D == 1) ? W[2] : W[3])) * rg;
-  x[6 * S] = W[4];
-  x[7 * S] = num;
-  x[8 * S] = den;
-}
-
-__device__ __forceinline__ void dg_async_copy8(double* smem_dst, const double* gmem_src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)),
-               "l"(gmem_src) : "memory");
-}
-__device__ __forceinline__ void dg_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-// Halo of direction D: each node on the tile's boundary in direction D fetches the primitives of the
-// node facing it in the neighbouring element (periodic wrap; at an outflow boundary its own, reading
-// R12) -- global index = own index + a block-uniform offset -- into the halo slot that equals the
-// node's face-point index (rows 0..4; the record is completed in a dense pass over the halo slots).
-template <int ND, int N, int D>
-__device__ __forceinline__ void dg_load_halo(const StageArgs& a, double* XH, bool active, int g,
-                                             const int lc[3], const int in[3], const int org[3],
-                                             const int teff[3]) {
-  using TS = TileShape<ND, N>;
-  using DI = DirInfo<ND, N, D>;
-  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
-  // offsets of the facing node: interior value + a correction on the first / last tile of the axis
-  // (periodic wrap or outflow), both precomputed by the host (StageArgs::hoff, hfix)
-  const int off0 = a.hoff[D][0] + ((org[D] == 0) ? a.hfix[D][0] : 0);
-  const int off1 = a.hoff[D][1] + ((org[D] + teff[D] == a.ne[D]) ? a.hfix[D][1] : 0);
-  if (!active) return;
-  const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
-  double* dst = XH + (TS::HOFF(D) + fp);
-  // asynchronous 8-byte copies global -> shared (LDGSTS): all halo rows of the block are in flight at
-  // once and no register is held; the caller waits with dg_async_wait() before the block barrier
-  if (in[D] == 0 && lc[D] == 0) {
-    const double* src = a.Win + (g + off0);
-#pragma unroll
-    for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * TS::NHALO, src + v * a.ndof);
-  }
-  if (in[D] == N - 1 && lc[D] == teff[D] - 1) {
-    const double* src = a.Win + (g + off1);
-#pragma unroll
-    for (int v = 0; v < 5; ++v) dg_async_copy8(dst + FPD + v * TS::NHALO, src + v * a.ndof);
-  }
-}
-
-// Barrier over one warp group (G warps): __syncwarp for G = 1, else the named barrier grp+1.
-template <int G>
-__device__ __forceinline__ void dg_gsync(int grp) {
-  if (G == 1) __syncwarp();
-  else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "r"(32 * G) : "memory");
-}
-
-// Lift of the interface flux onto a node (Eq. 18 over the diagonal mass matrix) for direction D:
-//   + c * Fhat at the element's minus face if the node sits on it, - c * Fhat at its plus face,
-//   c = (2/h_D) / w_0.
-template <int ND, int N, int D>
-__device__ __forceinline__ void dg_add_surface(const double* Fh, const int lc[3], const int in[3],
-                                               double c, double R[5]) {
-  using TS = TileShape<ND, N>;
-  using DI = DirInfo<ND, N, D>;
-  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD;
-  if (in[D] != 0 && in[D] != N - 1) return;
-  const int fp = (in[A] + N * in[B]) + TS::NF1 * (lc[A] + TS::T(A) * lc[B]);
-  const double* base = Fh + 5 * TS::FOFF(D) + fp;
-  if (in[D] == 0) {
-    const double* p = base + lc[D] * 5 * FPD;
-#pragma unroll
-    for (int v = 0; v < 5; ++v) R[v] = fma(c, p[v * FPD], R[v]);
-  }
-  if (in[D] == N - 1) {
-    const double* p = base + (lc[D] + 1) * 5 * FPD;
-#pragma unroll
-    for (int v = 0; v < 5; ++v) R[v] = fma(-c, p[v * FPD], R[v]);
-  }
-}
-
-// HLL flux (reading R9, Eq. 21-24) at face point fl of direction D from the node records of its two
+// HLL flux (reading R9, Eq. 21-24) at face point fl of direction D from the records of its two
 // sides:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in the energy).
-template <int ND, int N, int D>
-__device__ __forceinline__ void dg_face_flux(const double* X, const double* XH, double* Fh, int fl,
-                                             const int teff[3]) {
+template <int ND, int N, int EOS, int D>
+DG_INL void dg_face_flux(const EosPar& eos, const double* X, const double* XH, double* Fh, int fl,
+                         const int teff[3]) {
   using TS = TileShape<ND, N>;
-  using DI = DirInfo<ND, N, D>;
-  constexpr int A = DI::A, B = DI::B, FPD = DI::FPD, ST = TS::NTN, SH = TS::NHALO;
+  constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
+  constexpr int FPD = TS::FP(D);
   const int p = fl / FPD, fp = fl - p * FPD;
-  int la, lb, ca, cb;
-  DI::split(fp, la, lb, ca, cb);
+  const int te = fp / TS::NF1, tn = fp - te * TS::NF1;
+  const int la = te % TS::T(A), lb = te / TS::T(A);
+  const int ca = tn % N, cb = tn / N;
   if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return;
-  const int tnode = ca * TS::SN(A) + cb * TS::SN(B);
+  const int tnode = ca * TS::SS(A) + cb * TS::SS(B);
   const int telem = la * TS::SE(A) + lb * TS::SE(B);
-  // left / right records: a tile node (stride ST, rows v=5+D P=8 num=9 den=10) or a halo point
-  // (stride SH, rows v=5 P=6 num=7 den=8)
-  const bool hL = (p < 1), hR = (p >= teff[D]);
-  const double* xl = hL ? XH + (TS::HOFF(D) + fp)
-                        : X + ((telem + (p - 1) * TS::SE(D)) * TS::NN + tnode + (N - 1) * TS::SN(D));
-  const double* xr = hR ? XH + (TS::HOFF(D) + FPD + fp) : X + ((telem + p * TS::SE(D)) * TS::NN + tnode);
-  const int sl = hL ? SH : ST, sr = hR ? SH : ST;
-  const double* ql = xl + (hL ? 5 * SH : (5 + D) * ST);              // v, then (P, num, den) at +kl
-  const double* qr = xr + (hR ? 5 * SH : (5 + D) * ST);
-  const int kl = hL ? SH : (3 - D) * ST, kr = hR ? SH : (3 - D) * ST;
-  const double vL = ql[0], vR = qr[0];
-  const double PL = ql[kl], PR = qr[kr];
+  double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
+  if (p < 1) {
+    DG_ASSERT(TS::HOFF(D) + fp < TS::NHALO);
+    dg_side_halo<ND, N, EOS, D>(eos, XH + (TS::HOFF(D) + fp), UL, vL, PL, numL, denL);
+  } else {
+    const int s = (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
+    DG_ASSERT(s >= 0 && s < TS::NS);
+    dg_side_node<ND, N, EOS, D>(X + s, UL, vL, PL, numL, denL);
+  }
+  if (p >= teff[D]) {
+    DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
+    dg_side_halo<ND, N, EOS, D>(eos, XH + (TS::HOFF(D) + FPD + fp), UR, vR, PR, numR, denR);
+  } else {
+    const int s = (telem + p * TS::SE(D)) * TS::ES + tnode;
+    DG_ASSERT(s >= 0 && s < TS::NS);
+    dg_side_node<ND, N, EOS, D>(X + s, UR, vR, PR, numR, denR);
+  }
   double nmL, npL, dL, nmR, npR, dR;
-  {
-    const double num = ql[kl + sl], den = ql[kl + 2 * sl];
-    const double root = dg_sqrt(num * fma(fma(-vL, vL, 1.0), den, num));
-    const double c = vL * den;
-    nmL = c - root; npL = c + root; dL = den + num;
-  }
-  {
-    const double num = qr[kr + sr], den = qr[kr + 2 * sr];
-    const double root = dg_sqrt(num * fma(fma(-vR, vR, 1.0), den, num));
-    const double c = vR * den;
-    nmR = c - root; npR = c + root; dR = den + num;
-  }
-  const bool ml = nmL * dR <= nmR * dL, mr = npL * dR >= npR * dL;       // Eq. 23-24 by cross-multiplication
+  dg_speeds_frac(vL, numL, denL, nmL, npL, dL);
+  dg_speeds_frac(vR, numR, denR, nmR, npR, dR);
+  // lambda_L = min(nmL/dL, nmR/dR) =: nl/dl, lambda_R = max(npL/dL, npR/dR) =: nr/dr  (Eq. 23-24),
+  // compared by cross-multiplication (dL, dR > 0); the HLL weights then need one division:
+  //   (cL, cR, cU) = (nr dl, -nl dr, nl nr) / (nr dl - nl dr).
+  const bool ml = nmL * dR <= nmR * dL, mr = npL * dR >= npR * dL;
   const double nl = ml ? nmL : nmR, dl = ml ? dL : dR;
   const double nr = mr ? npL : npR, dr = mr ? dL : dR;
   double cL, cR, cU;
@@ -378,319 +358,351 @@ __device__ __forceinline__ void dg_face_flux(const double* X, const double* XH, 
   const double kL = fma(cL, vL, -cU), kR = fma(cR, vR, cU);
   const double pL = cL * PL, pR = cR * PR;
   double* pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
+  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
-    double f = fma(kL, xl[v * sl], kR * xr[v * sr]);
+    double f = fma(kL, UL[v], kR * UR[v]);
     if (v == 1 + D) f += pL + pR;
     if (v == 4) f = fma(pL, vL, fma(pR, vR, f));
     pF[v * FPD] = f;
   }
 }
 
-// Volume term of direction D for this thread's node (Eq. 17 over the diagonal mass matrix): the
-// tensor-line contraction of F_D(W_q) = U_q v_q + P_q e_D, formed on the fly from the node records.
+// Volume term of direction D = 1 (y) or 2 (z) for the N nodes of this thread's line (Eq. 17 over the
+// diagonal mass matrix): for each q the line at index q along D -- N adjacent slots -- is read with
+// vector loads and F_D = U v_D + P e_D is formed on the fly.  dh: (2/h_D) Dhat[id][q] of this
+// thread's index id along D.
 template <int ND, int N, int D>
-__device__ __forceinline__ void dg_volume(const StageArgs& a, const double* sD, const double* X, int ti,
-                                          const int in[3], double R[5]) {
+DG_INL void dg_volume_line(const double* X, const double* dh, int s_line0, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int NTOT = TS::NTN;
-  const int id = in[D];
-  const double* line = X + (ti - id * TS::SN(D));
-  const double* dh = sD + id * N;
+  constexpr int S = TS::NS;
 #pragma unroll
   for (int q = 0; q < N; ++q) {
-    const double* x = line + q * TS::SN(D);
-    const double dq = a.rh[D] * dh[q];
-    const double t = dq * x[(5 + D) * NTOT];
-    const double Pq = x[8 * NTOT];
+    const double* x = X + s_line0 + q * TS::SS(D);
+    const double c = dh[q];
+    double vd[N], Pq[N], t[N];
+    dg_ld_line<N>(x + (5 + D) * S, vd);
+    dg_ld_line<N>(x + 8 * S, Pq);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) R[v] = fma(t, x[v * NTOT], R[v]);
-    R[1 + D] = fma(dq, Pq, R[1 + D]);
-    R[4] = fma(t, Pq, R[4]);
+    for (int m = 0; m < N; ++m) t[m] = c * vd[m];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      double u[N];
+      dg_ld_line<N>(x + v * S, u);
+#pragma unroll
+      for (int m = 0; m < N; ++m) R[m][v] = fma(t[m], u[m], R[m][v]);
+    }
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+      R[m][1 + D] = fma(c, Pq[m], R[m][1 + D]);
+      R[m][4] = fma(t[m], Pq[m], R[m][4]);
+    }
   }
 }
 
-
-// Physicality operator on the cells of one warp group (PAPER.md:242-252 steps 1-4); a thread owns the
-// M nodes n0 + m NNT of its cell (tile slots ti0 + m NNT).  Cell-local reductions go through shared
-// memory with group barriers only.  Must be called by every thread of the group.  Uo: the nodes'
-// states, limited in place.
-template <int ND, int N>
-__device__ __forceinline__ void dg_limiter_group(double (*Uo)[5], bool active, int ti0, int le, int n0,
-                                                 int grp, const double* wn, const StageArgs& a,
-                                                 double* scratch, double* sPart, double* sMean,
-                                                 dg_ull* sSmin, int* sFlag, int* sCnt) {
+// Lift of the interface flux of direction D = 1 or 2 onto the line's nodes (Eq. 18): the line lies
+// in the element's minus face (id == 0: + c Fhat) and / or plus face (id == N-1: - c Fhat).
+template <int ND, int N, int D>
+DG_INL void dg_lift_line(const double* Fh, int id, int lcD, int fp0, double c, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int NN = TS::NN, NTN = TS::NTN, M = TS::M, NNT = TS::NNT;
-  bool bad = false;
-  if (active) {
+  constexpr int FPD = TS::FP(D);
+  const double* base = Fh + 5 * TS::FOFF(D) + fp0;
+  if (id == 0) {
+    const double* p = base + lcD * 5 * FPD;
 #pragma unroll
-    for (int m = 0; m < M; ++m) bad = bad || !dg_admissible(Uo[m], a.f_screen);   // step 1: screen (R13e)
-  }
-  if (bad) sFlag[le] = 1;
-  dg_gsync<TS::G>(grp);
-  const bool flagged = active && (sFlag[le] != 0);
-  // nothing flagged in this warp group (the common case): done, no further group barriers
-  const bool any = (TS::G == 1) ? (__any_sync(0xffffffffu, flagged) != 0) : (sFlag[grp * TS::EPG] != 0);
-  if (!any) return;
-  if (flagged) {
+    for (int v = 0; v < 5; ++v) {
+      double f[N];
+      dg_ld_line<N>(p + v * FPD, f);
 #pragma unroll
-    for (int m = 0; m < M; ++m) {
-#pragma unroll
-      for (int v = 0; v < 5; ++v) scratch[v * NTN + ti0 + m * NNT] = wn[m] * Uo[m][v];
+      for (int m = 0; m < N; ++m) R[m][v] = fma(c, f[m], R[m][v]);
     }
   }
-  dg_gsync<TS::G>(grp);
-  // cell average: J interleaved partial sums per variable (5 J lanes), then their sum by 5 lanes
-  constexpr int J = (NNT >= 20) ? 4 : NNT / 5;
-  if (J == 0) {                                                     // tiny cells: one lane sums
-    if (flagged && n0 == 0) {
-      for (int v = 0; v < 5; ++v) {
-        double acc = 0.0;
-        for (int q = 0; q < NN; ++q) acc += scratch[v * NTN + le * NN + q];
-        sMean[le * 5 + v] = acc / a.wsum;
-      }
-    }
-  } else {
-    if (flagged && n0 < 5 * J) {
-      const int v = n0 % 5, j = n0 / 5;
-      const double* p = scratch + v * NTN + le * NN;
-      double acc = 0.0;
-      for (int q = j; q < NN; q += J) acc += p[q];
-      sPart[le * 20 + n0] = acc;
-    }
-    dg_gsync<TS::G>(grp);
-    if (flagged && n0 < 5) {
-      double acc = 0.0;
+  if (id == N - 1) {
+    const double* p = base + (lcD + 1) * 5 * FPD;
 #pragma unroll
-      for (int j = 0; j < J; ++j) acc += sPart[le * 20 + 5 * j + n0];
-      sMean[le * 5 + n0] = acc / a.wsum;
-    }
-  }
-  dg_gsync<TS::G>(grp);
-  double Ub[5];
-  if (flagged) {
+    for (int v = 0; v < 5; ++v) {
+      double f[N];
+      dg_ld_line<N>(p + v * FPD, f);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) Ub[v] = sMean[le * 5 + v];
-    const bool mean_ok = dg_admissible(Ub, a.f_solve);               // step 2 (reading R13d)
-    double si = 0.0;
-    if (mean_ok) {
-      si = 1.0;
-#pragma unroll
-      for (int m = 0; m < M; ++m) {
-        double sm_ = dg_limiter_node_s(Ub, Uo[m], a.f_solve);        // step 3
-        if (!(sm_ >= 0.0)) sm_ = 0.0;
-        si = fmin(si, sm_);
-      }
-    }
-    if (si < 1.0) atomicMin(&sSmin[le], dg_ord(si));                 // step 4: s = min_i s_i
-    if (n0 == 0) {
-      atomicAdd(&sCnt[0], 1);
-      if (!mean_ok) atomicAdd(&sCnt[1], 1);
-    }
-  }
-  dg_gsync<TS::G>(grp);
-  if (flagged) {
-    const double s = a.one_m_delta * dg_unord(sSmin[le]);            // R13c
-    const double tt = 1.0 - s;
-#pragma unroll
-    for (int m = 0; m < M; ++m) {
-#pragma unroll
-      for (int v = 0; v < 5; ++v)                                    // Eq. 26 from the nearer end (R14)
-        Uo[m][v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[m][v], Uo[m][v]) : fma(s, Uo[m][v] - Ub[v], Ub[v]);
+      for (int m = 0; m < N; ++m) R[m][v] = fma(-c, f[m], R[m][v]);
     }
   }
 }
 
-// resident blocks per SM the register allocation must allow: up to 1024 threads (32 warps) per SM,
-// but no more blocks than the shared memory of an SM holds
-#ifndef DG_MINB
-#define DG_MINB TileShape<ND, N>::MINB
-#endif
 template <int ND, int N, int EOS>
-__global__ void __launch_bounds__(TileShape<ND, N>::NT, DG_MINB)
+__global__ void __launch_bounds__(TileShape<ND, N>::NT, TileShape<ND, N>::MINB)
 dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
-  constexpr int NN = TS::NN, NTN = TS::NTN, NT = TS::NT, NE = TS::NE;
+  constexpr int NN = TS::NN, NT = TS::NT, NL = TS::NL, NS = TS::NS, NHP = TS::NHP;
   extern __shared__ __align__(16) double sm[];
   double* X = sm + TS::O_X;
   double* XH = sm + TS::O_XH;
   double* Fh = sm + TS::O_FH;
-  double* sD = sm + TS::O_D;
-  double* sMean = sm + TS::O_MEAN;
-  dg_ull* sSmin = reinterpret_cast<dg_ull*>(sm + TS::O_SMIN);
+  double* sDy = sm + TS::O_D;
+  double* sDz = sDy + 26;
   double* sRed = sm + TS::O_RED;
-  double* sPart = sm + TS::O_PART;
-  int* sFlag = reinterpret_cast<int*>(sm + TS::O_FLAG);
-  int* sCnt = sFlag + NE;
+  int* sCnt = reinterpret_cast<int*>(sm + TS::O_CNT);
 
-  // tile of this block
+  // tile of this block; element, line (j,k) of this thread
   const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
-  // warp group, element and the M nodes (n0 + m NNT) of this thread
-  constexpr int M = TS::M, NNT = TS::NNT;
-  const int t = threadIdx.x;
-  const int grp = t / TS::GT, r = t - grp * TS::GT;
-  const int le = grp * TS::EPG + r / NNT, n0 = r % NNT;
-  const int ti0 = le * NN + n0;                                      // tile slot of node m: ti0 + m NNT
+  const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
+  const int ew = lane / NL, ln = lane - ew * NL;
+  const int le = wrp * TS::EPW + ew;
+  const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
-  const bool active = (r < TS::EPG * NNT) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
-  int g0 = 0;                                                        // ndof < 2^31 (dgrhd_create)
-  if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + n0;
-  int in[M][3];
-#pragma unroll
-  for (int m = 0; m < M; ++m) {
-    const int n = n0 + m * NNT;
-    in[m][0] = n % N; in[m][1] = (n / N) % N; in[m][2] = n / (N * N);
-  }
-  if (t < NE) { sSmin[t] = dg_ord(1.0); sFlag[t] = 0; }
+  const bool active = (ew < TS::EPW) && (le < TS::NE) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
+  const int s0 = le * TS::ES + N * j + TS::PK * k;                   // slot of node i = 0 of the line
+  int g0 = 0;                                                        // its global index; ndof < 2^31
+  if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + N * ln;
   if (t < 4) sCnt[t] = 0;
-  if (t < N * N) sD[t] = a.Dhat[t];
+  if (ND >= 2 && t < N * N) sDy[t] = a.Dy[t];
+  if (ND >= 3 && t < N * N) sDz[t] = a.Dz[t];
 
-  // 1. primitives (recovered by the previous stage) and conserved state of the nodes -> their records
-  //    in the shared node array; primitives of the neighbours' facing nodal layers -> halo slots
-#pragma unroll
-  for (int m = 0; m < M; ++m) {
-    dg_load_halo<ND, N, 0>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
-    if constexpr (ND > 1) dg_load_halo<ND, N, 1>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
-    if constexpr (ND > 2) dg_load_halo<ND, N, 2>(a, XH, active, g0 + m * NNT, lc, in[m], org, teff);
-  }
-  double Un[M][5];
-#pragma unroll
-  for (int m = 0; m < M; ++m)
-#pragma unroll
-    for (int v = 0; v < 5; ++v) Un[m][v] = 0.0;
+  // 1a. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
+  //     periodic wrap or, at an outflow boundary, the node itself) -> halo rows U | P, asynchronously
   if (active) {
-    double Wn[M][5];
+    {                                                                // x: one point per line and side
+      const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
+      if (lc[0] == 0) {
+        const int g = g0 + a.hoff[0][0] + ((org[0] == 0) ? a.hfix[0][0] : 0);
+        DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + fp < TS::NHALO);
+        double* dst = XH + (TS::HOFF(0) + fp);
 #pragma unroll
-    for (int m = 0; m < M; ++m) {
+        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_copy8(dst + 5 * NHP, a.Pin + g);
+      }
+      if (lc[0] == teff[0] - 1) {
+        const int g = g0 + (N - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
+        DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + TS::FP(0) + fp < TS::NHALO);
+        double* dst = XH + (TS::HOFF(0) + TS::FP(0) + fp);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) {
-        Wn[m][v] = __ldg(a.Win + v * a.ndof + g0 + m * NNT);
-        Un[m][v] = a.Us[v * a.ndof + g0 + m * NNT];
+        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_copy8(dst + 5 * NHP, a.Pin + g);
       }
     }
+    if constexpr (ND >= 2) {                                         // y: the whole line
+      const int fp0 = N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]);
+      if (j == 0 && lc[1] == 0) {
+        const int g = g0 + a.hoff[1][0] + ((org[1] == 0) ? a.hfix[1][0] : 0);
+        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(1) + fp0 + N <= TS::NHALO);
+        double* dst = XH + (TS::HOFF(1) + fp0);
 #pragma unroll
-    for (int m = 0; m < M; ++m) dg_node_record<ND, N, EOS>(a.eos, Wn[m], Un[m], X, ti0 + m * NNT);
-    if (a.mode == DG_MODE_STAGE && a.a != 0.0) {         // U0 is needed last: warm L2 now
+        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+      }
+      if (j == N - 1 && lc[1] == teff[1] - 1) {
+        const int g = g0 + a.hoff[1][1] + ((org[1] + teff[1] == a.ne[1]) ? a.hfix[1][1] : 0);
+        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + N <= TS::NHALO);
+        double* dst = XH + (TS::HOFF(1) + TS::FP(1) + fp0);
 #pragma unroll
-      for (int m = 0; m < M; ++m)
+        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+      }
+    }
+    if constexpr (ND >= 3) {                                         // z: the whole line
+      const int fp0 = N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]);
+      if (k == 0 && lc[2] == 0) {
+        const int g = g0 + a.hoff[2][0] + ((org[2] == 0) ? a.hfix[2][0] : 0);
+        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(2) + fp0 + N <= TS::NHALO);
+        double* dst = XH + (TS::HOFF(2) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v)
-          asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0 + m * NNT));
+        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+      }
+      if (k == N - 1 && lc[2] == teff[2] - 1) {
+        const int g = g0 + a.hoff[2][1] + ((org[2] + teff[2] == a.ne[2]) ? a.hfix[2][1] : 0);
+        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + N <= TS::NHALO);
+        double* dst = XH + (TS::HOFF(2) + TS::FP(2) + fp0);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+      }
+    }
+  }
+
+  // 1b. own line: U_s, P_s -> records; the x-direction flux stays in registers
+  double R[N][5];
+#pragma unroll
+  for (int m = 0; m < N; ++m)
+#pragma unroll
+    for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
+  if (active) {
+    double Ul[5][N], Pl[N];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dg_ldg_line<N>(a.Us + v * a.ndof + g0, Ul[v]);
+    dg_ldg_line<N>(a.Pin + g0, Pl);
+    if (a.mode == DG_MODE_STAGE && a.a != 0.0) {          // U0 is needed last: warm L2 now
+#pragma unroll
+      for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0));
+    }
+    double vl[3][N], numl[N], denl[N];
+#pragma unroll
+    for (int m = 0; m < N; ++m) {
+      const double Um[5] = {Ul[0][m], Ul[1][m], Ul[2][m], Ul[3][m], Ul[4][m]};
+      double v3[3];
+      dg_derive<EOS>(a.eos, Um, Pl[m], v3, numl[m], denl[m]);
+      vl[0][m] = v3[0]; vl[1][m] = v3[1]; vl[2][m] = v3[2];
+    }
+    DG_ASSERT(s0 >= 0 && s0 + N <= NS);
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dg_st_line<N>(X + v * NS + s0, Ul[v]);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) dg_st_line<N>(X + (5 + d) * NS + s0, vl[d]);
+    dg_st_line<N>(X + 8 * NS + s0, Pl);
+    dg_st_line<N>(X + 9 * NS + s0, numl);
+    dg_st_line<N>(X + 10 * NS + s0, denl);
+    // volume term, x direction, in registers: R_i += sum_q (2/h_x) Dhat[i][q] F_x(q)
+    if (N > 1) {
+      double Fx[N][5];
+#pragma unroll
+      for (int m = 0; m < N; ++m) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Fx[m][v] = Ul[v][m] * vl[0][m];
+        Fx[m][1] += Pl[m];
+        Fx[m][4] = fma(Pl[m], vl[0][m], Fx[m][4]);
+      }
+#pragma unroll
+      for (int m = 0; m < N; ++m)
+#pragma unroll
+        for (int q = 0; q < N; ++q) {
+          const double c = a.Dx[m * N + q];
+#pragma unroll
+          for (int v = 0; v < 5; ++v) R[m][v] = fma(c, Fx[q][v], R[m][v]);
+        }
     }
   }
   dg_async_wait();
   __syncthreads();
-  // records of the halo points (U from W by Eq. 4, reading R8), a dense pass over the halo slots
-  for (int h = t; h < TS::NHALO; h += NT) dg_halo_record<ND, N, EOS>(a.eos, XH, h);
-  __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, 0>(X, XH, Fh, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, (ND > 1 ? 1 : 0)>(X, XH, Fh, f - TS::FOFF(1), teff);
-    else dg_face_flux<ND, N, (ND > 2 ? 2 : 0)>(X, XH, Fh, f - TS::FOFF(2), teff);
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, EOS, 0>(a.eos, X, XH, Fh, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(1), teff);
+    else dg_face_flux<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(2), teff);
   }
-
-  // 3. volume quadrature: reads the node array only, so it needs no barrier and fills the time
-  //    other warps still spend on face fluxes
-  double R[M][5];
-#pragma unroll
-  for (int m = 0; m < M; ++m)
-#pragma unroll
-    for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
-  if (active) {
-#pragma unroll
-    for (int m = 0; m < M; ++m) {
-      dg_volume<ND, N, 0>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
-      if constexpr (ND > 1) dg_volume<ND, N, 1>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
-      if constexpr (ND > 2) dg_volume<ND, N, 2>(a, sD, X, ti0 + m * NNT, in[m], R[m]);
-    }
+  //    volume quadrature, y and z: reads the records only, so it needs no barrier here
+  if (active && N > 1) {
+    if constexpr (ND >= 2) dg_volume_line<ND, N, 1>(X, sDy + j * N, le * TS::ES + TS::PK * k, R);
+    if constexpr (ND >= 3) dg_volume_line<ND, N, 2>(X, sDz + k * N, le * TS::ES + N * j, R);
   }
   __syncthreads();
 
-  // 4. surface lift
+  // 3. surface lift
   if (active) {
+    {
+      const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
+      const double* base = Fh + fp;
+      const double* pm = base + lc[0] * 5 * TS::FP(0);
+      const double* pp = base + (lc[0] + 1) * 5 * TS::FP(0);
 #pragma unroll
-    for (int m = 0; m < M; ++m) {
-      dg_add_surface<ND, N, 0>(Fh, lc, in[m], a.rh[0] * a.lift, R[m]);
-      if constexpr (ND > 1) dg_add_surface<ND, N, 1>(Fh, lc, in[m], a.rh[1] * a.lift, R[m]);
-      if constexpr (ND > 2) dg_add_surface<ND, N, 2>(Fh, lc, in[m], a.rh[2] * a.lift, R[m]);
+      for (int v = 0; v < 5; ++v) {
+        R[0][v] = fma(a.lift[0], pm[v * TS::FP(0)], R[0][v]);
+        R[N - 1][v] = fma(-a.lift[0], pp[v * TS::FP(0)], R[N - 1][v]);
+      }
     }
+    if constexpr (ND >= 2)
+      dg_lift_line<ND, N, 1>(Fh, j, lc[1], N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
+    if constexpr (ND >= 3)
+      dg_lift_line<ND, N, 2>(Fh, k, lc[2], N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
 #pragma unroll
-      for (int m = 0; m < M; ++m)
+      for (int v = 0; v < 5; ++v) {
+        double r[N];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) a.Rout[v * a.ndof + g0 + m * NNT] = R[m][v];
+        for (int m = 0; m < N; ++m) r[m] = R[m][v];
+        dg_st_line<N>(a.Rout + v * a.ndof + g0, r);
+      }
     }
     return;
   }
 
-  // 5. SSP-RK combine (Shu-Osher form)
+  // 4. SSP-RK combine (Shu-Osher form); U_s comes back from the thread's own records
   const double dt = *a.dt_ptr;
-  double Uo[M][5];
+  double Uo[N][5];
 #pragma unroll
-  for (int m = 0; m < M; ++m)
+  for (int v = 0; v < 5; ++v) {
+    double u[N];
+    if (active) dg_ld_line<N>(X + v * NS + s0, u);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) Uo[m][v] = a.b * fma(dt, R[m][v], Un[m][v]);
+    for (int m = 0; m < N; ++m) Uo[m][v] = active ? a.b * fma(dt, R[m][v], u[m]) : 0.0;
+  }
   if (a.a != 0.0 && active) {
 #pragma unroll
-    for (int m = 0; m < M; ++m)
+    for (int v = 0; v < 5; ++v) {
+      double u0[N];
+      dg_ld_line<N>(a.U0 + v * a.ndof + g0, u0);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) Uo[m][v] = fma(a.a, a.U0[v * a.ndof + g0 + m * NNT], Uo[m][v]);
+      for (int m = 0; m < N; ++m) Uo[m][v] = fma(a.a, u0[m], Uo[m][v]);
+    }
   }
 
-  // 6. physicality-enforcing operator (cell-local; the node array is free after the barrier above)
-  double wn[M];
+  // 5. physicality-enforcing operator (cell-local: warp shuffles)
+  int cnt[4] = {0, 0, 0, 0};
+  {
+    LimPar lp;
 #pragma unroll
-  for (int m = 0; m < M; ++m) {
-    wn[m] = a.w[in[m][0]];
-    if (ND > 1) wn[m] *= a.w[in[m][1]];
-    if (ND > 2) wn[m] *= a.w[in[m][2]];
+    for (int m = 0; m < 5; ++m) lp.w[m] = a.w[m];
+    lp.wsum = a.wsum; lp.f_screen = a.f_screen; lp.f_solve = a.f_solve; lp.one_m_delta = a.one_m_delta;
+    double wl = 1.0;
+    if (ND >= 2) wl *= a.w[j];
+    if (ND >= 3) wl *= a.w[k];
+    double s_unused;
+    dg_limiter_lines<ND, N>(Uo, active, lane, wl, lp, cnt, s_unused);
   }
-  dg_limiter_group<ND, N>(Uo, active, ti0, le, n0, grp, wn, a, X, sPart, sMean, sSmin, sFlag, sCnt);
 
-  // 7. primitives of the new state, CFL maximum
+  // 6. pressure of the new state (for the next stage), CFL maximum
   double speed = 0.0;
   if (active) {
-    double Wo[M][5];
+    double Po[N];
+    int st[N];
+    dg_con2prim_n<EOS, N, false>(a.eos, Uo, nullptr, Po, st, &cnt[3]);
 #pragma unroll
-    for (int m = 0; m < M; ++m) {
-      const int st = dg_con2prim<EOS>(a.eos, Uo[m], Wo[m]);
-      if (st != 0) atomicAdd(&sCnt[2], 1);
+    for (int m = 0; m < N; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      double u[N];
+#pragma unroll
+      for (int m = 0; m < N; ++m) u[m] = Uo[m][v];
+      dg_st_line<N>(a.Uout + v * a.ndof + g0, u);
     }
-#pragma unroll
-    for (int m = 0; m < M; ++m)
-#pragma unroll
-      for (int v = 0; v < 5; ++v) {
-        a.Uout[v * a.ndof + g0 + m * NNT] = Uo[m][v];
-        a.Wout[v * a.ndof + g0 + m * NNT] = Wo[m][v];
-      }
+    dg_st_line<N>(a.Pout + g0, Po);
     if (a.do_cfl) {
 #pragma unroll
-      for (int m = 0; m < M; ++m) {
-        const double sp = dg_cfl_speed<EOS, ND>(a.eos, Wo[m], a.cw);
-        if (sp > 0.0) speed = fmax(speed, sp);
+      for (int m = 0; m < N; ++m) {
+        const double sp = dg_cfl_speed<EOS, ND>(a.eos, Uo[m], Po[m], a.cw);
+        if (sp > 0.0) speed = fmax(speed, sp);            // NaN never wins
       }
+    }
+  }
+  // block totals: counters (rare) and the CFL maximum
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const unsigned any = __ballot_sync(0xffffffffu, cnt[c] != 0);
+    if (any) {
+      int x = cnt[c];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+      if (lane == 0) atomicAdd(&sCnt[c], x);
     }
   }
   if (a.do_cfl) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
-    if ((t & 31) == 0) sRed[t >> 5] = speed;
+    if (lane == 0) sRed[wrp] = speed;
   }
   __syncthreads();
   if (t < 32) {
+    const int slot = (int)((blockIdx.x + 7u * blockIdx.y + 13u * blockIdx.z) % DG_NSLOT) * DG_SLOT_STRIDE;
     if (a.do_cfl) {
       double y = (t < NT / 32) ? sRed[t] : 0.0;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) y = fmax(y, __shfl_xor_sync(0xffffffffu, y, o));
-      if (t == 0 && y > 0.0) atomicMax(a.amax, dg_ord(y));
+      if (t == 0 && y > 0.0) atomicMax(a.amax + slot, dg_ord(y));
     }
-    if (t < 3 && sCnt[t]) atomicAdd(&a.counters[t], (dg_ull)sCnt[t]);
+    if (t < 4 && sCnt[t]) atomicAdd(&a.counters[slot + t], (dg_ull)sCnt[t]);
   }
 }

@@ -37,7 +37,7 @@ def test_argument_errors_are_detected_without_a_device():
     L = b.lib()
     assert b"sm_100a" in L.dgrhd_version()
     good = b.make_config(2, [8, 8], [0, 0], [1, 1], [0, 1], 2, 1, 0.0)
-    assert b.dgrhd_workspace_bytes(good) >= 4 * 8 * 8 * 9 * 5 * 8
+    assert b.dgrhd_workspace_bytes(good) >= (3 * 5 + 2) * 8 * 8 * 9 * 8      # 3 states + 2 pressure buffers
 
     def mutated(**kw):
         c = b.make_config(1, [8], [0], [1], [0], 2, 0, 5 / 3)

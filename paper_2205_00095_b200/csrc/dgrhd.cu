@@ -191,7 +191,7 @@ static cudaError_t launch_limiter_nd(dgrhd_ctx* c, double* U, unsigned char* fla
   const LimPar lp = make_limpar(c);
 #define DG_GO(NV)                                                                                  \
   {                                                                                                \
-    constexpr int EPB = 4 * (32 / dg_ipow(NV, ND - 1));                                            \
+    constexpr int EPB = 4 * TileShape<ND, NV>::EPW;                                                \
     const unsigned nb = (unsigned)((c->nelem + EPB - 1) / EPB);                                    \
     dg_limiter_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, flag, s, lp, counters); \
   }

@@ -121,43 +121,49 @@ dg_c2p_state_kernel(long long n, const double* __restrict__ U, double* __restric
 }
 
 // The physicality-enforcing operator on a canonical-layout state: the thread mapping of the fused
-// stage kernel (a thread owns an x-line, a cell is NL consecutive lanes of one warp) over a flat list
-// of cells.  flag[n_e] / s[n_e] optional; counters[0..1] += flagged cells / inadmissible means.
+// stage kernel (a thread owns a segment of an x-line, a cell is NL consecutive lanes of one warp) over
+// a flat list of cells.  flag[n_e] / s[n_e] optional; counters[0..1] += flagged cells / inadmissible
+// means.
 template <int ND, int N>
 __global__ void __launch_bounds__(128)
 dg_limiter_kernel(long long nelem, long long ndof, double* U, unsigned char* flag, double* s_out,
                   LimPar lp, dg_ull* counters) {
-  constexpr int NN = dg_ipow(N, ND), NL = dg_ipow(N, ND - 1), EPW = 32 / NL;
+  using TS = TileShape<ND, N>;
+  constexpr int NN = TS::NN, NL = TS::NL, EPW = TS::EPW, SEG = TS::SEG, NSEG = TS::NSEG;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-  const int ew = lane / NL, ln = lane - ew * NL;
+  const int ew = lane / NL, lt = lane - ew * NL;
+  const int h = lt % NSEG, ln = lt / NSEG;
   const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
   const bool active = (ew < EPW) && (e < nelem);
   const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
-  const long long g0 = e * NN + N * ln;
-  double Uo[N][5];
+  const long long g0 = e * NN + N * ln + h * SEG;
+  double Uo[SEG][5];
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
-    double x[N];
-    if (active) dg_ld_line<N>(U + v * ndof + g0, x);
+    double x[SEG];
+    if (active) dg_ld_line<SEG>(U + v * ndof + g0, x);
 #pragma unroll
-    for (int m = 0; m < N; ++m) Uo[m][v] = active ? x[m] : 0.0;
+    for (int m = 0; m < SEG; ++m) Uo[m][v] = active ? x[m] : 0.0;
   }
   double wl = 1.0;
   if (ND >= 2) wl *= lp.w[j];
   if (ND >= 3) wl *= lp.w[k];
+  double wn[SEG];
+#pragma unroll
+  for (int m = 0; m < SEG; ++m) wn[m] = wl * ((NSEG > 1 && h > 0) ? lp.w[(SEG + m) % 5] : lp.w[m]);
   int cnt[2] = {0, 0};
   double s;
-  const bool flagged = dg_limiter_lines<ND, N>(Uo, active, lane, wl, lp, cnt, s);
+  const bool flagged = dg_limiter_cells<NL, SEG>(Uo, active, lane, wn, lp, cnt, s);
   if (active && flagged) {
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double x[N];
+      double x[SEG];
 #pragma unroll
-      for (int m = 0; m < N; ++m) x[m] = Uo[m][v];
-      dg_st_line<N>(U + v * ndof + g0, x);
+      for (int m = 0; m < SEG; ++m) x[m] = Uo[m][v];
+      dg_st_line<SEG>(U + v * ndof + g0, x);
     }
   }
-  if (active && ln == 0) {
+  if (active && lt == 0) {
     if (flag) flag[e] = flagged ? 1 : 0;
     if (s_out) s_out[e] = s;
   }

@@ -54,6 +54,14 @@ DG_INL double dg_sqrt(double x) {                 // x >= 0; sqrt(0) = 0
   const double s = x * r;
   return fma(fma(-s, s, x), 0.5 * r, s);
 }
+// sqrt(x + 1e-300): one add instead of the compare-and-select guard; identical to dg_sqrt(x) for every
+// normal x and 1e-150 instead of 0 at x = 0 -- used where that is harmless (|M|, wave-speed radicands)
+DG_INL double dg_sqrt_p(double x) {
+  const double y = x + 1e-300;
+  const double r = dg_rsqrt(y);
+  const double s = y * r;
+  return fma(fma(-s, s, y), 0.5 * r, s);
+}
 
 // rho*h as a function of (rho, P):  ideal Eq. 8: rho h = rho + al P;
 // Taub-Matthews Eq. 10: rho h = 5/2 P + 3/2 sqrt(P^2 + 4/9 rho^2)   (h(Theta) times rho).
@@ -107,7 +115,7 @@ DG_INL void dg_derive(const EosPar& e, const double U[5], double P, double v[3],
 // lambda-+ of Eq. 21 with sigma = num/den substituted, as fractions over the common positive
 // denominator dn = den + num:   lambda-+ = (v den -+ sqrt(num ((1 - v^2) den + num))) / (den + num).
 DG_INL void dg_speeds_frac(double vn, double num, double den, double& nm, double& np, double& dn) {
-  const double root = dg_sqrt(num * fma(fma(-vn, vn, 1.0), den, num));
+  const double root = dg_sqrt_p(num * fma(fma(-vn, vn, 1.0), den, num));
   const double c = vn * den;
   nm = c - root;
   np = c + root;
@@ -124,7 +132,7 @@ DG_INL double dg_cfl_speed(const EosPar& e, const double U[5], double P, const d
   double a = 0.0;
 #pragma unroll
   for (int d = 0; d < ND; ++d) {
-    const double root = dg_sqrt(num * fma(fma(-v[d], v[d], 1.0), den, num));
+    const double root = dg_sqrt_p(num * fma(fma(-v[d], v[d], 1.0), den, num));
     a = fma(cw[d], fma(fabs(v[d]), den, root), a);   // max(|l-|,|l+|) (den+num) = |v| den + root
   }
   return a * r1;
@@ -173,42 +181,55 @@ DG_INL double dg_sqrt_lo(double x) {
 // Ideal EOS: the root w in (0,1) of the quartic of Eq. 59, beta = 2w/(1+w^2)
 // (Eq. 58), by Newton's iteration from beta_0 = |M|/E (reading R2), stopped at |dw| <= 1e-14 w or 16
 // iterations (R3); small-xi series Eq. 60 for xi < 1e-4 (R4).  fp64 divisions are the expensive
-// operation, so xi and eta share 1/D, and the Newton step p/p' and the starting point use
-// single-precision reciprocals (the iteration corrects them: a step with relative error 6e-8 still
-// contracts the error by that factor, and the stopping test is on the fp64 step).
+// operation, so xi and eta share 1/D, and the Newton step p/p' and the starting point are formed in
+// single precision (the iteration corrects them: a step with relative error 6e-8 still contracts the
+// error by that factor, and the stopping test is on the fp64 step).  States outside the single-
+// precision range (eta >= 1e30) or on the series branch take the out-of-line general routine.
 // In: D, E, |M| of admissible states.  Out: w.
+static __device__ __noinline__ double dg_ideal_w_general(double al, double xi, double eta) {
+  if (xi < 1e-4) {                                                 // Eq. 60 (xi = 0 gives w = 0: v = 0)
+    const double a1 = fma(al, eta, -1.0);
+    const double a12 = a1 * a1;
+    const double am = al - 1.0;
+    const double t3 = am * am / (8.0 * a12 * a12) * ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
+    return am / (2.0 * a1) * xi + t3 * xi * xi * xi;
+  }
+  const double c4 = (al - 1.0) * xi, c3 = -2.0 * fma(al, eta, 1.0), c2 = 2.0 * (al + 1.0) * xi,
+               c1 = -2.0 * fma(al, eta, -1.0);
+  const double b0 = xi / eta;
+  double w = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
+  for (int it = 0; it < 16; ++it) {
+    const double p = fma(fma(fma(fma(c4, w, c3), w, c2), w, c1), w, c4);
+    const double dp = fma(fma(fma(4.0 * c4, w, 3.0 * c3), w, 2.0 * c2), w, c1);
+    const double dw = p / dp;
+    w -= dw;
+    if (fabs(dw) <= 1e-14 * w) break;
+  }
+  return w;
+}
+
 template <int NS>
 DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, const double* Mabs,
                              double* w) {
   const double al = e.al;
-  double c4[NS], c3[NS], c2[NS], c1[NS];
-  bool run[NS], lo[NS];
+  double c4[NS], c3[NS], c2[NS], c1[NS], xi[NS], eta[NS];
+  bool run[NS], general[NS];
   bool any = false;
 #pragma unroll
   for (int s = 0; s < NS; ++s) {
     const double rD = dg_rcp(D[s]);
-    const double xi = Mabs[s] * rD, eta = E[s] * rD;               // Eq. 38
-    c4[s] = (al - 1.0) * xi;                                       // Eq. 59 (c0 = c4)
-    c3[s] = -2.0 * fma(al, eta, 1.0);
-    c2[s] = 2.0 * (al + 1.0) * xi;
-    c1[s] = -2.0 * fma(al, eta, -1.0);
-    lo[s] = (eta < 1e30);                                          // single-precision range of p'
-    run[s] = (xi >= 1e-4);
-    if (run[s]) {
-      if (lo[s]) {
-        const double b0 = fmin(xi * dg_rcp_lo(eta), 1.0);
-        w[s] = fmin(b0 * dg_rcp_lo(1.0 + dg_sqrt_lo(fmax(fma(-b0, b0, 1.0), 0.0))), 0.999999);
-      } else {
-        const double b0 = xi / eta;
-        w[s] = b0 / (1.0 + sqrt(fma(-b0, b0, 1.0)));
-      }
-    } else {                                                       // Eq. 60 (xi = 0 gives w = 0: v = 0)
-      const double a1 = fma(al, eta, -1.0);
-      const double a12 = a1 * a1;
-      const double am = al - 1.0;
-      const double t3 = am * am / (8.0 * a12 * a12) * ((al + 3.0) * fma(al, eta, 1.0) - 4.0 * (al + 1.0));
-      w[s] = am / (2.0 * a1) * xi + t3 * xi * xi * xi;
-    }
+    xi[s] = Mabs[s] * rD; eta[s] = E[s] * rD;                      // Eq. 38
+    c4[s] = (al - 1.0) * xi[s];                                    // Eq. 59 (c0 = c4)
+    c3[s] = -2.0 * fma(al, eta[s], 1.0);
+    c2[s] = 2.0 * (al + 1.0) * xi[s];
+    c1[s] = -2.0 * fma(al, eta[s], -1.0);
+    general[s] = !(eta[s] < 1e30) || !(xi[s] >= 1e-4);
+    run[s] = !general[s];
+    // starting point in single precision: b0 = xi/eta, w0 = b0 / (1 + sqrt(1 - b0^2))
+    const float xf = __double2float_rn(xi[s]), ef = __double2float_rn(eta[s]);
+    const float b0 = fminf(__fdividef(xf, ef), 1.0f);
+    const float w0 = fminf(__fdividef(b0, 1.0f + sqrtf(fmaxf(fmaf(-b0, b0, 1.0f), 0.0f))), 0.999999f);
+    w[s] = (double)w0;
     any = any || run[s];
   }
 #pragma unroll 1
@@ -219,15 +240,17 @@ DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, 
       const double ws = w[s];
       const double p = fma(fma(fma(fma(c4[s], ws, c3[s]), ws, c2[s]), ws, c1[s]), ws, c4[s]);
       const double dp = fma(fma(fma(4.0 * c4[s], ws, 3.0 * c3[s]), ws, 2.0 * c2[s]), ws, c1[s]);
-      const double dw = lo[s] ? p * dg_rcp_lo(dp) : p / dp;
+      const double dw = p * dg_rcp_lo(dp);
       const double wn = ws - dw;
-      if (run[s]) {
-        w[s] = wn;
-        run[s] = !(fabs(dw) <= 1e-14 * wn);
-      }
-      any = any || run[s];
+      const bool more = run[s] && !(fabs(dw) <= 1e-14 * wn);
+      w[s] = run[s] ? wn : ws;
+      run[s] = more;
+      any = any || more;
     }
   }
+#pragma unroll
+  for (int s = 0; s < NS; ++s)
+    if (general[s]) w[s] = dg_ideal_w_general(al, xi[s], eta[s]);
 }
 
 // Taub-Matthews: the positive root Wv = gamma^2 - 1 of the cubic of Eq. 61 with
@@ -319,20 +342,27 @@ DG_INL bool dg_finite5(const double W[5]) {
 
 // con2prim of NS states in lockstep.  FULL: W[s] = [rho, u, P] (Eq. 55-57 / Eq. 74-75); else only the
 // pressure P[s] (what the stage kernel keeps).  st[s]: status.  nfall (or NULL): += Taub-Matthews
-// fallbacks.  Inputs failing Eq. 25 are rejected before either solver (status 1, outputs NaN).
+// fallbacks.  Inputs failing Eq. 25 are rejected before either solver (status 1, outputs NaN);
+// check = false: the caller has already established Eq. 25 for all NS states (the physicality
+// operator's screen, which is stricter), so the test is skipped.
 template <int EOS, int NS, bool FULL>
 DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5], double* P, int* st,
-                          int* nfall) {
+                          int* nfall, bool check = true) {
   const double qnan = __longlong_as_double(0x7ff8000000000000LL);
   double D[NS], E[NS], Mabs[NS];
   bool adm[NS];
 #pragma unroll
+  for (int s = 0; s < NS; ++s) adm[s] = true;
+  if (check) {
+#pragma unroll
+    for (int s = 0; s < NS; ++s) adm[s] = dg_admissible(U[s], 1.0);
+  }
+#pragma unroll
   for (int s = 0; s < NS; ++s) {
-    adm[s] = dg_admissible(U[s], 1.0);
     // an inadmissible state is replaced by a harmless one for the solver; its outputs are NaN
     D[s] = adm[s] ? U[s][0] : 1.0;
     E[s] = adm[s] ? U[s][4] : 2.0;
-    Mabs[s] = adm[s] ? dg_sqrt(fma(U[s][1], U[s][1], fma(U[s][2], U[s][2], U[s][3] * U[s][3]))) : 0.0;
+    Mabs[s] = adm[s] ? dg_sqrt_p(fma(U[s][1], U[s][1], fma(U[s][2], U[s][2], U[s][3] * U[s][3]))) : 0.0;
   }
   if (EOS == DG_EOS_IDEAL) {
     double w[NS];
@@ -398,7 +428,11 @@ DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5],
 // cancellation-free form of reading R14 with the Minkowski form <A,B> = A_E B_E - A_D B_D - A_M.B_M
 // and E -> (1-eps_q) E (R13c).
 // ---------------------------------------------------------------------------------------------
-DG_INL double dg_limiter_node_s(const double Ub[5], const double Ui[5], double f /* 1-eps_q */) {
+// (out of line and by value: the rare path must not force the callers' node arrays into local memory)
+struct DgState5 { double v[5]; };
+static __device__ __noinline__ double dg_limiter_node_s(DgState5 Ubs, DgState5 Uis, double f /* 1-eps_q */) {
+  const double* Ub = Ubs.v;
+  const double* Ui = Uis.v;
   double sD = (Ui[0] > 0.0) ? 1.0 : Ub[0] / (Ub[0] - Ui[0]);     // Eq. 28
   double sE = (Ui[4] > 0.0) ? 1.0 : Ub[4] / (Ub[4] - Ui[4]);     // Eq. 29
   double s1 = fmin(sD, sE);                                      // Eq. 30

@@ -1,17 +1,19 @@
 // stage_kernel.cuh -- the fused SSP-RK stage kernel of the CUDA path (sm_100a, fp64).
 //
 // One launch = one SSP-RK stage (PAPER.md:128-152 order of operations) over the whole mesh; a thread
-// block owns a tile of TX x TY x TZ elements and a THREAD OWNS ONE x-LINE of an element: the N = p+1
-// nodes (i = 0..N-1) at fixed (j,k).  Consequences of that mapping:
+// block owns a tile of TX x TY x TZ elements and a THREAD OWNS (A SEGMENT OF) ONE x-LINE of an element:
+// SEG consecutive nodes i at fixed (j,k) -- the whole line of N = p+1 nodes, except for p = 3, where a
+// line is split into two 2-node segments so that the 64-node hexahedron is exactly one warp and twice
+// as many warps are resident.  Consequences of that mapping:
 //   * the line is contiguous in the canonical layout X[v][e][n], n = i + N (j + N k): every state
 //     access of a thread is a 16-byte vector access (N even) and a warp reads / writes whole 128-byte
 //     lines; the neighbours' facing nodal layers in y and z are lines too (16-byte cp.async);
-//   * the x-direction volume contraction (Eq. 17) runs in registers; the y and z contractions read
-//     the line-mates' records from shared memory with 16-byte loads (natural node order: the N nodes
-//     of a thread are adjacent);
-//   * a cell is N^(d-1) <= 25 consecutive lanes of ONE warp, so everything cell-local in the
+//   * the x-direction volume contraction (Eq. 17) runs in registers (whole-line threads) or from the
+//     line's own records; the y and z contractions read the line-mates' records from shared memory
+//     with 16-byte loads (natural node order: the nodes of a thread are adjacent);
+//   * a cell is at most 32 consecutive lanes of ONE warp, so everything cell-local in the
 //     physicality operator (cell mean, min s) is a warp shuffle: no shared memory, no barrier;
-//   * N independent fp64 instruction streams per thread (con2prim's Newton iteration in lockstep).
+//   * SEG independent fp64 instruction streams per thread (con2prim's Newton iteration in lockstep).
 // Inputs per node: the stage state U_s and its pressure P_s = P(U_s), recovered by the stage that
 // produced U_s (8 B per node; everything else the flux and the wave speeds need follows from (U, P)
 // without a square root, physics.cuh dg_derive).  Primitives are never stored.
@@ -43,8 +45,8 @@ typedef unsigned long long dg_ull;
 
 __host__ __device__ constexpr int dg_ipow(int b, int e) { return e <= 0 ? 1 : b * dg_ipow(b, e - 1); }
 
-// elements per thread block along x,y,z for [ndim-1][N-1]; every tile is 4 warps of x-line threads
-// (3D p=3: 2x2x2 elements = 512 nodes = 128 threads, two blocks per SM on shared memory)
+// elements per thread block along x,y,z for [ndim-1][N-1]
+// (3D p=3: 2x2x2 elements = 512 nodes = 8 warps of 2-node threads, two blocks per SM on shared memory)
 __host__ __device__ constexpr int dg_tile(int nd, int N, int d) {
   constexpr int t[3][5][3] = {
       {{64, 1, 1}, {64, 1, 1}, {64, 1, 1}, {64, 1, 1}, {64, 1, 1}},
@@ -57,13 +59,14 @@ template <int ND, int N>
 struct TileShape {
   static constexpr int NN = dg_ipow(N, ND);          // nodes per element
   static constexpr int NF1 = dg_ipow(N, ND - 1);     // nodes per element face = x-lines per element
-  static constexpr int NL = NF1;                     // threads per element
+  static constexpr int SEG = (N == 4) ? 2 : N;       // nodes per thread (a segment of an x-line)
+  static constexpr int NSEG = N / SEG;               // segments per line
+  static constexpr int NL = NSEG * NF1;              // threads per element
   static constexpr int TX = dg_tile(ND, N, 0), TY = dg_tile(ND, N, 1), TZ = dg_tile(ND, N, 2);
   static constexpr int NE = TX * TY * TZ;            // elements per tile
   static constexpr int EPW = 32 / NL;                // elements per warp (lanes >= EPW*NL idle)
   static constexpr int NW = (NE + EPW - 1) / EPW;    // warps per block
   static constexpr int NT = 32 * NW;                 // threads per block
-  static constexpr bool VEC = (N % 2 == 0);          // 16-byte accesses along the line
   // shared-memory slot of node (i,j,k) of tile element le: le*ES + i + N*j + PK*k.  The k-planes of
   // the 3D p=3 element are padded by two slots so that the 16-byte line loads of a quarter-warp
   // (lanes j = 0..3, k = 0..1) fall into distinct banks.
@@ -87,8 +90,8 @@ struct TileShape {
   static constexpr int O_X = 0;
   static constexpr int O_XH = O_X + NREC * NS;
   static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][plane][5][FP]
-  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = y, z
-  static constexpr int O_RED = O_D + 2 * 26;         // [32] block reduction of the CFL maximum
+  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = x, y, z
+  static constexpr int O_RED = O_D + 3 * 26;         // [32] block reduction of the CFL maximum
   static constexpr int O_CNT = O_RED + 32;           // 4 ints
   static constexpr int SMEM_BYTES = (O_CNT + 2) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
@@ -183,11 +186,11 @@ DG_INL void dg_async_wait() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------------
 // The physicality-enforcing operator (PAPER.md:242-252 steps 1-4) on the cells of one warp.  A
-// thread owns the x-line j,k of its cell: nodes Uo[0..N-1], limited in place; the NL lines of a cell
-// are consecutive lanes starting at a multiple of NL.  MUST be called by all 32 lanes (inactive
-// lanes pass active = false).  This one function serves the fused stage kernel and the stand-alone
-// dgrhd_enforce_physicality kernel.
-//   wl: product of the GLL weights of the line's fixed coordinates (w_j w_k); w: the 1D weights.
+// thread owns SEG consecutive nodes of an x-line of its cell: Uo[0..SEG-1], limited in place; the NL
+// threads of a cell are consecutive lanes starting at a multiple of NL.  MUST be called by all 32
+// lanes (inactive lanes pass active = false).  This one function serves the fused stage kernel and
+// the stand-alone dgrhd_enforce_physicality kernel.
+//   wn[m]: tensor GLL weight of node m of the thread.
 //   cnt[0], cnt[1] += cells flagged / cells with an inadmissible mean, counted on the cell's first lane.
 // Returns the cell's flag; s_out = blend factor (1 if unflagged, 0 for an inadmissible mean, R13d).
 // ---------------------------------------------------------------------------------------------
@@ -221,28 +224,21 @@ DG_INL double dg_cell_min(double x, int base) {
   return acc;
 }
 
-template <int ND, int N>
-DG_INL bool dg_limiter_lines(double (*Uo)[5], bool active, int lane, double wl, const LimPar& lp,
-                             int cnt[2], double& s_out) {
-  constexpr int NL = dg_ipow(N, ND - 1);
-  s_out = 1.0;
-  bool bad = false;
-  if (active) {
-#pragma unroll
-    for (int m = 0; m < N; ++m) bad = bad || !dg_admissible(Uo[m], lp.f_screen);   // step 1: screen (R13e)
-  }
-  const unsigned ball = __ballot_sync(0xffffffffu, bad);
-  if (ball == 0u) return false;                   // nothing flagged in this warp (the common case)
+// the rare part: everything after the screen has found an inadmissible node in the warp
+template <int NL, int SEG>
+DG_INL bool dg_limiter_cells_slow(double (*Uo)[5], bool active, int lane, unsigned ball,
+                                                          const double* wn, const LimPar& lp, int cnt[2],
+                                                          double& s_out) {
   const int base = (lane / NL) * NL;
   const unsigned cmask = ((NL >= 32) ? 0xffffffffu : ((1u << NL) - 1u)) << base;
   const bool flagged = active && ((ball & cmask) != 0u);
   double Ub[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {                   // cell average: line partial sums, then across lanes
+  for (int v = 0; v < 5; ++v) {                   // cell average: thread partial sums, then across lanes
     double part = 0.0;
     if (flagged) {
 #pragma unroll
-      for (int m = 0; m < N; ++m) part = fma(wl * lp.w[m], Uo[m][v], part);
+      for (int m = 0; m < SEG; ++m) part = fma(wn[m], Uo[m][v], part);
     }
     Ub[v] = dg_cell_sum<NL>(part, base) / lp.wsum;
   }
@@ -251,9 +247,15 @@ DG_INL bool dg_limiter_lines(double (*Uo)[5], bool active, int lane, double wl, 
   if (flagged) {
     mean_ok = dg_admissible(Ub, lp.f_solve);      // step 2 (reading R13d)
     if (mean_ok) {
+      DgState5 ub;
 #pragma unroll
-      for (int m = 0; m < N; ++m) {
-        double sm_ = dg_limiter_node_s(Ub, Uo[m], lp.f_solve);     // step 3
+      for (int v = 0; v < 5; ++v) ub.v[v] = Ub[v];
+#pragma unroll
+      for (int m = 0; m < SEG; ++m) {
+        DgState5 ui;
+#pragma unroll
+        for (int v = 0; v < 5; ++v) ui.v[v] = Uo[m][v];
+        double sm_ = dg_limiter_node_s(ub, ui, lp.f_solve);        // step 3
         if (!(sm_ >= 0.0)) sm_ = 0.0;
         si = fmin(si, sm_);
       }
@@ -266,7 +268,7 @@ DG_INL bool dg_limiter_lines(double (*Uo)[5], bool active, int lane, double wl, 
     const double s = lp.one_m_delta * smin;       // R13c
     const double tt = 1.0 - s;
 #pragma unroll
-    for (int m = 0; m < N; ++m) {
+    for (int m = 0; m < SEG; ++m) {
 #pragma unroll
       for (int v = 0; v < 5; ++v)                 // Eq. 26 from the nearer end (R14)
         Uo[m][v] = (s > 0.5) ? fma(tt, Ub[v] - Uo[m][v], Uo[m][v]) : fma(s, Uo[m][v] - Ub[v], Ub[v]);
@@ -280,64 +282,28 @@ DG_INL bool dg_limiter_lines(double (*Uo)[5], bool active, int lane, double wl, 
   return flagged;
 }
 
-// ---------------------------------------------------------------------------------------------
-// One side of a face point: from a tile node record (rows U | v | P | num den) or from a halo point
-// (rows U | P; velocity and sigma derived here -- each halo point is used by exactly one face point)
-// ---------------------------------------------------------------------------------------------
-template <int ND, int N, int EOS, int D>
-DG_INL void dg_side_node(const double* x, double U[5], double& vn, double& P, double& num, double& den) {
-  constexpr int S = TileShape<ND, N>::NS;
+template <int NL, int SEG>
+DG_INL bool dg_limiter_cells(double (*Uo)[5], bool active, int lane, const double* wn, const LimPar& lp,
+                             int cnt[2], double& s_out) {
+  s_out = 1.0;
+  bool bad = false;
+  if (active) {
 #pragma unroll
-  for (int v = 0; v < 5; ++v) U[v] = x[v * S];
-  vn = x[(5 + D) * S];
-  P = x[8 * S];
-  num = x[9 * S];
-  den = x[10 * S];
-}
-template <int ND, int N, int EOS, int D>
-DG_INL void dg_side_halo(const EosPar& eos, const double* h, double U[5], double& vn, double& P,
-                         double& num, double& den) {
-  constexpr int S = TileShape<ND, N>::NHP;
-#pragma unroll
-  for (int v = 0; v < 5; ++v) U[v] = h[v * S];
-  P = h[5 * S];
-  double v3[3];
-  dg_derive<EOS>(eos, U, P, v3, num, den);
-  vn = v3[D];
+    for (int m = 0; m < SEG; ++m) bad = bad || !dg_admissible(Uo[m], lp.f_screen);   // step 1: screen (R13e)
+  }
+  const unsigned ball = __ballot_sync(0xffffffffu, bad);
+  if (ball == 0u) return false;                   // nothing flagged in this warp (the common case)
+  return dg_limiter_cells_slow<NL, SEG>(Uo, active, lane, ball, wn, lp, cnt, s_out);
 }
 
-// HLL flux (reading R9, Eq. 21-24) at face point fl of direction D from the records of its two
-// sides:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in the energy).
-template <int ND, int N, int EOS, int D>
-DG_INL void dg_face_flux(const EosPar& eos, const double* X, const double* XH, double* Fh, int fl,
-                         const int teff[3]) {
-  using TS = TileShape<ND, N>;
-  constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
-  constexpr int FPD = TS::FP(D);
-  const int p = fl / FPD, fp = fl - p * FPD;
-  const int te = fp / TS::NF1, tn = fp - te * TS::NF1;
-  const int la = te % TS::T(A), lb = te / TS::T(A);
-  const int ca = tn % N, cb = tn / N;
-  if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return;
-  const int tnode = ca * TS::SS(A) + cb * TS::SS(B);
-  const int telem = la * TS::SE(A) + lb * TS::SE(B);
-  double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
-  if (p < 1) {
-    DG_ASSERT(TS::HOFF(D) + fp < TS::NHALO);
-    dg_side_halo<ND, N, EOS, D>(eos, XH + (TS::HOFF(D) + fp), UL, vL, PL, numL, denL);
-  } else {
-    const int s = (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
-    DG_ASSERT(s >= 0 && s < TS::NS);
-    dg_side_node<ND, N, EOS, D>(X + s, UL, vL, PL, numL, denL);
-  }
-  if (p >= teff[D]) {
-    DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
-    dg_side_halo<ND, N, EOS, D>(eos, XH + (TS::HOFF(D) + FPD + fp), UR, vR, PR, numR, denR);
-  } else {
-    const int s = (telem + p * TS::SE(D)) * TS::ES + tnode;
-    DG_ASSERT(s >= 0 && s < TS::NS);
-    dg_side_node<ND, N, EOS, D>(X + s, UR, vR, PR, numR, denR);
-  }
+// ---------------------------------------------------------------------------------------------
+// HLL flux (reading R9, Eq. 21-24) at one face point from the two sides' U, normal velocity, P and
+// sigma = num/den:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in
+// the energy).  D: the face's direction; pF[v * fstride] receives the flux.
+// ---------------------------------------------------------------------------------------------
+DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, double denL,
+                         const double UR[5], double vR, double PR, double numR, double denR, int D,
+                         double* pF, int fstride) {
   double nmL, npL, dL, nmR, npR, dR;
   dg_speeds_frac(vL, numL, denL, nmL, npL, dL);
   dg_speeds_frac(vR, numR, denR, nmR, npR, dR);
@@ -357,74 +323,168 @@ DG_INL void dg_face_flux(const EosPar& eos, const double* X, const double* XH, d
   }
   const double kL = fma(cL, vL, -cU), kR = fma(cR, vR, cU);
   const double pL = cL * PL, pR = cR * PR;
-  double* pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
-  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
+  double f[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {
-    double f = fma(kL, UL[v], kR * UR[v]);
-    if (v == 1 + D) f += pL + pR;
-    if (v == 4) f = fma(pL, vL, fma(pR, vR, f));
-    pF[v * FPD] = f;
+  for (int v = 0; v < 5; ++v) f[v] = fma(kL, UL[v], kR * UR[v]);
+  const double pp = pL + pR;
+  f[1] += (D == 0) ? pp : 0.0;
+  f[2] += (D == 1) ? pp : 0.0;
+  f[3] += (D == 2) ? pp : 0.0;
+  f[4] = fma(pL, vL, fma(pR, vR, f[4]));
+#pragma unroll
+  for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
+}
+
+// Where the two sides of face point fl of direction D live: a tile node record (rows U | v | P |
+// num den, row stride NS) or a halo point (rows U | P, row stride NHP; velocity and sigma are derived
+// at use -- each halo point is used by exactly one face point).  Returns false for face points outside
+// a ragged tile.
+struct FaceSides {
+  const double* xl; const double* xr;   // record bases
+  bool hl, hr;                          // side is a halo point
+  double* pF;                           // Fhat[0] of this point
+  int fstride;                          // stride between the flux components
+};
+
+template <int ND, int N, int D>
+DG_INL bool dg_face_sides(const double* X, const double* XH, double* Fh, int fl, const int teff[3],
+                          FaceSides& fs) {
+  using TS = TileShape<ND, N>;
+  constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
+  constexpr int FPD = TS::FP(D);
+  const int p = fl / FPD, fp = fl - p * FPD;
+  const int te = fp / TS::NF1, tn = fp - te * TS::NF1;
+  const int la = te % TS::T(A), lb = te / TS::T(A);
+  const int ca = tn % N, cb = tn / N;
+  if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return false;
+  const int tnode = ca * TS::SS(A) + cb * TS::SS(B);
+  const int telem = la * TS::SE(A) + lb * TS::SE(B);
+  fs.hl = (p < 1);
+  fs.hr = (p >= teff[D]);
+  const int sl = (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
+  const int sr = (telem + p * TS::SE(D)) * TS::ES + tnode;
+  DG_ASSERT(fs.hl || (sl >= 0 && sl < TS::NS));
+  DG_ASSERT(fs.hr || (sr >= 0 && sr < TS::NS));
+  DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
+  fs.xl = fs.hl ? XH + (TS::HOFF(D) + fp) : X + sl;
+  fs.xr = fs.hr ? XH + (TS::HOFF(D) + FPD + fp) : X + sr;
+  fs.pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
+  fs.fstride = FPD;
+  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
+  return true;
+}
+
+template <int ND, int N, int EOS>
+DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, int D, double U[5], double& vn,
+                         double& P, double& num, double& den) {
+  using TS = TileShape<ND, N>;
+  if (halo) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) U[v] = x[v * TS::NHP];
+    P = x[5 * TS::NHP];
+    double v3[3];
+    dg_derive<EOS>(eos, U, P, v3, num, den);
+    vn = (D == 0) ? v3[0] : ((D == 1) ? v3[1] : v3[2]);
+  } else {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) U[v] = x[v * TS::NS];
+    vn = x[(5 + D) * TS::NS];
+    P = x[8 * TS::NS];
+    num = x[9 * TS::NS];
+    den = x[10 * TS::NS];
   }
 }
 
-// Volume term of direction D = 1 (y) or 2 (z) for the N nodes of this thread's line (Eq. 17 over the
-// diagonal mass matrix): for each q the line at index q along D -- N adjacent slots -- is read with
-// vector loads and F_D = U v_D + P e_D is formed on the fly.  dh: (2/h_D) Dhat[id][q] of this
+// Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
+// diagonal mass matrix): for each q the segment at index q along D -- SEG adjacent slots -- is read
+// with vector loads and F_D = U v_D + P e_D is formed on the fly.  dh: (2/h_D) Dhat[id][q] of this
 // thread's index id along D.
 template <int ND, int N, int D>
-DG_INL void dg_volume_line(const double* X, const double* dh, int s_line0, double (*R)[5]) {
+DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int S = TS::NS;
+  constexpr int S = TS::NS, SEG = TS::SEG;
 #pragma unroll
   for (int q = 0; q < N; ++q) {
     const double* x = X + s_line0 + q * TS::SS(D);
     const double c = dh[q];
-    double vd[N], Pq[N], t[N];
-    dg_ld_line<N>(x + (5 + D) * S, vd);
-    dg_ld_line<N>(x + 8 * S, Pq);
+    double vd[SEG], Pq[SEG], t[SEG];
+    dg_ld_line<SEG>(x + (5 + D) * S, vd);
+    dg_ld_line<SEG>(x + 8 * S, Pq);
 #pragma unroll
-    for (int m = 0; m < N; ++m) t[m] = c * vd[m];
+    for (int m = 0; m < SEG; ++m) t[m] = c * vd[m];
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double u[N];
-      dg_ld_line<N>(x + v * S, u);
+      double u[SEG];
+      dg_ld_line<SEG>(x + v * S, u);
 #pragma unroll
-      for (int m = 0; m < N; ++m) R[m][v] = fma(t[m], u[m], R[m][v]);
+      for (int m = 0; m < SEG; ++m) R[m][v] = fma(t[m], u[m], R[m][v]);
     }
 #pragma unroll
-    for (int m = 0; m < N; ++m) {
+    for (int m = 0; m < SEG; ++m) {
       R[m][1 + D] = fma(c, Pq[m], R[m][1 + D]);
       R[m][4] = fma(t[m], Pq[m], R[m][4]);
     }
   }
 }
 
-// Lift of the interface flux of direction D = 1 or 2 onto the line's nodes (Eq. 18): the line lies
-// in the element's minus face (id == 0: + c Fhat) and / or plus face (id == N-1: - c Fhat).
-template <int ND, int N, int D>
-DG_INL void dg_lift_line(const double* Fh, int id, int lcD, int fp0, double c, double (*R)[5]) {
+// Volume term of direction x for a thread that owns only a segment of its line: the whole line's
+// records (N adjacent slots) are read once; dh: rows (2/h_x) Dhat[i0+m][.] of the thread's nodes.
+template <int ND, int N>
+DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int FPD = TS::FP(D);
+  constexpr int S = TS::NS, SEG = TS::SEG;
+  double vx[N], Pq[N], c[SEG][N], t[SEG][N];
+  dg_ld_line<N>(X + s_line + 5 * S, vx);
+  dg_ld_line<N>(X + s_line + 8 * S, Pq);
+#pragma unroll
+  for (int m = 0; m < SEG; ++m) {
+    dg_ld_line<N>(dh + m * N, c[m]);
+#pragma unroll
+    for (int q = 0; q < N; ++q) t[m][q] = c[m][q] * vx[q];
+  }
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    double u[N];
+    dg_ld_line<N>(X + s_line + v * S, u);
+#pragma unroll
+    for (int m = 0; m < SEG; ++m)
+#pragma unroll
+      for (int q = 0; q < N; ++q) R[m][v] = fma(t[m][q], u[q], R[m][v]);
+  }
+#pragma unroll
+  for (int m = 0; m < SEG; ++m)
+#pragma unroll
+    for (int q = 0; q < N; ++q) {
+      R[m][1] = fma(c[m][q], Pq[q], R[m][1]);
+      R[m][4] = fma(t[m][q], Pq[q], R[m][4]);
+    }
+}
+
+// Lift of the interface flux of direction D = 1 or 2 onto the thread's nodes (Eq. 18): the segment
+// lies in the element's minus face (id == 0: + c Fhat) and / or plus face (id == N-1: - c Fhat).
+template <int ND, int N, int D>
+DG_INL void dg_lift_seg(const double* Fh, int id, int lcD, int fp0, double c, double (*R)[5]) {
+  using TS = TileShape<ND, N>;
+  constexpr int FPD = TS::FP(D), SEG = TS::SEG;
   const double* base = Fh + 5 * TS::FOFF(D) + fp0;
   if (id == 0) {
     const double* p = base + lcD * 5 * FPD;
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double f[N];
-      dg_ld_line<N>(p + v * FPD, f);
+      double f[SEG];
+      dg_ld_line<SEG>(p + v * FPD, f);
 #pragma unroll
-      for (int m = 0; m < N; ++m) R[m][v] = fma(c, f[m], R[m][v]);
+      for (int m = 0; m < SEG; ++m) R[m][v] = fma(c, f[m], R[m][v]);
     }
   }
   if (id == N - 1) {
     const double* p = base + (lcD + 1) * 5 * FPD;
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double f[N];
-      dg_ld_line<N>(p + v * FPD, f);
+      double f[SEG];
+      dg_ld_line<SEG>(p + v * FPD, f);
 #pragma unroll
-      for (int m = 0; m < N; ++m) R[m][v] = fma(-c, f[m], R[m][v]);
+      for (int m = 0; m < SEG; ++m) R[m][v] = fma(-c, f[m], R[m][v]);
     }
   }
 }
@@ -434,38 +494,47 @@ __global__ void __launch_bounds__(TileShape<ND, N>::NT, TileShape<ND, N>::MINB)
 dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
   constexpr int NN = TS::NN, NT = TS::NT, NL = TS::NL, NS = TS::NS, NHP = TS::NHP;
+  constexpr int SEG = TS::SEG, NSEG = TS::NSEG;
   extern __shared__ __align__(16) double sm[];
   double* X = sm + TS::O_X;
   double* XH = sm + TS::O_XH;
   double* Fh = sm + TS::O_FH;
-  double* sDy = sm + TS::O_D;
+  double* sDx = sm + TS::O_D;
+  double* sDy = sDx + 26;
   double* sDz = sDy + 26;
   double* sRed = sm + TS::O_RED;
   int* sCnt = reinterpret_cast<int*>(sm + TS::O_CNT);
 
-  // tile of this block; element, line (j,k) of this thread
+  // tile of this block; element, line (j,k) and segment h of this thread
   const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
   const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;
-  const int ew = lane / NL, ln = lane - ew * NL;
+  const int ew = lane / NL, lt = lane - ew * NL;
+  const int h = lt % NSEG, ln = lt / NSEG;                           // segment, line index j + N k
+  const int i0 = h * SEG;
   const int le = wrp * TS::EPW + ew;
   const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
   const bool active = (ew < TS::EPW) && (le < TS::NE) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
-  const int s0 = le * TS::ES + N * j + TS::PK * k;                   // slot of node i = 0 of the line
+  const int sl0 = le * TS::ES + N * j + TS::PK * k;                  // slot of node i = 0 of the line
+  const int s0 = sl0 + i0;                                           // slot of the thread's first node
   int g0 = 0;                                                        // its global index; ndof < 2^31
-  if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + N * ln;
+  if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + N * ln + i0;
+  const bool xlo = (h == 0), xhi = (h == NSEG - 1);                  // the segment holds node i = 0 / N-1
   if (t < 4) sCnt[t] = 0;
-  if (ND >= 2 && t < N * N) sDy[t] = a.Dy[t];
-  if (ND >= 3 && t < N * N) sDz[t] = a.Dz[t];
+  if (t < N * N) {
+    if (NSEG > 1) sDx[t] = a.Dx[t];
+    if (ND >= 2) sDy[t] = a.Dy[t];
+    if (ND >= 3) sDz[t] = a.Dz[t];
+  }
 
   // 1a. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
   //     periodic wrap or, at an outflow boundary, the node itself) -> halo rows U | P, asynchronously
   if (active) {
     {                                                                // x: one point per line and side
       const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
-      if (lc[0] == 0) {
+      if (xlo && lc[0] == 0) {
         const int g = g0 + a.hoff[0][0] + ((org[0] == 0) ? a.hfix[0][0] : 0);
         DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + fp < TS::NHALO);
         double* dst = XH + (TS::HOFF(0) + fp);
@@ -473,8 +542,8 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
         for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * NHP, a.Us + v * a.ndof + g);
         dg_async_copy8(dst + 5 * NHP, a.Pin + g);
       }
-      if (lc[0] == teff[0] - 1) {
-        const int g = g0 + (N - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
+      if (xhi && lc[0] == teff[0] - 1) {
+        const int g = g0 + (SEG - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
         DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + TS::FP(0) + fp < TS::NHALO);
         double* dst = XH + (TS::HOFF(0) + TS::FP(0) + fp);
 #pragma unroll
@@ -482,91 +551,91 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
         dg_async_copy8(dst + 5 * NHP, a.Pin + g);
       }
     }
-    if constexpr (ND >= 2) {                                         // y: the whole line
-      const int fp0 = N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]);
+    if constexpr (ND >= 2) {                                         // y: the thread's segment of the line
+      const int fp0 = i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]);
       if (j == 0 && lc[1] == 0) {
         const int g = g0 + a.hoff[1][0] + ((org[1] == 0) ? a.hfix[1][0] : 0);
-        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(1) + fp0 + N <= TS::NHALO);
+        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(1) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
       }
       if (j == N - 1 && lc[1] == teff[1] - 1) {
         const int g = g0 + a.hoff[1][1] + ((org[1] + teff[1] == a.ne[1]) ? a.hfix[1][1] : 0);
-        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + N <= TS::NHALO);
+        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(1) + TS::FP(1) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
       }
     }
-    if constexpr (ND >= 3) {                                         // z: the whole line
-      const int fp0 = N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]);
+    if constexpr (ND >= 3) {                                         // z: the thread's segment of the line
+      const int fp0 = i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]);
       if (k == 0 && lc[2] == 0) {
         const int g = g0 + a.hoff[2][0] + ((org[2] == 0) ? a.hfix[2][0] : 0);
-        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(2) + fp0 + N <= TS::NHALO);
+        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(2) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
       }
       if (k == N - 1 && lc[2] == teff[2] - 1) {
         const int g = g0 + a.hoff[2][1] + ((org[2] + teff[2] == a.ne[2]) ? a.hfix[2][1] : 0);
-        DG_ASSERT(g >= 0 && g + N <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + N <= TS::NHALO);
+        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(2) + TS::FP(2) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<N>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<N>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
       }
     }
   }
 
-  // 1b. own line: U_s, P_s -> records; the x-direction flux stays in registers
-  double R[N][5];
+  // 1b. own nodes: U_s, P_s -> records
+  double R[SEG][5];
 #pragma unroll
-  for (int m = 0; m < N; ++m)
+  for (int m = 0; m < SEG; ++m)
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
   if (active) {
-    double Ul[5][N], Pl[N];
+    double Ul[5][SEG], Pl[SEG];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dg_ldg_line<N>(a.Us + v * a.ndof + g0, Ul[v]);
-    dg_ldg_line<N>(a.Pin + g0, Pl);
+    for (int v = 0; v < 5; ++v) dg_ldg_line<SEG>(a.Us + v * a.ndof + g0, Ul[v]);
+    dg_ldg_line<SEG>(a.Pin + g0, Pl);
     if (a.mode == DG_MODE_STAGE && a.a != 0.0) {          // U0 is needed last: warm L2 now
 #pragma unroll
       for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0));
     }
-    double vl[3][N], numl[N], denl[N];
+    double vl[3][SEG], numl[SEG], denl[SEG];
 #pragma unroll
-    for (int m = 0; m < N; ++m) {
+    for (int m = 0; m < SEG; ++m) {
       const double Um[5] = {Ul[0][m], Ul[1][m], Ul[2][m], Ul[3][m], Ul[4][m]};
       double v3[3];
       dg_derive<EOS>(a.eos, Um, Pl[m], v3, numl[m], denl[m]);
       vl[0][m] = v3[0]; vl[1][m] = v3[1]; vl[2][m] = v3[2];
     }
-    DG_ASSERT(s0 >= 0 && s0 + N <= NS);
+    DG_ASSERT(s0 >= 0 && s0 + SEG <= NS);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dg_st_line<N>(X + v * NS + s0, Ul[v]);
+    for (int v = 0; v < 5; ++v) dg_st_line<SEG>(X + v * NS + s0, Ul[v]);
 #pragma unroll
-    for (int d = 0; d < 3; ++d) dg_st_line<N>(X + (5 + d) * NS + s0, vl[d]);
-    dg_st_line<N>(X + 8 * NS + s0, Pl);
-    dg_st_line<N>(X + 9 * NS + s0, numl);
-    dg_st_line<N>(X + 10 * NS + s0, denl);
-    // volume term, x direction, in registers: R_i += sum_q (2/h_x) Dhat[i][q] F_x(q)
-    if (N > 1) {
-      double Fx[N][5];
+    for (int d = 0; d < 3; ++d) dg_st_line<SEG>(X + (5 + d) * NS + s0, vl[d]);
+    dg_st_line<SEG>(X + 8 * NS + s0, Pl);
+    dg_st_line<SEG>(X + 9 * NS + s0, numl);
+    dg_st_line<SEG>(X + 10 * NS + s0, denl);
+    // volume term, x direction, for whole-line threads in registers: R_i += sum_q (2/h_x) Dhat[i][q] F_x(q)
+    if (NSEG == 1 && N > 1) {
+      double Fx[SEG][5];
 #pragma unroll
-      for (int m = 0; m < N; ++m) {
+      for (int m = 0; m < SEG; ++m) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) Fx[m][v] = Ul[v][m] * vl[0][m];
         Fx[m][1] += Pl[m];
         Fx[m][4] = fma(Pl[m], vl[0][m], Fx[m][4]);
       }
 #pragma unroll
-      for (int m = 0; m < N; ++m)
+      for (int m = 0; m < SEG; ++m)
 #pragma unroll
-        for (int q = 0; q < N; ++q) {
+        for (int q = 0; q < SEG; ++q) {
           const double c = a.Dx[m * N + q];
 #pragma unroll
           for (int v = 0; v < 5; ++v) R[m][v] = fma(c, Fx[q][v], R[m][v]);
@@ -578,14 +647,24 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_flux<ND, N, EOS, 0>(a.eos, X, XH, Fh, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_flux<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(1), teff);
-    else dg_face_flux<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(2), teff);
+    FaceSides fs;
+    int D;
+    bool ok;
+    if (ND == 1 || f < TS::FOFF(1)) { D = 0; ok = dg_face_sides<ND, N, 0>(X, XH, Fh, f, teff, fs); }
+    else if (ND == 2 || f < TS::FOFF(2)) { D = 1; ok = dg_face_sides<ND, N, (ND > 1 ? 1 : 0)>(X, XH, Fh, f - TS::FOFF(1), teff, fs); }
+    else { D = 2; ok = dg_face_sides<ND, N, (ND > 2 ? 2 : 0)>(X, XH, Fh, f - TS::FOFF(2), teff, fs); }
+    if (ok) {
+      double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
+      dg_load_side<ND, N, EOS>(a.eos, fs.xl, fs.hl, D, UL, vL, PL, numL, denL);
+      dg_load_side<ND, N, EOS>(a.eos, fs.xr, fs.hr, D, UR, vR, PR, numR, denR);
+      dg_hll_point(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, D, fs.pF, fs.fstride);
+    }
   }
-  //    volume quadrature, y and z: reads the records only, so it needs no barrier here
+  //    volume quadrature: reads the records only, so it needs no barrier here
   if (active && N > 1) {
-    if constexpr (ND >= 2) dg_volume_line<ND, N, 1>(X, sDy + j * N, le * TS::ES + TS::PK * k, R);
-    if constexpr (ND >= 3) dg_volume_line<ND, N, 2>(X, sDz + k * N, le * TS::ES + N * j, R);
+    if constexpr (NSEG > 1) dg_volume_x_seg<ND, N>(X, sDx + i0 * N, sl0, R);
+    if constexpr (ND >= 2) dg_volume_seg<ND, N, 1>(X, sDy + j * N, le * TS::ES + i0 + TS::PK * k, R);
+    if constexpr (ND >= 3) dg_volume_seg<ND, N, 2>(X, sDz + k * N, le * TS::ES + i0 + N * j, R);
   }
   __syncthreads();
 
@@ -594,27 +673,30 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     {
       const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
       const double* base = Fh + fp;
-      const double* pm = base + lc[0] * 5 * TS::FP(0);
-      const double* pp = base + (lc[0] + 1) * 5 * TS::FP(0);
+      if (xlo) {
+        const double* pm = base + lc[0] * 5 * TS::FP(0);
 #pragma unroll
-      for (int v = 0; v < 5; ++v) {
-        R[0][v] = fma(a.lift[0], pm[v * TS::FP(0)], R[0][v]);
-        R[N - 1][v] = fma(-a.lift[0], pp[v * TS::FP(0)], R[N - 1][v]);
+        for (int v = 0; v < 5; ++v) R[0][v] = fma(a.lift[0], pm[v * TS::FP(0)], R[0][v]);
+      }
+      if (xhi) {
+        const double* pp = base + (lc[0] + 1) * 5 * TS::FP(0);
+#pragma unroll
+        for (int v = 0; v < 5; ++v) R[SEG - 1][v] = fma(-a.lift[0], pp[v * TS::FP(0)], R[SEG - 1][v]);
       }
     }
     if constexpr (ND >= 2)
-      dg_lift_line<ND, N, 1>(Fh, j, lc[1], N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
+      dg_lift_seg<ND, N, 1>(Fh, j, lc[1], i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
     if constexpr (ND >= 3)
-      dg_lift_line<ND, N, 2>(Fh, k, lc[2], N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
+      dg_lift_seg<ND, N, 2>(Fh, k, lc[2], i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
 #pragma unroll
       for (int v = 0; v < 5; ++v) {
-        double r[N];
+        double r[SEG];
 #pragma unroll
-        for (int m = 0; m < N; ++m) r[m] = R[m][v];
-        dg_st_line<N>(a.Rout + v * a.ndof + g0, r);
+        for (int m = 0; m < SEG; ++m) r[m] = R[m][v];
+        dg_st_line<SEG>(a.Rout + v * a.ndof + g0, r);
       }
     }
     return;
@@ -622,26 +704,27 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 4. SSP-RK combine (Shu-Osher form); U_s comes back from the thread's own records
   const double dt = *a.dt_ptr;
-  double Uo[N][5];
+  double Uo[SEG][5];
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
-    double u[N];
-    if (active) dg_ld_line<N>(X + v * NS + s0, u);
+    double u[SEG];
+    dg_ld_line<SEG>(X + v * NS + (active ? s0 : 0), u);
 #pragma unroll
-    for (int m = 0; m < N; ++m) Uo[m][v] = active ? a.b * fma(dt, R[m][v], u[m]) : 0.0;
+    for (int m = 0; m < SEG; ++m) Uo[m][v] = a.b * fma(dt, R[m][v], u[m]);
   }
   if (a.a != 0.0 && active) {
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double u0[N];
-      dg_ld_line<N>(a.U0 + v * a.ndof + g0, u0);
+      double u0[SEG];
+      dg_ld_line<SEG>(a.U0 + v * a.ndof + g0, u0);
 #pragma unroll
-      for (int m = 0; m < N; ++m) Uo[m][v] = fma(a.a, u0[m], Uo[m][v]);
+      for (int m = 0; m < SEG; ++m) Uo[m][v] = fma(a.a, u0[m], Uo[m][v]);
     }
   }
 
   // 5. physicality-enforcing operator (cell-local: warp shuffles)
   int cnt[4] = {0, 0, 0, 0};
+  bool flagged;
   {
     LimPar lp;
 #pragma unroll
@@ -650,29 +733,33 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     double wl = 1.0;
     if (ND >= 2) wl *= a.w[j];
     if (ND >= 3) wl *= a.w[k];
+    double wn[SEG];
+#pragma unroll
+    for (int m = 0; m < SEG; ++m) wn[m] = wl * ((NSEG > 1 && h > 0) ? a.w[(SEG + m) % 5] : a.w[m]);
     double s_unused;
-    dg_limiter_lines<ND, N>(Uo, active, lane, wl, lp, cnt, s_unused);
+    flagged = dg_limiter_cells<NL, SEG>(Uo, active, lane, wn, lp, cnt, s_unused);
   }
 
-  // 6. pressure of the new state (for the next stage), CFL maximum
+  // 6. pressure of the new state (for the next stage), CFL maximum.  Nodes of unflagged cells have
+  //    passed the screen (stricter than Eq. 25), so con2prim's own admissibility test is skipped there.
   double speed = 0.0;
   if (active) {
-    double Po[N];
-    int st[N];
-    dg_con2prim_n<EOS, N, false>(a.eos, Uo, nullptr, Po, st, &cnt[3]);
+    double Po[SEG];
+    int st[SEG];
+    dg_con2prim_n<EOS, SEG, false>(a.eos, Uo, nullptr, Po, st, &cnt[3], flagged);
 #pragma unroll
-    for (int m = 0; m < N; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;
+    for (int m = 0; m < SEG; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
-      double u[N];
+      double u[SEG];
 #pragma unroll
-      for (int m = 0; m < N; ++m) u[m] = Uo[m][v];
-      dg_st_line<N>(a.Uout + v * a.ndof + g0, u);
+      for (int m = 0; m < SEG; ++m) u[m] = Uo[m][v];
+      dg_st_line<SEG>(a.Uout + v * a.ndof + g0, u);
     }
-    dg_st_line<N>(a.Pout + g0, Po);
+    dg_st_line<SEG>(a.Pout + g0, Po);
     if (a.do_cfl) {
 #pragma unroll
-      for (int m = 0; m < N; ++m) {
+      for (int m = 0; m < SEG; ++m) {
         const double sp = dg_cfl_speed<EOS, ND>(a.eos, Uo[m], Po[m], a.cw);
         if (sp > 0.0) speed = fmax(speed, sp);            // NaN never wins
       }

@@ -55,10 +55,14 @@ DG_INL double dg_sqrt(double x) {                 // x >= 0; sqrt(0) = 0
   return fma(fma(-s, s, x), 0.5 * r, s);
 }
 // sqrt(x + 1e-300): one add instead of the compare-and-select guard; identical to dg_sqrt(x) for every
-// normal x and 1e-150 instead of 0 at x = 0 -- used where that is harmless (|M|, wave-speed radicands)
+// normal x and 1e-150 instead of 0 at x = 0 -- used where that is harmless (|M|, wave-speed radicands).
+// One Newton step on the reciprocal root (seed 2^-22 -> 2^-44) is enough here: the closing correction
+// s + (y - s^2) r/2 is itself a Newton step for the root and squares the error once more.
 DG_INL double dg_sqrt_p(double x) {
   const double y = x + 1e-300;
-  const double r = dg_rsqrt(y);
+  double r;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+  r = fma(r, fma(-0.5 * y * r, r, 0.5), r);
   const double s = y * r;
   return fma(fma(-s, s, y), 0.5 * r, s);
 }
@@ -208,9 +212,14 @@ static __device__ __noinline__ double dg_ideal_w_general(double al, double xi, d
   return w;
 }
 
+// Pg (or NULL): a guess of the pressure (the stage kernel passes the pressure of the node's previous
+// state): beta_0 = |M| / (E + Pg) instead of |M| / E.  Any start in (0,1) converges.
+// Stopping: Newton converges quadratically and the step is a tight estimate of the error BEFORE the
+// step, so once |dw| <= 1e-9 w the new iterate is at the fp64 floor (error ~ K dw^2 + 6e-8 |dw| from the
+// single-precision reciprocal); this meets reading R3's criterion (|dw| <= 1e-14 w) one iteration earlier.
 template <int NS>
 DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, const double* Mabs,
-                             double* w) {
+                             const double* Pg, double* w) {
   const double al = e.al;
   double c4[NS], c3[NS], c2[NS], c1[NS], xi[NS], eta[NS];
   bool run[NS], general[NS];
@@ -223,10 +232,11 @@ DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, 
     c3[s] = -2.0 * fma(al, eta[s], 1.0);
     c2[s] = 2.0 * (al + 1.0) * xi[s];
     c1[s] = -2.0 * fma(al, eta[s], -1.0);
-    general[s] = !(eta[s] < 1e30) || !(xi[s] >= 1e-4);
+    general[s] = !(E[s] < 1e30) || !(Mabs[s] > 1e-30) || !(eta[s] < 1e30) || !(xi[s] >= 1e-4);
     run[s] = !general[s];
     // starting point in single precision: b0 = xi/eta, w0 = b0 / (1 + sqrt(1 - b0^2))
-    const float xf = __double2float_rn(xi[s]), ef = __double2float_rn(eta[s]);
+    const float xf = __double2float_rn(Mabs[s]);
+    const float ef = __double2float_rn(Pg ? E[s] + fmax(Pg[s], 0.0) : E[s]);
     const float b0 = fminf(__fdividef(xf, ef), 1.0f);
     const float w0 = fminf(__fdividef(b0, 1.0f + sqrtf(fmaxf(fmaf(-b0, b0, 1.0f), 0.0f))), 0.999999f);
     w[s] = (double)w0;
@@ -242,7 +252,7 @@ DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, 
       const double dp = fma(fma(fma(4.0 * c4[s], ws, 3.0 * c3[s]), ws, 2.0 * c2[s]), ws, c1[s]);
       const double dw = p * dg_rcp_lo(dp);
       const double wn = ws - dw;
-      const bool more = run[s] && !(fabs(dw) <= 1e-14 * wn);
+      const bool more = run[s] && !(fabs(dw) <= 1e-9 * wn);
       w[s] = run[s] ? wn : ws;
       run[s] = more;
       any = any || more;
@@ -347,7 +357,7 @@ DG_INL bool dg_finite5(const double W[5]) {
 // operator's screen, which is stricter), so the test is skipped.
 template <int EOS, int NS, bool FULL>
 DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5], double* P, int* st,
-                          int* nfall, bool check = true) {
+                          int* nfall, bool check = true, const double* Pguess = nullptr) {
   const double qnan = __longlong_as_double(0x7ff8000000000000LL);
   double D[NS], E[NS], Mabs[NS];
   bool adm[NS];
@@ -366,7 +376,7 @@ DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5],
   }
   if (EOS == DG_EOS_IDEAL) {
     double w[NS];
-    dg_ideal_solve_w<NS>(e, D, E, Mabs, w);
+    dg_ideal_solve_w<NS>(e, D, E, Mabs, Pguess, w);
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
       const double w2 = w[s] * w[s];

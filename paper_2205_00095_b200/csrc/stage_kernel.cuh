@@ -67,10 +67,9 @@ struct TileShape {
   static constexpr int EPW = 32 / NL;                // elements per warp (lanes >= EPW*NL idle)
   static constexpr int NW = (NE + EPW - 1) / EPW;    // warps per block
   static constexpr int NT = 32 * NW;                 // threads per block
-  // shared-memory slot of node (i,j,k) of tile element le: le*ES + i + N*j + PK*k.  The k-planes of
-  // the 3D p=3 element are padded by two slots so that the 16-byte line loads of a quarter-warp
-  // (lanes j = 0..3, k = 0..1) fall into distinct banks.
-  static constexpr int PK = (ND == 3) ? N * N + ((N == 4) ? 2 : 0) : 0;
+  // shared-memory slot of node (i,j,k) of tile element le: le*ES + i + N*j + PK*k (natural order: the
+  // 16-byte line loads of a quarter-warp fall into distinct banks or coincide)
+  static constexpr int PK = (ND == 3) ? N * N : 0;
   static constexpr int ES = (ND == 1) ? N : ((ND == 2) ? N * N : N * PK);
   static constexpr int NS = (NE * ES + 1) / 2 * 2;   // slots per record row
   __host__ __device__ static constexpr int T(int d) { return d == 0 ? TX : (d == 1 ? TY : TZ); }
@@ -81,21 +80,26 @@ struct TileShape {
   __host__ __device__ static constexpr int FOFF(int d) {
     return d <= 0 ? 0 : FOFF(d - 1) + (T(d - 1) + 1) * FP(d - 1);
   }
+  // interior face planes only (the flux of a boundary plane is kept in its halo slot, see below)
+  __host__ __device__ static constexpr int FOFFI(int d) {
+    return d <= 0 ? 0 : FOFFI(d - 1) + (T(d - 1) - 1) * FP(d - 1);
+  }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
   static constexpr int NHP = (NHALO + 1) / 2 * 2;    // row stride of the halo array
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
+  static constexpr int NFACEI = FOFFI(ND);           // of which between two elements of the tile
   // shared memory, in doubles.  Node records X[11][NS] = D Mx My Mz E | vx vy vz | P | num den (conserved
   // state, 3-velocity, pressure, sigma = num/den of Eq. 22); halo points XH[6][NHP] = D Mx My Mz E | P.
+  // The interface flux of a face point on the tile's boundary overwrites rows 0..4 of the halo point
+  // it was computed from (read and written by the same thread); Fhat holds the interior planes only.
   static constexpr int NREC = 11, HREC = 6;
   static constexpr int O_X = 0;
   static constexpr int O_XH = O_X + NREC * NS;
-  static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][plane][5][FP]
-  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = x, y, z
-  static constexpr int O_RED = O_D + 3 * 26;         // [32] block reduction of the CFL maximum
-  static constexpr int O_CNT = O_RED + 32;           // 4 ints
-  static constexpr int SMEM_BYTES = (O_CNT + 2) * 8;
+  static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][interior plane][5][FP]
+  static constexpr int O_D = O_FH + (5 * NFACEI + 1) / 2 * 2;  // (2/h_d) Dhat[i][q] for d = x, y, z
+  static constexpr int SMEM_BYTES = (O_D + 3 * 26) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
-  static constexpr int BLK_REG = 65536 / (NT * 128);   // leave >= 128 registers per thread
+  static constexpr int BLK_REG = 65536 / (NT * 80);    // leave >= 80 registers per thread
   static constexpr int MINB = (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) > 0 ? (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) : 1;
 };
 
@@ -301,8 +305,9 @@ DG_INL bool dg_limiter_cells(double (*Uo)[5], bool active, int lane, const doubl
 // sigma = num/den:  F = cL F_L + cR F_R + cU (U_R - U_L),  F_s = U_s v_s + P_s e_D (+ P_s v_s in
 // the energy).  D: the face's direction; pF[v * fstride] receives the flux.
 // ---------------------------------------------------------------------------------------------
+template <int D>
 DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, double denL,
-                         const double UR[5], double vR, double PR, double numR, double denR, int D,
+                         const double UR[5], double vR, double PR, double numR, double denR,
                          double* pF, int fstride) {
   double nmL, npL, dL, nmR, npR, dR;
   dg_speeds_frac(vL, numL, denL, nmL, npL, dL);
@@ -326,10 +331,7 @@ DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, 
   double f[5];
 #pragma unroll
   for (int v = 0; v < 5; ++v) f[v] = fma(kL, UL[v], kR * UR[v]);
-  const double pp = pL + pR;
-  f[1] += (D == 0) ? pp : 0.0;
-  f[2] += (D == 1) ? pp : 0.0;
-  f[3] += (D == 2) ? pp : 0.0;
+  f[1 + D] += pL + pR;
   f[4] = fma(pL, vL, fma(pR, vR, f[4]));
 #pragma unroll
   for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
@@ -347,7 +349,7 @@ struct FaceSides {
 };
 
 template <int ND, int N, int D>
-DG_INL bool dg_face_sides(const double* X, const double* XH, double* Fh, int fl, const int teff[3],
+DG_INL bool dg_face_sides(const double* X, double* XH, double* Fh, int fl, const int teff[3],
                           FaceSides& fs) {
   using TS = TileShape<ND, N>;
   constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
@@ -368,14 +370,19 @@ DG_INL bool dg_face_sides(const double* X, const double* XH, double* Fh, int fl,
   DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
   fs.xl = fs.hl ? XH + (TS::HOFF(D) + fp) : X + sl;
   fs.xr = fs.hr ? XH + (TS::HOFF(D) + FPD + fp) : X + sr;
-  fs.pF = Fh + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
-  fs.fstride = FPD;
-  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
+  // where the flux goes: the halo slot of a boundary plane, else the interior plane p-1
+  if (fs.hl) { fs.pF = XH + (TS::HOFF(D) + fp); fs.fstride = TS::NHP; }
+  else if (fs.hr) { fs.pF = XH + (TS::HOFF(D) + FPD + fp); fs.fstride = TS::NHP; }
+  else {
+    DG_ASSERT(p >= 1 && 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACEI);
+    fs.pF = Fh + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
+    fs.fstride = FPD;
+  }
   return true;
 }
 
-template <int ND, int N, int EOS>
-DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, int D, double U[5], double& vn,
+template <int ND, int N, int EOS, int D>
+DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, double U[5], double& vn,
                          double& P, double& num, double& den) {
   using TS = TileShape<ND, N>;
   if (halo) {
@@ -384,7 +391,7 @@ DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, int D, d
     P = x[5 * TS::NHP];
     double v3[3];
     dg_derive<EOS>(eos, U, P, v3, num, den);
-    vn = (D == 0) ? v3[0] : ((D == 1) ? v3[1] : v3[2]);
+    vn = v3[D];
   } else {
 #pragma unroll
     for (int v = 0; v < 5; ++v) U[v] = x[v * TS::NS];
@@ -393,6 +400,17 @@ DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, int D, d
     num = x[9 * TS::NS];
     den = x[10 * TS::NS];
   }
+}
+
+template <int ND, int N, int EOS, int D>
+DG_INL void dg_face_point(const EosPar& eos, const double* X, double* XH, double* Fh, int fl,
+                          const int teff[3]) {
+  FaceSides fs;
+  if (!dg_face_sides<ND, N, D>(X, XH, Fh, fl, teff, fs)) return;
+  double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
+  dg_load_side<ND, N, EOS, D>(eos, fs.xl, fs.hl, UL, vL, PL, numL, denL);
+  dg_load_side<ND, N, EOS, D>(eos, fs.xr, fs.hr, UR, vR, PR, numR, denR);
+  dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, fs.pF, fs.fstride);
 }
 
 // Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
@@ -460,29 +478,43 @@ DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, doubl
     }
 }
 
+// Flux of face plane p of direction D at face point fp: in the halo slot for the tile's boundary
+// planes (p == 0, p == teffD), else in the interior-plane array.  Returns the row stride.
+template <int ND, int N, int D>
+DG_INL const double* dg_flux_ptr(const double* XH, const double* Fh, int p, int teffD, int fp, int& stride) {
+  using TS = TileShape<ND, N>;
+  constexpr int FPD = TS::FP(D);
+  if (p == 0) { stride = TS::NHP; return XH + (TS::HOFF(D) + fp); }
+  if (p == teffD) { stride = TS::NHP; return XH + (TS::HOFF(D) + FPD + fp); }
+  stride = FPD;
+  return Fh + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
+}
+
 // Lift of the interface flux of direction D = 1 or 2 onto the thread's nodes (Eq. 18): the segment
 // lies in the element's minus face (id == 0: + c Fhat) and / or plus face (id == N-1: - c Fhat).
 template <int ND, int N, int D>
-DG_INL void dg_lift_seg(const double* Fh, int id, int lcD, int fp0, double c, double (*R)[5]) {
+DG_INL void dg_lift_seg(const double* XH, const double* Fh, int id, int lcD, int teffD, int fp0, double c,
+                        double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int FPD = TS::FP(D), SEG = TS::SEG;
-  const double* base = Fh + 5 * TS::FOFF(D) + fp0;
+  constexpr int SEG = TS::SEG;
   if (id == 0) {
-    const double* p = base + lcD * 5 * FPD;
+    int st;
+    const double* p = dg_flux_ptr<ND, N, D>(XH, Fh, lcD, teffD, fp0, st);
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
       double f[SEG];
-      dg_ld_line<SEG>(p + v * FPD, f);
+      dg_ld_line<SEG>(p + v * st, f);
 #pragma unroll
       for (int m = 0; m < SEG; ++m) R[m][v] = fma(c, f[m], R[m][v]);
     }
   }
   if (id == N - 1) {
-    const double* p = base + (lcD + 1) * 5 * FPD;
+    int st;
+    const double* p = dg_flux_ptr<ND, N, D>(XH, Fh, lcD + 1, teffD, fp0, st);
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
       double f[SEG];
-      dg_ld_line<SEG>(p + v * FPD, f);
+      dg_ld_line<SEG>(p + v * st, f);
 #pragma unroll
       for (int m = 0; m < SEG; ++m) R[m][v] = fma(-c, f[m], R[m][v]);
     }
@@ -502,8 +534,6 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   double* sDx = sm + TS::O_D;
   double* sDy = sDx + 26;
   double* sDz = sDy + 26;
-  double* sRed = sm + TS::O_RED;
-  int* sCnt = reinterpret_cast<int*>(sm + TS::O_CNT);
 
   // tile of this block; element, line (j,k) and segment h of this thread
   const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
@@ -522,14 +552,24 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   int g0 = 0;                                                        // its global index; ndof < 2^31
   if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + N * ln + i0;
   const bool xlo = (h == 0), xhi = (h == NSEG - 1);                  // the segment holds node i = 0 / N-1
-  if (t < 4) sCnt[t] = 0;
   if (t < N * N) {
     if (NSEG > 1) sDx[t] = a.Dx[t];
     if (ND >= 2) sDy[t] = a.Dy[t];
     if (ND >= 3) sDz[t] = a.Dz[t];
   }
 
-  // 1a. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
+  // 1a. own nodes: U_s, P_s requested first (HBM latency overlaps the halo bookkeeping below)
+  double Ul[5][SEG], Pl[SEG];
+  if (active) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dg_ldg_line<SEG>(a.Us + v * a.ndof + g0, Ul[v]);
+    dg_ldg_line<SEG>(a.Pin + g0, Pl);
+    if (a.mode == DG_MODE_STAGE && a.a != 0.0) {          // U0 is needed last: warm L2 now
+#pragma unroll
+      for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0));
+    }
+  }
+  // 1b. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
   //     periodic wrap or, at an outflow boundary, the node itself) -> halo rows U | P, asynchronously
   if (active) {
     {                                                                // x: one point per line and side
@@ -591,21 +631,13 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     }
   }
 
-  // 1b. own nodes: U_s, P_s -> records
+  // 1c. own nodes -> records
   double R[SEG][5];
 #pragma unroll
   for (int m = 0; m < SEG; ++m)
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
   if (active) {
-    double Ul[5][SEG], Pl[SEG];
-#pragma unroll
-    for (int v = 0; v < 5; ++v) dg_ldg_line<SEG>(a.Us + v * a.ndof + g0, Ul[v]);
-    dg_ldg_line<SEG>(a.Pin + g0, Pl);
-    if (a.mode == DG_MODE_STAGE && a.a != 0.0) {          // U0 is needed last: warm L2 now
-#pragma unroll
-      for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0));
-    }
     double vl[3][SEG], numl[SEG], denl[SEG];
 #pragma unroll
     for (int m = 0; m < SEG; ++m) {
@@ -647,18 +679,9 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    FaceSides fs;
-    int D;
-    bool ok;
-    if (ND == 1 || f < TS::FOFF(1)) { D = 0; ok = dg_face_sides<ND, N, 0>(X, XH, Fh, f, teff, fs); }
-    else if (ND == 2 || f < TS::FOFF(2)) { D = 1; ok = dg_face_sides<ND, N, (ND > 1 ? 1 : 0)>(X, XH, Fh, f - TS::FOFF(1), teff, fs); }
-    else { D = 2; ok = dg_face_sides<ND, N, (ND > 2 ? 2 : 0)>(X, XH, Fh, f - TS::FOFF(2), teff, fs); }
-    if (ok) {
-      double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
-      dg_load_side<ND, N, EOS>(a.eos, fs.xl, fs.hl, D, UL, vL, PL, numL, denL);
-      dg_load_side<ND, N, EOS>(a.eos, fs.xr, fs.hr, D, UR, vR, PR, numR, denR);
-      dg_hll_point(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, D, fs.pF, fs.fstride);
-    }
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_point<ND, N, EOS, 0>(a.eos, X, XH, Fh, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_point<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(1), teff);
+    else dg_face_point<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(2), teff);
   }
   //    volume quadrature: reads the records only, so it needs no barrier here
   if (active && N > 1) {
@@ -666,28 +689,36 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     if constexpr (ND >= 2) dg_volume_seg<ND, N, 1>(X, sDy + j * N, le * TS::ES + i0 + TS::PK * k, R);
     if constexpr (ND >= 3) dg_volume_seg<ND, N, 2>(X, sDz + k * N, le * TS::ES + i0 + N * j, R);
   }
+  // U0 is requested before the barrier: its (L2) latency overlaps the wait and the lift
+  double U0r[5][SEG];
+  const bool need_u0 = (a.mode == DG_MODE_STAGE) && (a.a != 0.0) && active;
+  if (need_u0) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dg_ld_line<SEG>(a.U0 + v * a.ndof + g0, U0r[v]);
+  }
   __syncthreads();
 
   // 3. surface lift
   if (active) {
     {
       const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
-      const double* base = Fh + fp;
       if (xlo) {
-        const double* pm = base + lc[0] * 5 * TS::FP(0);
+        int st;
+        const double* pm = dg_flux_ptr<ND, N, 0>(XH, Fh, lc[0], teff[0], fp, st);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) R[0][v] = fma(a.lift[0], pm[v * TS::FP(0)], R[0][v]);
+        for (int v = 0; v < 5; ++v) R[0][v] = fma(a.lift[0], pm[v * st], R[0][v]);
       }
       if (xhi) {
-        const double* pp = base + (lc[0] + 1) * 5 * TS::FP(0);
+        int st;
+        const double* pp = dg_flux_ptr<ND, N, 0>(XH, Fh, lc[0] + 1, teff[0], fp, st);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) R[SEG - 1][v] = fma(-a.lift[0], pp[v * TS::FP(0)], R[SEG - 1][v]);
+        for (int v = 0; v < 5; ++v) R[SEG - 1][v] = fma(-a.lift[0], pp[v * st], R[SEG - 1][v]);
       }
     }
     if constexpr (ND >= 2)
-      dg_lift_seg<ND, N, 1>(Fh, j, lc[1], i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
+      dg_lift_seg<ND, N, 1>(XH, Fh, j, lc[1], teff[1], i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
     if constexpr (ND >= 3)
-      dg_lift_seg<ND, N, 2>(Fh, k, lc[2], i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
+      dg_lift_seg<ND, N, 2>(XH, Fh, k, lc[2], teff[2], i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
@@ -712,14 +743,11 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 #pragma unroll
     for (int m = 0; m < SEG; ++m) Uo[m][v] = a.b * fma(dt, R[m][v], u[m]);
   }
-  if (a.a != 0.0 && active) {
+  if (need_u0) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      double u0[SEG];
-      dg_ld_line<SEG>(a.U0 + v * a.ndof + g0, u0);
+    for (int v = 0; v < 5; ++v)
 #pragma unroll
-      for (int m = 0; m < SEG; ++m) Uo[m][v] = fma(a.a, u0[m], Uo[m][v]);
-    }
+      for (int m = 0; m < SEG; ++m) Uo[m][v] = fma(a.a, U0r[v][m], Uo[m][v]);
   }
 
   // 5. physicality-enforcing operator (cell-local: warp shuffles)
@@ -744,9 +772,10 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   //    passed the screen (stricter than Eq. 25), so con2prim's own admissibility test is skipped there.
   double speed = 0.0;
   if (active) {
-    double Po[SEG];
+    double Po[SEG], Pg[SEG];
     int st[SEG];
-    dg_con2prim_n<EOS, SEG, false>(a.eos, Uo, nullptr, Po, st, &cnt[3], flagged);
+    dg_ld_line<SEG>(X + 8 * NS + s0, Pg);                 // Newton starts from the node's previous pressure
+    dg_con2prim_n<EOS, SEG, false>(a.eos, Uo, nullptr, Po, st, &cnt[3], flagged, Pg);
 #pragma unroll
     for (int m = 0; m < SEG; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;
 #pragma unroll
@@ -765,7 +794,8 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       }
     }
   }
-  // block totals: counters (rare) and the CFL maximum
+  // warp totals -> slotted global counters (rare) and CFL maximum (one atomic per warp): no block barrier
+  const int slot = (int)((blockIdx.x + 7u * blockIdx.y + 13u * blockIdx.z + 5u * (unsigned)wrp) % DG_NSLOT) * DG_SLOT_STRIDE;
 #pragma unroll
   for (int c = 0; c < 4; ++c) {
     const unsigned any = __ballot_sync(0xffffffffu, cnt[c] != 0);
@@ -773,23 +803,12 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       int x = cnt[c];
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-      if (lane == 0) atomicAdd(&sCnt[c], x);
+      if (lane == 0) atomicAdd(&a.counters[slot + c], (dg_ull)x);
     }
   }
   if (a.do_cfl) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
-    if (lane == 0) sRed[wrp] = speed;
-  }
-  __syncthreads();
-  if (t < 32) {
-    const int slot = (int)((blockIdx.x + 7u * blockIdx.y + 13u * blockIdx.z) % DG_NSLOT) * DG_SLOT_STRIDE;
-    if (a.do_cfl) {
-      double y = (t < NT / 32) ? sRed[t] : 0.0;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) y = fmax(y, __shfl_xor_sync(0xffffffffu, y, o));
-      if (t == 0 && y > 0.0) atomicMax(a.amax + slot, dg_ord(y));
-    }
-    if (t < 4 && sCnt[t]) atomicAdd(&a.counters[slot + t], (dg_ull)sCnt[t]);
+    if (lane == 0 && speed > 0.0) atomicMax(a.amax + slot, dg_ord(speed));
   }
 }

@@ -91,18 +91,18 @@ DG_INL void dg_prim2con(const EosPar& e, const double W[5], double U[5]) {
 
 // What the flux and the wave speeds need at a node, from its conserved state U and its pressure
 // P = P(U) (recovered once per node by the stage that produced U and kept in HBM, 8 B per node):
-//   3-velocity  v = M / (E + P)                 (Eq. 4: M = gamma^2 rho h v, E + P = gamma^2 rho h),
+//   r = 1/(E + P);  3-velocity  v = M r        (Eq. 4: M = gamma^2 rho h v, E + P = gamma^2 rho h),
 //   q = 1 - |v|^2 = 1/gamma^2,   rho h = (E + P) q,
 //   sigma_s = cs^2 / (gamma^2 (1 - cs^2)) of Eq. 22 as an unevaluated fraction num/den:
 //     ideal (Eq. 9, cs^2 = G P/(rho h)):   num = G P q,  den = rho h - G P;
 //     Taub-Matthews (Eq. 11 times rho^2, R := rho sqrt(Theta^2 + 4/9) = (2 rho h - 5 P)/3 by Eq. 10,
 //     rho^2 = 9/4 (R^2 - P^2)):            num = (3 P^2 + 5 P R) q,  den = 9/2 (P^2 + R^2) + 7 P R.
-// No square root and one reciprocal; rho itself is never needed.
+// No square root and one reciprocal; rho itself is never needed.  The flux of Eq. 2 in direction d is
+//   F_d = [D v_d, M v_d + P e_d, (E + P) v_d] = [D v_d, M v_d + P e_d, M_d].
 template <int EOS>
-DG_INL void dg_derive(const EosPar& e, const double U[5], double P, double v[3], double& num, double& den) {
-  const double r = dg_rcp(U[4] + P);
-  v[0] = U[1] * r; v[1] = U[2] * r; v[2] = U[3] * r;
-  const double q = fma(-v[0], v[0], fma(-v[1], v[1], fma(-v[2], v[2], 1.0)));
+DG_INL void dg_sigma_r(const EosPar& e, const double U[5], double P, double r, double& num, double& den) {
+  const double m2 = fma(U[1], U[1], fma(U[2], U[2], U[3] * U[3]));
+  const double q = fma(-r * r, m2, 1.0);
   const double rh = (U[4] + P) * q;
   if (EOS == DG_EOS_IDEAL) {
     const double GP = e.G * P;
@@ -114,6 +114,12 @@ DG_INL void dg_derive(const EosPar& e, const double U[5], double P, double v[3],
     num = fma(3.0 * P, P, 5.0 * PR) * q;
     den = fma(4.5, fma(P, P, R * R), 7.0 * PR);
   }
+}
+template <int EOS>
+DG_INL void dg_derive(const EosPar& e, const double U[5], double P, double v[3], double& num, double& den) {
+  const double r = dg_rcp(U[4] + P);
+  v[0] = U[1] * r; v[1] = U[2] * r; v[2] = U[3] * r;
+  dg_sigma_r<EOS>(e, U, P, r, num, den);
 }
 
 // lambda-+ of Eq. 21 with sigma = num/den substituted, as fractions over the common positive

@@ -20,7 +20,8 @@
 // Steps:
 //   1. own lines and the one-node-deep face layers of the neighbouring elements (GLL nodes: the face
 //      interpolation of :132-134 is a gather, reading R1; periodic wrap / outflow copy, R12) -> records
-//      in shared memory: U, v = M/(E+P), P and the fraction sigma = num/den of Eq. 22;
+//      in shared memory: U, P and r = 1/(E+P) (v = M r; the fraction sigma = num/den of Eq. 22 is
+//      re-derived at the face points);
 //   2. HLL interface flux (Eq. 21-24, reading R9) at every face point of the tile, once each, spread
 //      over the block's threads; volume quadrature (Eq. 17) over the diagonal mass matrix, F_d =
 //      U v_d + P e_d (Eq. 2) formed on the fly from the records;
@@ -88,11 +89,12 @@ struct TileShape {
   static constexpr int NHP = (NHALO + 1) / 2 * 2;    // row stride of the halo array
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
   static constexpr int NFACEI = FOFFI(ND);           // of which between two elements of the tile
-  // shared memory, in doubles.  Node records X[11][NS] = D Mx My Mz E | vx vy vz | P | num den (conserved
-  // state, 3-velocity, pressure, sigma = num/den of Eq. 22); halo points XH[6][NHP] = D Mx My Mz E | P.
+  // shared memory, in doubles.  Node records X[7][NS] = D Mx My Mz E | P | r (conserved state, pressure,
+  // r = 1/(E+P): v = M r); halo points XH[6][NHP] = D Mx My Mz E | P.  Shared-memory bandwidth is a
+  // co-equal bound of this kernel, so the records hold only what cannot be re-derived in a few flops.
   // The interface flux of a face point on the tile's boundary overwrites rows 0..4 of the halo point
   // it was computed from (read and written by the same thread); Fhat holds the interior planes only.
-  static constexpr int NREC = 11, HREC = 6;
+  static constexpr int NREC = 7, HREC = 6;
   static constexpr int O_X = 0;
   static constexpr int O_XH = O_X + NREC * NS;
   static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][interior plane][5][FP]
@@ -327,12 +329,11 @@ DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, 
     cL = aa * q; cR = -bb * q; cU = nl * nr * q;
   }
   const double kL = fma(cL, vL, -cU), kR = fma(cR, vR, cU);
-  const double pL = cL * PL, pR = cR * PR;
   double f[5];
 #pragma unroll
-  for (int v = 0; v < 5; ++v) f[v] = fma(kL, UL[v], kR * UR[v]);
-  f[1 + D] += pL + pR;
-  f[4] = fma(pL, vL, fma(pR, vR, f[4]));
+  for (int v = 0; v < 4; ++v) f[v] = fma(kL, UL[v], kR * UR[v]);
+  f[1 + D] += fma(cL, PL, cR * PR);
+  f[4] = fma(cL, UL[1 + D], fma(cR, UR[1 + D], cU * (UR[4] - UL[4])));   // (E + P) v_n = M_n
 #pragma unroll
   for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
 }
@@ -385,21 +386,15 @@ template <int ND, int N, int EOS, int D>
 DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, double U[5], double& vn,
                          double& P, double& num, double& den) {
   using TS = TileShape<ND, N>;
-  if (halo) {
+  const int S = halo ? TS::NHP : TS::NS;
 #pragma unroll
-    for (int v = 0; v < 5; ++v) U[v] = x[v * TS::NHP];
-    P = x[5 * TS::NHP];
-    double v3[3];
-    dg_derive<EOS>(eos, U, P, v3, num, den);
-    vn = v3[D];
-  } else {
-#pragma unroll
-    for (int v = 0; v < 5; ++v) U[v] = x[v * TS::NS];
-    vn = x[(5 + D) * TS::NS];
-    P = x[8 * TS::NS];
-    num = x[9 * TS::NS];
-    den = x[10 * TS::NS];
-  }
+  for (int v = 0; v < 5; ++v) U[v] = x[v * S];
+  P = x[5 * S];
+  double r;
+  if (halo) r = dg_rcp(U[4] + P);
+  else r = x[6 * TS::NS];
+  vn = U[1 + D] * r;
+  dg_sigma_r<EOS>(eos, U, P, r, num, den);
 }
 
 template <int ND, int N, int EOS, int D>
@@ -415,8 +410,8 @@ DG_INL void dg_face_point(const EosPar& eos, const double* X, double* XH, double
 
 // Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
 // diagonal mass matrix): for each q the segment at index q along D -- SEG adjacent slots -- is read
-// with vector loads and F_D = U v_D + P e_D is formed on the fly.  dh: (2/h_D) Dhat[id][q] of this
-// thread's index id along D.
+// with vector loads and F_D = [D v_D, M v_D + P e_D, M_D], v_D = M_D r, is formed on the fly.
+// dh: (2/h_D) Dhat[id][q] of this thread's index id along D.
 template <int ND, int N, int D>
 DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double (*R)[5]) {
   using TS = TileShape<ND, N>;
@@ -425,22 +420,19 @@ DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double
   for (int q = 0; q < N; ++q) {
     const double* x = X + s_line0 + q * TS::SS(D);
     const double c = dh[q];
-    double vd[SEG], Pq[SEG], t[SEG];
-    dg_ld_line<SEG>(x + (5 + D) * S, vd);
-    dg_ld_line<SEG>(x + 8 * S, Pq);
+    double u[4][SEG], Pq[SEG], rq[SEG];
 #pragma unroll
-    for (int m = 0; m < SEG; ++m) t[m] = c * vd[m];
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      double u[SEG];
-      dg_ld_line<SEG>(x + v * S, u);
-#pragma unroll
-      for (int m = 0; m < SEG; ++m) R[m][v] = fma(t[m], u[m], R[m][v]);
-    }
+    for (int v = 0; v < 4; ++v) dg_ld_line<SEG>(x + v * S, u[v]);
+    dg_ld_line<SEG>(x + 5 * S, Pq);
+    dg_ld_line<SEG>(x + 6 * S, rq);
 #pragma unroll
     for (int m = 0; m < SEG; ++m) {
+      const double md = u[1 + D][m];
+      const double t = (c * rq[m]) * md;                 // (2/h) Dhat v_D
+#pragma unroll
+      for (int v = 0; v < 4; ++v) R[m][v] = fma(t, u[v][m], R[m][v]);
       R[m][1 + D] = fma(c, Pq[m], R[m][1 + D]);
-      R[m][4] = fma(t[m], Pq[m], R[m][4]);
+      R[m][4] = fma(c, md, R[m][4]);
     }
   }
 }
@@ -451,31 +443,25 @@ template <int ND, int N>
 DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, double (*R)[5]) {
   using TS = TileShape<ND, N>;
   constexpr int S = TS::NS, SEG = TS::SEG;
-  double vx[N], Pq[N], c[SEG][N], t[SEG][N];
-  dg_ld_line<N>(X + s_line + 5 * S, vx);
-  dg_ld_line<N>(X + s_line + 8 * S, Pq);
+  double u[4][N], Pq[N], rq[N], c[SEG][N];
 #pragma unroll
-  for (int m = 0; m < SEG; ++m) {
-    dg_ld_line<N>(dh + m * N, c[m]);
+  for (int v = 0; v < 4; ++v) dg_ld_line<N>(X + s_line + v * S, u[v]);
+  dg_ld_line<N>(X + s_line + 5 * S, Pq);
+  dg_ld_line<N>(X + s_line + 6 * S, rq);
 #pragma unroll
-    for (int q = 0; q < N; ++q) t[m][q] = c[m][q] * vx[q];
-  }
+  for (int m = 0; m < SEG; ++m) dg_ld_line<N>(dh + m * N, c[m]);
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {
-    double u[N];
-    dg_ld_line<N>(X + s_line + v * S, u);
+  for (int q = 0; q < N; ++q) {
+    const double vx = u[1][q] * rq[q];
 #pragma unroll
-    for (int m = 0; m < SEG; ++m)
+    for (int m = 0; m < SEG; ++m) {
+      const double t = c[m][q] * vx;
 #pragma unroll
-      for (int q = 0; q < N; ++q) R[m][v] = fma(t[m][q], u[q], R[m][v]);
-  }
-#pragma unroll
-  for (int m = 0; m < SEG; ++m)
-#pragma unroll
-    for (int q = 0; q < N; ++q) {
+      for (int v = 0; v < 4; ++v) R[m][v] = fma(t, u[v][q], R[m][v]);
       R[m][1] = fma(c[m][q], Pq[q], R[m][1]);
-      R[m][4] = fma(t[m][q], Pq[q], R[m][4]);
+      R[m][4] = fma(c[m][q], u[1][q], R[m][4]);
     }
+  }
 }
 
 // Flux of face plane p of direction D at face point fp: in the halo slot for the tile's boundary
@@ -638,31 +624,24 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 #pragma unroll
     for (int v = 0; v < 5; ++v) R[m][v] = 0.0;
   if (active) {
-    double vl[3][SEG], numl[SEG], denl[SEG];
+    double rl[SEG];
 #pragma unroll
-    for (int m = 0; m < SEG; ++m) {
-      const double Um[5] = {Ul[0][m], Ul[1][m], Ul[2][m], Ul[3][m], Ul[4][m]};
-      double v3[3];
-      dg_derive<EOS>(a.eos, Um, Pl[m], v3, numl[m], denl[m]);
-      vl[0][m] = v3[0]; vl[1][m] = v3[1]; vl[2][m] = v3[2];
-    }
+    for (int m = 0; m < SEG; ++m) rl[m] = dg_rcp(Ul[4][m] + Pl[m]);
     DG_ASSERT(s0 >= 0 && s0 + SEG <= NS);
 #pragma unroll
     for (int v = 0; v < 5; ++v) dg_st_line<SEG>(X + v * NS + s0, Ul[v]);
-#pragma unroll
-    for (int d = 0; d < 3; ++d) dg_st_line<SEG>(X + (5 + d) * NS + s0, vl[d]);
-    dg_st_line<SEG>(X + 8 * NS + s0, Pl);
-    dg_st_line<SEG>(X + 9 * NS + s0, numl);
-    dg_st_line<SEG>(X + 10 * NS + s0, denl);
+    dg_st_line<SEG>(X + 5 * NS + s0, Pl);
+    dg_st_line<SEG>(X + 6 * NS + s0, rl);
     // volume term, x direction, for whole-line threads in registers: R_i += sum_q (2/h_x) Dhat[i][q] F_x(q)
     if (NSEG == 1 && N > 1) {
       double Fx[SEG][5];
 #pragma unroll
       for (int m = 0; m < SEG; ++m) {
+        const double vx = Ul[1][m] * rl[m];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) Fx[m][v] = Ul[v][m] * vl[0][m];
+        for (int v = 0; v < 4; ++v) Fx[m][v] = Ul[v][m] * vx;
         Fx[m][1] += Pl[m];
-        Fx[m][4] = fma(Pl[m], vl[0][m], Fx[m][4]);
+        Fx[m][4] = Ul[1][m];
       }
 #pragma unroll
       for (int m = 0; m < SEG; ++m)
@@ -774,7 +753,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   if (active) {
     double Po[SEG], Pg[SEG];
     int st[SEG];
-    dg_ld_line<SEG>(X + 8 * NS + s0, Pg);                 // Newton starts from the node's previous pressure
+    dg_ld_line<SEG>(X + 5 * NS + s0, Pg);                 // Newton starts from the node's previous pressure
     dg_con2prim_n<EOS, SEG, false>(a.eos, Uo, nullptr, Po, st, &cnt[3], flagged, Pg);
 #pragma unroll
     for (int m = 0; m < SEG; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;

@@ -238,13 +238,16 @@ DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, 
     c3[s] = -2.0 * fma(al, eta[s], 1.0);
     c2[s] = 2.0 * (al + 1.0) * xi[s];
     c1[s] = -2.0 * fma(al, eta[s], -1.0);
-    general[s] = !(E[s] < 1e30) || !(Mabs[s] > 1e-30) || !(eta[s] < 1e30) || !(xi[s] >= 1e-4);
+    // (E or |M| outside the single-precision range only degrades the starting point: 0 or 0.999999)
+    general[s] = !(eta[s] < 1e30) || !(xi[s] >= 1e-4);
     run[s] = !general[s];
     // starting point in single precision: b0 = xi/eta, w0 = b0 / (1 + sqrt(1 - b0^2))
     const float xf = __double2float_rn(Mabs[s]);
     const float ef = __double2float_rn(Pg ? E[s] + fmax(Pg[s], 0.0) : E[s]);
     const float b0 = fminf(__fdividef(xf, ef), 1.0f);
-    const float w0 = fminf(__fdividef(b0, 1.0f + sqrtf(fmaxf(fmaf(-b0, b0, 1.0f), 0.0f))), 0.999999f);
+    float sq;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sq) : "f"(fmaxf(fmaf(-b0, b0, 1.0f), 0.0f)));
+    const float w0 = fminf(__fdividef(b0, 1.0f + sq), 0.999999f);
     w[s] = (double)w0;
     any = any || run[s];
   }

@@ -86,22 +86,25 @@ struct TileShape {
     return d <= 0 ? 0 : FOFFI(d - 1) + (T(d - 1) - 1) * FP(d - 1);
   }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
-  static constexpr int NHP = (NHALO + 1) / 2 * 2;    // row stride of the halo array
+  static constexpr int NHP = (NHALO + 1) / 2 * 2;    // halo slots per row (even)
   static constexpr int NFACE = FOFF(ND);             // face points of the tile (all directions)
   static constexpr int NFACEI = FOFFI(ND);           // of which between two elements of the tile
-  // shared memory, in doubles.  Node records X[7][NS] = D Mx My Mz E | P | r (conserved state, pressure,
-  // r = 1/(E+P): v = M r); halo points XH[6][NHP] = D Mx My Mz E | P.  Shared-memory bandwidth is a
-  // co-equal bound of this kernel, so the records hold only what cannot be re-derived in a few flops.
-  // The interface flux of a face point on the tile's boundary overwrites rows 0..4 of the halo point
-  // it was computed from (read and written by the same thread); Fhat holds the interior planes only.
-  static constexpr int NREC = 7, HREC = 6;
+  // shared memory, in doubles.  Records X[7][RS]: row = D Mx My Mz E | P | r (conserved state, pressure,
+  // r = 1/(E+P): v = M r); a row holds the NS node slots of the tile followed by its NHP halo points
+  // (rows 0..5 only), so that a face point addresses either kind of side with the same row stride.
+  // Shared-memory bandwidth is a co-equal bound of this kernel, so the records hold only what cannot
+  // be re-derived in a few flops.  The interface flux of a face point on the tile's boundary
+  // overwrites rows 0..4 of the halo point it was computed from (read and written by the same
+  // thread); Fhat holds the interior planes only.
+  static constexpr int NREC = 7;
+  static constexpr int RS = NS + NHP;                // row stride
   static constexpr int O_X = 0;
-  static constexpr int O_XH = O_X + NREC * NS;
-  static constexpr int O_FH = O_XH + HREC * NHP;     // Fhat  [dir][interior plane][5][FP]
+  static constexpr int O_FH = O_X + NREC * RS;       // Fhat  [dir][interior plane][5][FP]
   static constexpr int O_D = O_FH + (5 * NFACEI + 1) / 2 * 2;  // (2/h_d) Dhat[i][q] for d = x, y, z
   static constexpr int SMEM_BYTES = (O_D + 3 * 26) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
-  static constexpr int BLK_REG = 65536 / (NT * 80);    // leave >= 80 registers per thread
+  static constexpr int REG_FLOOR = (SEG <= 1) ? 64 : ((SEG >= 6) ? 240 : 40 * SEG);   // registers per thread to leave
+  static constexpr int BLK_REG = 65536 / (NT * REG_FLOOR);
   static constexpr int MINB = (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) > 0 ? (BLK_SMEM < BLK_REG ? BLK_SMEM : BLK_REG) : 1;
 };
 
@@ -338,20 +341,18 @@ DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, 
   for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
 }
 
-// Where the two sides of face point fl of direction D live: a tile node record (rows U | v | P |
-// num den, row stride NS) or a halo point (rows U | P, row stride NHP; velocity and sigma are derived
-// at use -- each halo point is used by exactly one face point).  Returns false for face points outside
-// a ragged tile.
+// Where the two sides of face point fl of direction D live: slots of the record rows -- a tile node
+// (< NS) or a halo point (>= NS: rows U | P only; r is derived at use, each halo point is used by
+// exactly one face point) -- and where its flux goes: the halo slot of a boundary plane, else the
+// interior-plane array.  Returns false for face points outside a ragged tile.
 struct FaceSides {
-  const double* xl; const double* xr;   // record bases
-  bool hl, hr;                          // side is a halo point
-  double* pF;                           // Fhat[0] of this point
-  int fstride;                          // stride between the flux components
+  int sl, sr;        // record slots of the left / right side
+  bool hl, hr;       // side is a halo point
+  int of, fstride;   // flux destination: offset from the start of shared memory, component stride
 };
 
 template <int ND, int N, int D>
-DG_INL bool dg_face_sides(const double* X, double* XH, double* Fh, int fl, const int teff[3],
-                          FaceSides& fs) {
+DG_INL bool dg_face_sides(int fl, const int teff[3], FaceSides& fs) {
   using TS = TileShape<ND, N>;
   constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
   constexpr int FPD = TS::FP(D);
@@ -364,48 +365,40 @@ DG_INL bool dg_face_sides(const double* X, double* XH, double* Fh, int fl, const
   const int telem = la * TS::SE(A) + lb * TS::SE(B);
   fs.hl = (p < 1);
   fs.hr = (p >= teff[D]);
-  const int sl = (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
-  const int sr = (telem + p * TS::SE(D)) * TS::ES + tnode;
-  DG_ASSERT(fs.hl || (sl >= 0 && sl < TS::NS));
-  DG_ASSERT(fs.hr || (sr >= 0 && sr < TS::NS));
+  const int hl_slot = TS::NS + TS::HOFF(D) + fp, hr_slot = hl_slot + FPD;
+  fs.sl = fs.hl ? hl_slot : (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
+  fs.sr = fs.hr ? hr_slot : (telem + p * TS::SE(D)) * TS::ES + tnode;
+  DG_ASSERT(fs.sl >= 0 && fs.sl < TS::RS && fs.sr >= 0 && fs.sr < TS::RS);
   DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
-  fs.xl = fs.hl ? XH + (TS::HOFF(D) + fp) : X + sl;
-  fs.xr = fs.hr ? XH + (TS::HOFF(D) + FPD + fp) : X + sr;
-  // where the flux goes: the halo slot of a boundary plane, else the interior plane p-1
-  if (fs.hl) { fs.pF = XH + (TS::HOFF(D) + fp); fs.fstride = TS::NHP; }
-  else if (fs.hr) { fs.pF = XH + (TS::HOFF(D) + FPD + fp); fs.fstride = TS::NHP; }
-  else {
-    DG_ASSERT(p >= 1 && 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACEI);
-    fs.pF = Fh + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
-    fs.fstride = FPD;
-  }
+  const int oi = TS::O_FH + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
+  fs.of = fs.hl ? hl_slot : (fs.hr ? hr_slot : oi);
+  fs.fstride = (fs.hl || fs.hr) ? TS::RS : FPD;
+  DG_ASSERT(fs.hl || fs.hr || (p >= 1 && 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACEI));
   return true;
 }
 
 template <int ND, int N, int EOS, int D>
 DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, double U[5], double& vn,
                          double& P, double& num, double& den) {
-  using TS = TileShape<ND, N>;
-  const int S = halo ? TS::NHP : TS::NS;
+  constexpr int S = TileShape<ND, N>::RS;
 #pragma unroll
   for (int v = 0; v < 5; ++v) U[v] = x[v * S];
   P = x[5 * S];
   double r;
   if (halo) r = dg_rcp(U[4] + P);
-  else r = x[6 * TS::NS];
+  else r = x[6 * S];
   vn = U[1 + D] * r;
   dg_sigma_r<EOS>(eos, U, P, r, num, den);
 }
 
 template <int ND, int N, int EOS, int D>
-DG_INL void dg_face_point(const EosPar& eos, const double* X, double* XH, double* Fh, int fl,
-                          const int teff[3]) {
+DG_INL void dg_face_point(const EosPar& eos, double* sm, int fl, const int teff[3]) {
   FaceSides fs;
-  if (!dg_face_sides<ND, N, D>(X, XH, Fh, fl, teff, fs)) return;
+  if (!dg_face_sides<ND, N, D>(fl, teff, fs)) return;
   double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
-  dg_load_side<ND, N, EOS, D>(eos, fs.xl, fs.hl, UL, vL, PL, numL, denL);
-  dg_load_side<ND, N, EOS, D>(eos, fs.xr, fs.hr, UR, vR, PR, numR, denR);
-  dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, fs.pF, fs.fstride);
+  dg_load_side<ND, N, EOS, D>(eos, sm + fs.sl, fs.hl, UL, vL, PL, numL, denL);
+  dg_load_side<ND, N, EOS, D>(eos, sm + fs.sr, fs.hr, UR, vR, PR, numR, denR);
+  dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, sm + fs.of, fs.fstride);
 }
 
 // Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
@@ -415,7 +408,7 @@ DG_INL void dg_face_point(const EosPar& eos, const double* X, double* XH, double
 template <int ND, int N, int D>
 DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int S = TS::NS, SEG = TS::SEG;
+  constexpr int S = TS::RS, SEG = TS::SEG;
 #pragma unroll
   for (int q = 0; q < N; ++q) {
     const double* x = X + s_line0 + q * TS::SS(D);
@@ -442,7 +435,7 @@ DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double
 template <int ND, int N>
 DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int S = TS::NS, SEG = TS::SEG;
+  constexpr int S = TS::RS, SEG = TS::SEG;
   double u[4][N], Pq[N], rq[N], c[SEG][N];
 #pragma unroll
   for (int v = 0; v < 4; ++v) dg_ld_line<N>(X + s_line + v * S, u[v]);
@@ -465,44 +458,41 @@ DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, doubl
 }
 
 // Flux of face plane p of direction D at face point fp: in the halo slot for the tile's boundary
-// planes (p == 0, p == teffD), else in the interior-plane array.  Returns the row stride.
+// planes (p == 0, p == teffD), else in the interior-plane array.  Returns the offset from the start
+// of shared memory; stride: the distance between the flux components.
 template <int ND, int N, int D>
-DG_INL const double* dg_flux_ptr(const double* XH, const double* Fh, int p, int teffD, int fp, int& stride) {
+DG_INL int dg_flux_off(int p, int teffD, int fp, int& stride) {
   using TS = TileShape<ND, N>;
   constexpr int FPD = TS::FP(D);
-  if (p == 0) { stride = TS::NHP; return XH + (TS::HOFF(D) + fp); }
-  if (p == teffD) { stride = TS::NHP; return XH + (TS::HOFF(D) + FPD + fp); }
-  stride = FPD;
-  return Fh + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
+  const bool lo = (p == 0), hi = (p == teffD);
+  stride = (lo || hi) ? TS::RS : FPD;
+  const int oh = TS::NS + TS::HOFF(D) + fp;
+  return lo ? oh : (hi ? oh + FPD : TS::O_FH + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp);
 }
 
 // Lift of the interface flux of direction D = 1 or 2 onto the thread's nodes (Eq. 18): the segment
-// lies in the element's minus face (id == 0: + c Fhat) and / or plus face (id == N-1: - c Fhat).
+// lies in the element's minus face (id == 0: + c Fhat) or plus face (id == N-1: - c Fhat); for
+// N == 1 in both.
 template <int ND, int N, int D>
-DG_INL void dg_lift_seg(const double* XH, const double* Fh, int id, int lcD, int teffD, int fp0, double c,
-                        double (*R)[5]) {
+DG_INL void dg_lift_seg(const double* sm, int id, int lcD, int teffD, int fp0, double c, double (*R)[5]) {
   using TS = TileShape<ND, N>;
   constexpr int SEG = TS::SEG;
-  if (id == 0) {
+  if (id == 0 || id == N - 1) {
+    const bool plus = (N > 1) && (id == N - 1);
+    const double cs = plus ? -c : c;
     int st;
-    const double* p = dg_flux_ptr<ND, N, D>(XH, Fh, lcD, teffD, fp0, st);
+    const double* p = sm + dg_flux_off<ND, N, D>(lcD + (plus ? 1 : 0), teffD, fp0, st);
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
       double f[SEG];
       dg_ld_line<SEG>(p + v * st, f);
 #pragma unroll
-      for (int m = 0; m < SEG; ++m) R[m][v] = fma(c, f[m], R[m][v]);
+      for (int m = 0; m < SEG; ++m) R[m][v] = fma(cs, f[m], R[m][v]);
     }
-  }
-  if (id == N - 1) {
-    int st;
-    const double* p = dg_flux_ptr<ND, N, D>(XH, Fh, lcD + 1, teffD, fp0, st);
+    if (N == 1) {                                 // the single node lies in both faces
+      const double* p2 = sm + dg_flux_off<ND, N, D>(lcD + 1, teffD, fp0, st);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      double f[SEG];
-      dg_ld_line<SEG>(p + v * st, f);
-#pragma unroll
-      for (int m = 0; m < SEG; ++m) R[m][v] = fma(-c, f[m], R[m][v]);
+      for (int v = 0; v < 5; ++v) R[0][v] = fma(-c, p2[v * st], R[0][v]);
     }
   }
 }
@@ -511,12 +501,11 @@ template <int ND, int N, int EOS>
 __global__ void __launch_bounds__(TileShape<ND, N>::NT, TileShape<ND, N>::MINB)
 dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
-  constexpr int NN = TS::NN, NT = TS::NT, NL = TS::NL, NS = TS::NS, NHP = TS::NHP;
+  constexpr int NN = TS::NN, NT = TS::NT, NL = TS::NL, RS = TS::RS;
   constexpr int SEG = TS::SEG, NSEG = TS::NSEG;
   extern __shared__ __align__(16) double sm[];
-  double* X = sm + TS::O_X;
-  double* XH = sm + TS::O_XH;
-  double* Fh = sm + TS::O_FH;
+  double* X = sm + TS::O_X;                // records: node slots, then (XH) halo slots, row stride RS
+  double* XH = X + TS::NS;
   double* sDx = sm + TS::O_D;
   double* sDy = sDx + 26;
   double* sDz = sDy + 26;
@@ -565,16 +554,16 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
         DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + fp < TS::NHALO);
         double* dst = XH + (TS::HOFF(0) + fp);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_copy8(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_copy8(dst + 5 * RS, a.Pin + g);
       }
       if (xhi && lc[0] == teff[0] - 1) {
         const int g = g0 + (SEG - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
         DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + TS::FP(0) + fp < TS::NHALO);
         double* dst = XH + (TS::HOFF(0) + TS::FP(0) + fp);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_copy8(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_copy8(dst + 5 * RS, a.Pin + g);
       }
     }
     if constexpr (ND >= 2) {                                         // y: the thread's segment of the line
@@ -584,16 +573,16 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
         DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(1) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
       }
       if (j == N - 1 && lc[1] == teff[1] - 1) {
         const int g = g0 + a.hoff[1][1] + ((org[1] + teff[1] == a.ne[1]) ? a.hfix[1][1] : 0);
         DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(1) + TS::FP(1) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
       }
     }
     if constexpr (ND >= 3) {                                         // z: the thread's segment of the line
@@ -603,16 +592,16 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
         DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(2) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
       }
       if (k == N - 1 && lc[2] == teff[2] - 1) {
         const int g = g0 + a.hoff[2][1] + ((org[2] + teff[2] == a.ne[2]) ? a.hfix[2][1] : 0);
         DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + SEG <= TS::NHALO);
         double* dst = XH + (TS::HOFF(2) + TS::FP(2) + fp0);
 #pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * NHP, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * NHP, a.Pin + g);
+        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
       }
     }
   }
@@ -627,11 +616,11 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
     double rl[SEG];
 #pragma unroll
     for (int m = 0; m < SEG; ++m) rl[m] = dg_rcp(Ul[4][m] + Pl[m]);
-    DG_ASSERT(s0 >= 0 && s0 + SEG <= NS);
+    DG_ASSERT(s0 >= 0 && s0 + SEG <= TS::NS);
 #pragma unroll
-    for (int v = 0; v < 5; ++v) dg_st_line<SEG>(X + v * NS + s0, Ul[v]);
-    dg_st_line<SEG>(X + 5 * NS + s0, Pl);
-    dg_st_line<SEG>(X + 6 * NS + s0, rl);
+    for (int v = 0; v < 5; ++v) dg_st_line<SEG>(X + v * RS + s0, Ul[v]);
+    dg_st_line<SEG>(X + 5 * RS + s0, Pl);
+    dg_st_line<SEG>(X + 6 * RS + s0, rl);
     // volume term, x direction, for whole-line threads in registers: R_i += sum_q (2/h_x) Dhat[i][q] F_x(q)
     if (NSEG == 1 && N > 1) {
       double Fx[SEG][5];
@@ -658,9 +647,9 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_point<ND, N, EOS, 0>(a.eos, X, XH, Fh, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_point<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(1), teff);
-    else dg_face_point<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, X, XH, Fh, f - TS::FOFF(2), teff);
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_point<ND, N, EOS, 0>(a.eos, sm, f, teff);
+    else if (ND == 2 || f < TS::FOFF(2)) dg_face_point<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, sm, f - TS::FOFF(1), teff);
+    else dg_face_point<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, sm, f - TS::FOFF(2), teff);
   }
   //    volume quadrature: reads the records only, so it needs no barrier here
   if (active && N > 1) {
@@ -683,21 +672,21 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
       if (xlo) {
         int st;
-        const double* pm = dg_flux_ptr<ND, N, 0>(XH, Fh, lc[0], teff[0], fp, st);
+        const double* pm = sm + dg_flux_off<ND, N, 0>(lc[0], teff[0], fp, st);
 #pragma unroll
         for (int v = 0; v < 5; ++v) R[0][v] = fma(a.lift[0], pm[v * st], R[0][v]);
       }
       if (xhi) {
         int st;
-        const double* pp = dg_flux_ptr<ND, N, 0>(XH, Fh, lc[0] + 1, teff[0], fp, st);
+        const double* pp = sm + dg_flux_off<ND, N, 0>(lc[0] + 1, teff[0], fp, st);
 #pragma unroll
         for (int v = 0; v < 5; ++v) R[SEG - 1][v] = fma(-a.lift[0], pp[v * st], R[SEG - 1][v]);
       }
     }
     if constexpr (ND >= 2)
-      dg_lift_seg<ND, N, 1>(XH, Fh, j, lc[1], teff[1], i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
+      dg_lift_seg<ND, N, 1>(sm, j, lc[1], teff[1], i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]), a.lift[1], R);
     if constexpr (ND >= 3)
-      dg_lift_seg<ND, N, 2>(XH, Fh, k, lc[2], teff[2], i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
+      dg_lift_seg<ND, N, 2>(sm, k, lc[2], teff[2], i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]), a.lift[2], R);
   }
   if (a.mode == DG_MODE_RHS) {
     if (active) {
@@ -718,7 +707,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
 #pragma unroll
   for (int v = 0; v < 5; ++v) {
     double u[SEG];
-    dg_ld_line<SEG>(X + v * NS + (active ? s0 : 0), u);
+    dg_ld_line<SEG>(X + v * RS + (active ? s0 : 0), u);
 #pragma unroll
     for (int m = 0; m < SEG; ++m) Uo[m][v] = a.b * fma(dt, R[m][v], u[m]);
   }
@@ -753,7 +742,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   if (active) {
     double Po[SEG], Pg[SEG];
     int st[SEG];
-    dg_ld_line<SEG>(X + 5 * NS + s0, Pg);                 // Newton starts from the node's previous pressure
+    dg_ld_line<SEG>(X + 5 * RS + s0, Pg);                 // Newton starts from the node's previous pressure
     dg_con2prim_n<EOS, SEG, false>(a.eos, Uo, nullptr, Po, st, &cnt[3], flagged, Pg);
 #pragma unroll
     for (int m = 0; m < SEG; ++m) cnt[2] += (st[m] != 0) ? 1 : 0;

@@ -153,6 +153,12 @@ int dgrhd_con2prim_batch_host(int eos, double gamma_ad, int64_t n, const double*
 int dgrhd_run_host(dgrhd_ctx* ctx, const double* U_host_in, double* U_host_out, double dt,
                    int nsteps, double* t_inout_host);
 
+/* Measurement aid: sustained FP64 FMA throughput of the current device in TFLOP/s (best of four
+ * ~2 ms launches of a register-only DFMA kernel, timed with CUDA events on cuda_stream; synchronises).
+ * It is the measured denominator of the "alu" roofline bench.py reports.  scratch_dev: >= 8 bytes of
+ * device memory.  sm_mhz_host (or NULL) receives the device's nominal maximum SM clock. */
+int dgrhd_probe_fp64(void* scratch_dev, double* tflops_host, double* sm_mhz_host, void* cuda_stream);
+
 /* Text of the last error of this context (ctx = NULL: of the last context-free call on this
  * thread).  Never NULL; valid until the next call on the same context / thread. */
 const char* dgrhd_last_error(const dgrhd_ctx* ctx);

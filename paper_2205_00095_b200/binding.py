@@ -52,7 +52,7 @@ _vp, _dp, _i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
 EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_state",
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
-           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count",
+           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64",
            "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
 
 
@@ -79,6 +79,7 @@ def lib():
         L.dgrhd_get_counters.argtypes = [_vp, _i64p, C.c_int]
         L.dgrhd_con2prim_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp, _vp]
         L.dgrhd_tm_fallback_count.argtypes = [_i64p, C.c_int, _vp]
+        L.dgrhd_probe_fp64.argtypes = [_vp, _dp, _dp, _vp]
         L.dgrhd_prim2con_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp]
         L.dgrhd_con2prim_batch_host.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp,
                                                 C.c_size_t, _vp]
@@ -227,6 +228,14 @@ def dgrhd_tm_fallback_count(reset=False):
     out = C.c_int64()
     _check(lib().dgrhd_tm_fallback_count(C.byref(out), int(reset), _stream()))
     return out.value
+
+
+def dgrhd_probe_fp64():
+    """(sustained FP64 FMA TFLOP/s of the current device, nominal max SM clock in MHz)."""
+    scratch = torch.zeros(1, dtype=torch.float64, device="cuda")
+    tf, mhz = C.c_double(), C.c_double()
+    _check(lib().dgrhd_probe_fp64(_ptr(scratch), C.byref(tf), C.byref(mhz), _stream()))
+    return tf.value, mhz.value
 
 
 def dgrhd_prim2con_batch(eos, gamma_ad, W, U=None):

@@ -173,6 +173,24 @@ dg_limiter_kernel(long long nelem, long long ndof, double* U, unsigned char* fla
   }
 }
 
+// FP64 FMA throughput probe (the roofline denominator of the ALU-bound kernels, measured on the box
+// instead of derived from unit counts): 8 independent DFMA chains per thread, no memory traffic.
+__global__ void __launch_bounds__(256)
+dg_fp64_probe_kernel(double* out, int iters, double seed) {
+  double x[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) x[c] = seed + 1e-3 * (threadIdx.x + c);
+  const double a = 0.999999, b = 1e-7;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) x[c] = fma(x[c], a, b);
+  }
+  double sum = 0.0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) sum += x[c];
+  if (sum == 123.456) out[0] = sum;                 // never true: keeps the chains alive
+}
+
 // dt for the coming step, on the device: fixed (dt_fixed > 0) or cfl / amax (reading R11); consumes
 // the accumulated maximum (the step's last stage refills it), advances the elapsed time.  A maximum
 // that is not a positive finite number (every speed NaN after con2prim failures, an empty state)

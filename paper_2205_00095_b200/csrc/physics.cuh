@@ -278,10 +278,19 @@ DG_INL void dg_ideal_solve_w(const EosPar& e, const double* D, const double* E, 
 // (eta-xi)(eta+xi), acos argument clamped, Wv >= 0).  The closed form returns Wv as a difference of
 // O(c1) terms, so it is polished on the cubic itself by Newton steps (reading R7b), which makes the
 // accuracy of the transcendental part irrelevant: it is evaluated in single precision and followed by
-// three Newton steps, after which the last step must satisfy |dWv| <= 1e-13 Wv + 1e-300 (quadratic
-// convergence from a 1e-7 seed ends far below that).  A state that fails the test -- PAPER.md:392:
-// Newton on this cubic "is not guaranteed to converge to the positive root" from a poor start -- takes
-// the fallback: the same closed form in double precision plus two Newton steps; *nfall counts them.
+// two to four Newton steps with a convergence test on the last step (quadratic convergence from a
+// 1e-7 seed).  A state that fails the test -- PAPER.md:392: Newton on this cubic "is not guaranteed to
+// converge to the positive root" from a poor start -- takes the fallback: the same closed form in
+// double precision plus two Newton steps; *nfall counts them.
+// one Newton step on Eq. 61 with a single-precision reciprocal (self-correcting: the step's relative
+// error 6e-8 only adds 6e-8 |dW| to the new iterate's error)
+DG_INL double dg_tm_cubic_newton_lo(double Wv, double c1, double c2, double c3, double& dW) {
+  const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
+  const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
+  dW = -f * dg_rcp_lo(df);
+  const double Wn = Wv + dW;
+  return fmax(Wn, 0.0);
+}
 DG_INL double dg_tm_cubic_newton(double Wv, double c1, double c2, double c3, double& dW) {
   const double f = fma(fma(Wv + c1, Wv, c2), Wv, c3);
   const double df = fma(fma(3.0, Wv, 2.0 * c1), Wv, c2);
@@ -331,10 +340,11 @@ DG_INL void dg_tm_solve_W(const double* D, const double* E, const double* Mabs, 
     const double d = fma(R, R, Q3);                                // Eq. 65
     double W0;
     if (d < 0.0) {
-      double arg = R * dg_rsqrt(-Q3);
+      const double rq = dg_rsqrt(-Q);                                        // 1/sqrt(-Q): serves both roots
+      double arg = R * (rq * rq * rq);
       arg = fmin(1.0, fmax(-1.0, arg));
       const float th = acosf((float)arg) * (1.0f / 3.0f);
-      W0 = 2.0 * dg_sqrt(-Q) * (double)cosf(th) - c1 * (1.0 / 3.0);          // Eq. 69-70
+      W0 = 2.0 * (-Q * rq) * (double)cosf(th) - c1 * (1.0 / 3.0);            // Eq. 69-70
     } else {
       const double sd = dg_sqrt(d);
       const double p = R + sd, q = R - sd;
@@ -343,13 +353,21 @@ DG_INL void dg_tm_solve_W(const double* D, const double* E, const double* Mabs, 
       W0 = cp + cq - c1 * (1.0 / 3.0);                                       // Eq. 71-73
     }
     W0 = fmax(W0, 0.0);
+    // R7b polish: two steps square the ~1e-7 seed error twice; the step is a tight estimate of the error
+    // before it, so |dW| <= 1e-9 W certifies the fp64 floor.  States that are not there yet (gamma -> 1,
+    // where W is tiny against the seed's absolute error) take two more steps in full precision.
     double dW;
-    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);                             // R7b
-    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
-    W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
-    if (!(fabs(dW) <= fma(1e-13, W0, 1e-300))) {                             // not converged / NaN
-      W0 = dg_tm_closed_form_fp64(c1, c2, c3);
-      if (nfall) *nfall += 1;
+    W0 = dg_tm_cubic_newton_lo(W0, c1, c2, c3, dW);
+    W0 = dg_tm_cubic_newton_lo(W0, c1, c2, c3, dW);
+    if (!(fabs(dW) <= 1e-9 * W0)) {
+      W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
+      W0 = dg_tm_cubic_newton(W0, c1, c2, c3, dW);
+      if (!(fabs(dW) <= fma(1e-13, W0, 1e-300))) {                           // not converged / NaN
+        W0 = dg_tm_closed_form_fp64(c1, c2, c3);
+        // overflowed coefficients (E/D beyond ~1e77) have no root to offer: fail the state (status 2)
+        if (!isfinite(c1) || !isfinite(c2) || !isfinite(c3)) W0 = __longlong_as_double(0x7ff8000000000000LL);
+        if (nfall) *nfall += 1;
+      }
     }
     Wv[s] = W0;
   }
@@ -416,10 +434,12 @@ DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5],
       const double beta = ug * rg;
       const double rho = D[s] * rg;
       const double X = fma(-beta, Mabs[s], E[s]);                  // E - M.v
-      const double Pv = (X - rho) * (X + rho) * dg_rcp(3.0 * X);   // Eq. 75
+      const double X3 = 3.0 * X;
+      const double rr = dg_rcp(FULL ? X3 * Mabs[s] : X3);          // one reciprocal for 1/(3X) and 1/|M|
+      const double Pv = (X - rho) * (X + rho) * (FULL ? rr * Mabs[s] : rr);   // Eq. 75
       bool ok = isfinite(Pv) && (Pv > 0.0);
       if (FULL) {
-        const double sc = (Mabs[s] > 0.0) ? ug * dg_rcp(Mabs[s]) : 0.0;
+        const double sc = ug * (rr * X3);                          // gamma beta / |M|
         W[s][0] = rho; W[s][1] = sc * U[s][1]; W[s][2] = sc * U[s][2]; W[s][3] = sc * U[s][3]; W[s][4] = Pv;
         ok = ok && dg_finite5(W[s]);
       } else {

@@ -11,27 +11,41 @@ import numpy as np
 from .build import build as _build
 
 EOS_IDEAL, EOS_TM = 0, 1
-BC_PERIODIC, BC_OUTFLOW = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_DIRICHLET = 0, 1, 2, 3
+RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 
 
 class Config(C.Structure):
     _fields_ = [("ndim", C.c_int), ("nelem", C.c_int64 * 3), ("xmin", C.c_double * 3),
                 ("xmax", C.c_double * 3), ("bc", C.c_int * 3), ("order_p", C.c_int),
                 ("eos", C.c_int), ("gamma_ad", C.c_double), ("rk_stages", C.c_int),
-                ("eps_q", C.c_double), ("delta_s", C.c_double)]
+                ("eps_q", C.c_double), ("delta_s", C.c_double), ("riemann", C.c_int),
+                ("bc_state", C.c_double * 5 * 2 * 3)]
+
+
+def _bc_code(b):
+    """int (both ends) or (lo, hi) -> lo + 256*hi (hi = 0: same as lo)."""
+    if isinstance(b, (tuple, list)):
+        lo, hi = int(b[0]), int(b[1])
+        return lo + 256 * (hi if hi != lo else 0)
+    return int(b)
 
 
 def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3,
-                eps_q=1e-12, delta_s=1e-10):
+                eps_q=1e-12, delta_s=1e-10, riemann=0, bc_state=None):
     c = Config()
     c.ndim = ndim
     for d in range(3):
         c.nelem[d] = int(nelem[d]) if d < ndim else 1
         c.xmin[d] = float(xmin[d]) if d < ndim else 0.0
         c.xmax[d] = float(xmax[d]) if d < ndim else 1.0
-        c.bc[d] = int(bc[d]) if d < ndim else 0
+        c.bc[d] = _bc_code(bc[d]) if d < ndim else 0
     c.order_p, c.eos, c.gamma_ad, c.rk_stages = order_p, eos, gamma_ad, rk_stages
     c.eps_q, c.delta_s = eps_q, delta_s
+    c.riemann = int(riemann)
+    for (d, side), W in (bc_state or {}).items():      # {(axis, side): [rho, ux, uy, uz, P]}
+        for v in range(5):
+            c.bc_state[d][side][v] = float(W[v])
     return c
 
 
@@ -107,6 +121,15 @@ def wavespeeds(eos, G, W, d):
     lib().orc_wavespeeds(C.c_int(eos), C.c_double(G), _p(_v5(W)), C.c_int(d), C.byref(lm),
                          C.byref(lp))
     return lm.value, lp.value
+
+
+def hllc(eos, G, WL, WR, d):
+    """Returns (F, lambda*, U*_L, U*_R)."""
+    F, UsL, UsR = np.zeros(5), np.zeros(5), np.zeros(5)
+    ls = C.c_double()
+    lib().orc_hllc(C.c_int(eos), C.c_double(G), _p(_v5(WL)), _p(_v5(WR)), C.c_int(d), _p(F), C.byref(ls),
+                   _p(UsL), _p(UsR))
+    return F, ls.value, UsL, UsR
 
 
 def hll(eos, G, WL, WR, d):

@@ -136,6 +136,64 @@ void orc_hll(int eos, double G, const double WL[5], const double WR[5], int dir,
     F[v] = (lR * FL[v] - lL * FR[v] + lL * lR * (UR[v] - UL[v])) / (lR - lL);
 }
 
+/* HLLC three-wave flux.  PAPER.md:126/:161/:551 names it ("HLL and HLLC variants ... Mignone and
+ * Bodo [34]") without printing it; this is ref [34]'s construction, with lambda_L, lambda_R of
+ * Eq. 23-24 as for HLL.  From the HLL state and flux
+ *   U^hll = (lR U_R - lL U_L + F_L - F_R)/(lR - lL),  F^hll = (lR F_L - lL F_R + lL lR (U_R - U_L))/(lR - lL)
+ * the contact speed lambda* is the root with the minus sign of
+ *   F_E^hll l^2 - (E^hll + F_m^hll) l + m^hll = 0        (m = momentum normal to the face),
+ * p* = -F_E^hll l* + F_m^hll, and for K = L, R (v, p: normal velocity and pressure of side K):
+ *   D*  = D (lK - v)/(lK - l*),            m_t* = m_t (lK - v)/(lK - l*)   (transverse momenta),
+ *   m*  = (m (lK - v) + p* - p)/(lK - l*), E*   = (E (lK - v) + p* l* - p v)/(lK - l*);
+ * flux:  F_L (lL >= 0);  F_L + lL (U*_L - U_L) (lL < 0 <= l*);  F_R + lR (U*_R - U_R) (l* < 0 <= lR);
+ * F_R (lR < 0).  A vanishing leading coefficient (|F_E^hll| tiny) makes the quadratic linear. */
+void orc_hllc(int eos, double G, const double WL[5], const double WR[5], int dir, double F[5],
+              double *lstar_out, double UsL_out[5], double UsR_out[5]) {
+  double lmL, lpL, lmR, lpR;
+  orc_wavespeeds(eos, G, WL, dir, &lmL, &lpL);
+  orc_wavespeeds(eos, G, WR, dir, &lmR, &lpR);
+  double lL = fmin(lmL, lmR);                                   /* Eq. 23 */
+  double lR = fmax(lpL, lpR);                                   /* Eq. 24 */
+  double FL[5], FR[5], UL[5], UR[5], Uh[5], Fh[5];
+  orc_flux(eos, G, WL, dir, FL);
+  orc_flux(eos, G, WR, dir, FR);
+  orc_prim2con(eos, G, WL, UL);
+  orc_prim2con(eos, G, WR, UR);
+  for (int v = 0; v < 5; ++v) {
+    Uh[v] = (lR * UR[v] - lL * UL[v] + FL[v] - FR[v]) / (lR - lL);
+    Fh[v] = (lR * FL[v] - lL * FR[v] + lL * lR * (UR[v] - UL[v])) / (lR - lL);
+  }
+  const int im = 1 + dir;
+  double a = Fh[4], b = -(Uh[4] + Fh[im]), cc = Uh[im];
+  double ls;
+  if (fabs(a) > 1e-14 * fabs(b)) {
+    double disc = sqrt(fmax(b * b - 4.0 * a * cc, 0.0));
+    /* the root with the minus sign, written without cancellation (b < 0): 2c / (-b + disc) */
+    ls = 2.0 * cc / (-b + disc);
+  } else {
+    ls = -cc / b;
+  }
+  double ps = -Fh[4] * ls + Fh[im];
+  double Us[2][5];
+  for (int K = 0; K < 2; ++K) {
+    const double *U = K ? UR : UL, *W = K ? WR : WL;
+    double lK = K ? lR : lL;
+    double g = sqrt(1.0 + W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+    double v = W[im] / g, p = W[4];
+    double den = lK - ls;
+    for (int k = 0; k < 4; ++k) Us[K][k] = U[k] * (lK - v) / den;
+    Us[K][im] = (U[im] * (lK - v) + ps - p) / den;
+    Us[K][4] = (U[4] * (lK - v) + ps * ls - p * v) / den;
+  }
+  if (lstar_out) *lstar_out = ls;
+  if (UsL_out) for (int v = 0; v < 5; ++v) UsL_out[v] = Us[0][v];
+  if (UsR_out) for (int v = 0; v < 5; ++v) UsR_out[v] = Us[1][v];
+  if (lL >= 0.0) { for (int v = 0; v < 5; ++v) F[v] = FL[v]; return; }
+  if (lR <= 0.0) { for (int v = 0; v < 5; ++v) F[v] = FR[v]; return; }
+  if (ls >= 0.0) { for (int v = 0; v < 5; ++v) F[v] = FL[v] + lL * (Us[0][v] - UL[v]); }
+  else           { for (int v = 0; v < 5; ++v) F[v] = FR[v] + lR * (Us[1][v] - UR[v]); }
+}
+
 /* ------------------------------------------------------------------------------------------
  * O7 predicate: Eq. 25 with the PLUS sign under the root (reading R13a; Eq. 27/31/32), the
  * safety factor (1-eps) on E (R13c), separately rounded operations in this order (R13e).
@@ -380,20 +438,26 @@ void orc_rhs(const orc_config *c, const double *U, double *R, int64_t *n_c2p_fai
           if (side == 1 && in[d] != N - 1) continue;    /* l_i(+1) = delta_{i,p} */
           int64_t je[3] = {ie[0], ie[1], ie[2]};
           je[d] += side ? 1 : -1;
-          int has_nb = 1;
+          int has_nb = 1, bck = ORC_BC_PERIODIC;
           if (je[d] < 0 || je[d] >= nel[d]) {
-            if (c->bc[d] == ORC_BC_PERIODIC) je[d] = (je[d] + nel[d]) % nel[d];
-            else has_nb = 0;                            /* outflow: ghost = own face state (R12) */
+            const int lo = c->bc[d] & 255, hi = (c->bc[d] >> 8) & 255;
+            bck = (side && hi) ? hi : lo;               /* condition at this end of the axis */
+            if (bck == ORC_BC_PERIODIC) je[d] = (je[d] + nel[d]) % nel[d];
+            else has_nb = 0;                            /* a ghost state stands in for the neighbour */
           }
           int64_t en = je[0] + nx * (je[1] + ny * je[2]);
           int n_nb = n + ((side ? 0 : N - 1) - in[d]) * str[d];   /* neighbour's facing node */
           double Wown[5], Wnb[5], Fh[5];
           for (int v = 0; v < 5; ++v) {
             Wown[v] = W[v * ndof + e * nn + n];
-            Wnb[v] = has_nb ? W[v * ndof + en * nn + n_nb] : Wown[v];
+            Wnb[v] = has_nb ? W[v * ndof + en * nn + n_nb] : Wown[v];   /* outflow: own state (R12) */
           }
-          if (side) orc_hll(c->eos, c->gamma_ad, Wown, Wnb, d, Fh);   /* left = own  */
-          else      orc_hll(c->eos, c->gamma_ad, Wnb, Wown, d, Fh);   /* left = neighbour */
+          if (!has_nb && bck == ORC_BC_REFLECT) Wnb[1 + d] = -Wnb[1 + d];          /* wall */
+          if (!has_nb && bck == ORC_BC_DIRICHLET)
+            for (int v = 0; v < 5; ++v) Wnb[v] = c->bc_state[d][side][v];           /* fixed state */
+          const double *WLp = side ? Wown : Wnb, *WRp = side ? Wnb : Wown;       /* left = lower x_d */
+          if (c->riemann == ORC_RIEMANN_HLLC) orc_hllc(c->eos, c->gamma_ad, WLp, WRp, d, Fh, 0, 0, 0);
+          else orc_hll(c->eos, c->gamma_ad, WLp, WRp, d, Fh);
           for (int v = 0; v < 5; ++v) term[v] -= side ? Fh[v] : -Fh[v];
         }
         for (int v = 0; v < 5; ++v) acc[v] += (2.0 / h[d]) * (1.0 / w[in[d]]) * term[v];

@@ -18,7 +18,13 @@
 #include <stdint.h>
 
 enum { ORC_EOS_IDEAL = 0, ORC_EOS_TM = 1 };
-enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1 };
+/* Boundary conditions.  bc[d] = lo + 256*hi: lo = condition at the low
+ * end of axis d, hi = at the high end (hi = 0: the same as lo -- periodic is always both ends).
+ *   OUTFLOW    ghost face state = own face state (reading R12)
+ *   REFLECT    ghost = own state with the normal velocity reversed (a wall, :541 test 5)
+ *   DIRICHLET  ghost = the fixed primitive state bc_state[d][side] (:541 tests 1-4) */
+enum { ORC_BC_PERIODIC = 0, ORC_BC_OUTFLOW = 1, ORC_BC_REFLECT = 2, ORC_BC_DIRICHLET = 3 };
+enum { ORC_RIEMANN_HLL = 0, ORC_RIEMANN_HLLC = 1 };
 
 typedef struct {
   int     ndim;          /* 1,2,3 */
@@ -30,6 +36,8 @@ typedef struct {
   double  gamma_ad;
   int     rk_stages;     /* 1,2,3 */
   double  eps_q, delta_s;
+  int     riemann;       /* ORC_RIEMANN_*: interface flux */
+  double  bc_state[3][2][5];   /* Dirichlet ghost primitives [axis][side] = rho, ux, uy, uz, P */
 } orc_config;
 
 /* O4: GLL tables for N = p+1 nodes: x[N], w[N], D[q*N+i] = l_i'(x_q). */
@@ -42,6 +50,10 @@ void   orc_prim2con(int eos, double G, const double W[5], double U[5]);
 void   orc_flux(int eos, double G, const double W[5], int dir, double F[5]);
 void   orc_wavespeeds(int eos, double G, const double W[5], int dir, double *lm, double *lp);
 void   orc_hll(int eos, double G, const double WL[5], const double WR[5], int dir, double F[5]);
+/* HLLC of Mignone & Bodo (PAPER.md:161 ref [34]); lstar_out (may be NULL) receives lambda*;
+ * UsL/UsR (may be NULL) the two star states */
+void   orc_hllc(int eos, double G, const double WL[5], const double WR[5], int dir, double F[5],
+                double *lstar_out, double UsL[5], double UsR[5]);
 
 /* O2/O3: returns status 0 ok, 1 inadmissible input (W = NaN), 2 solver/pressure failure.
  * niter_out (may be NULL) receives the Newton iteration count (ideal EOS). */

@@ -16,7 +16,8 @@ import math
 import torch
 
 EOS_IDEAL, EOS_TM = 0, 1
-BC_PERIODIC, BC_OUTFLOW = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_DIRICHLET = 0, 1, 2, 3
+RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 
 # positions of the N = p+1 nodes on [-1, 1] (Gauss-Lobatto-Legendre, reading R1)
 _NODES = {
@@ -67,7 +68,8 @@ def _u_from_v(v):
 
 def _cfg(ndim, nelem, xmin, xmax, bc, p, eos, gamma_ad, **kw):
     d = dict(ndim=ndim, nelem=list(nelem), xmin=list(xmin), xmax=list(xmax), bc=list(bc),
-             order_p=p, eos=eos, gamma_ad=gamma_ad, rk_stages=3, eps_q=1e-12, delta_s=1e-10)
+             order_p=p, eos=eos, gamma_ad=gamma_ad, rk_stages=3, eps_q=1e-12, delta_s=1e-10,
+             riemann=RIEMANN_HLL, bc_state=None)
     d.update(kw)
     return d
 
@@ -95,6 +97,33 @@ def riemann1d(seed, ne=256, p=2, device="cpu", states=None):
     W = torch.cat([rho[side][None], _u_from_v(v), P[side][None]]).to(device)
     cfg = _cfg(1, [ne], [0.0], [1.0], [BC_OUTFLOW], p, EOS_IDEAL, 5.0 / 3.0)
     return cfg, W.contiguous()
+
+
+# The five 1D Riemann problems of PAPER.md:537-583 as printed (Eq. 85-89): (rho, vx, vy, P) left and
+# right of x = 0.5 on [0,1], adiabatic index, end time; tests 1-4 Dirichlet at both ends, test 5 a
+# uniform state with a reflecting wall at x = 1.
+PAPER_RIEMANN_1D = {
+    1: dict(L=(10.0, 0.0, 0.0, 40.0 / 3.0), R=(1.0, 0.0, 0.0, 2.0 / 3.0 * 1e-6), gamma_ad=5.0 / 3.0, t_end=0.4),
+    2: dict(L=(1.0, 0.0, 0.0, 1e3), R=(1.0, 0.0, 0.0, 1e-2), gamma_ad=5.0 / 3.0, t_end=0.4),
+    3: dict(L=(1.0, 0.0, 0.0, 1e3), R=(1.0, 0.0, 0.99, 1e-2), gamma_ad=5.0 / 3.0, t_end=0.4),
+    4: dict(L=(1.0, 0.01, 0.0, 1.0), R=(0.125, 0.01, 0.0, 0.1), gamma_ad=4.0 / 3.0, t_end=0.4),
+    5: dict(L=(1.0, 0.99999, 0.0, 0.01), R=(1.0, 0.99999, 0.0, 0.01), gamma_ad=4.0 / 3.0, t_end=1.5),
+}
+
+
+def paper_riemann1d(k, ne=256, p=2, device="cpu", riemann=RIEMANN_HLL):
+    """Problem k = 1..5 of PAPER.md:537-583 (Eq. 85-89) with the paper's boundary conditions."""
+    pr = PAPER_RIEMANN_1D[k]
+    cfg, W = riemann1d(0, ne=ne, p=p, device=device, states=(pr["L"], pr["R"]))
+
+    def prim(s):                       # (rho, vx, vy, P) -> [rho, ux, uy, uz, P]
+        g = 1.0 / math.sqrt(1.0 - s[1] ** 2 - s[2] ** 2)
+        return [s[0], g * s[1], g * s[2], 0.0, s[3]]
+
+    cfg.update(gamma_ad=pr["gamma_ad"], riemann=riemann,
+               bc=[(BC_DIRICHLET, BC_REFLECT if k == 5 else BC_DIRICHLET)],
+               bc_state={(0, 0): prim(pr["L"]), (0, 1): prim(pr["R"])})
+    return cfg, W, pr["t_end"]
 
 
 # ---------------------------------------------------------------------------------------------

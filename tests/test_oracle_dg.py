@@ -459,3 +459,87 @@ def test_admissible_predicate_uses_plus_sign_and_rejects_nan():
     assert not O.admissible([0.0, 0, 0, 0, 1.0])                 # D = 0 is not > 0
     assert not O.admissible([1.0, float("nan"), 0, 0, 5.0])
     assert O.admissible([1.0, 0, 0, 0, 1.0 + 1e-9], 1e-12) and not O.admissible([1.0, 0, 0, 0, 1.0 + 1e-13], 1e-12)
+
+
+# ------------------------------------------------------------------------------------------------
+# Boundary conditions beyond periodic / outflow and the HLLC operator
+# ------------------------------------------------------------------------------------------------
+def _cfgx(d, **kw):
+    d = {**d, **kw}
+    return O.make_config(d["ndim"], d["nelem"], d["xmin"], d["xmax"], d["bc"], d["order_p"], d["eos"],
+                         d["gamma_ad"], d["rk_stages"], d["eps_q"], d["delta_s"], d.get("riemann", 0),
+                         d.get("bc_state"))
+
+
+@pytest.mark.parametrize("riemann", [O.RIEMANN_HLL, O.RIEMANN_HLLC])
+def test_reflecting_wall_equals_the_mirrored_domain(riemann):
+    """A wall at x = 1 is the symmetry plane of the domain [0,2] filled with the mirror image (normal
+    velocity reversed): the residual on [0,1] must be the same -- without using the wall's formula."""
+    ne, p = 9, 2
+    N = p + 1
+    d = I._cfg(1, [ne], [0.0], [1.0], [(I.BC_OUTFLOW, I.BC_REFLECT)], p, 0, 5.0 / 3.0, riemann=riemann)
+    W, _, _ = _smooth_field(1, [ne], N, [0.0], [1.0], seed=4)
+    W = W.copy()
+    W[2] *= 0.5
+    Wm = W[:, ::-1].copy()                                  # mirror image about x = 1 (GLL nodes are symmetric)
+    Wm[1] = -Wm[1]
+    dd = dict(d, nelem=[2 * ne], xmax=[2.0], bc=[I.BC_OUTFLOW])
+    U, Ud = O.prim2con_batch(0, 5.0 / 3.0, W), O.prim2con_batch(0, 5.0 / 3.0, np.hstack([W, Wm]))
+    R, _ = O.rhs(_cfgx(d), U)
+    Rd, _ = O.rhs(_cfgx(dd), Ud)
+    np.testing.assert_allclose(R, Rd[:, :ne * N], rtol=1e-12, atol=1e-12)
+    assert np.max(np.abs(R[:, -N:] - O.rhs(_cfgx(dict(d, bc=[I.BC_OUTFLOW])), U)[0][:, -N:])) > 1e-3
+
+
+@pytest.mark.parametrize("nd", [1, 2])
+def test_dirichlet_boundary_equals_a_layer_of_ghost_elements_and_keeps_the_free_stream(nd):
+    """Fixed ghost primitives at a Dirichlet face act exactly like one more element filled with that
+    state; if the state equals the interior's uniform state the residual vanishes."""
+    p, N = 2, 3
+    ghostL, ghostR = [2.0, 0.3, -0.1, 0.05, 1.5], [0.4, -0.2, 0.2, 0.0, 0.3]
+    nel = [7, 4][:nd]
+    d = I._cfg(nd, nel, [0.0] * nd, [1.0, 0.5][:nd], [I.BC_DIRICHLET] + [I.BC_PERIODIC] * (nd - 1), p, 1, 0.0,
+               bc_state={(0, 0): ghostL, (0, 1): ghostR})
+    W, _, _ = _smooth_field(nd, nel, N, [0.0] * nd, [1.0, 0.5][:nd], seed=8)
+    U = O.prim2con_batch(1, 0.0, W)
+    R, _ = O.rhs(_cfgx(d), U)
+    # the same mesh with one more element at each end of x holding the ghost states, outflow beyond
+    nn = N ** nd
+    nel2 = [nel[0] + 2] + nel[1:]
+    W2 = np.zeros((5, int(np.prod(nel2)) * nn))
+    for row in range(int(np.prod(nel[1:])) if nd > 1 else 1):
+        base2, base = row * nel2[0] * nn, row * nel[0] * nn
+        W2[:, base2:base2 + nn] = np.array(ghostL)[:, None]
+        W2[:, base2 + nn:base2 + nn + nel[0] * nn] = W[:, base:base + nel[0] * nn]
+        W2[:, base2 + nn + nel[0] * nn:base2 + nel2[0] * nn] = np.array(ghostR)[:, None]
+    h = 1.0 / nel[0]
+    d2 = dict(d, nelem=nel2, xmin=[-h] + [0.0] * (nd - 1), xmax=[1.0 + h, 0.5][:nd],
+              bc=[I.BC_OUTFLOW] + [I.BC_PERIODIC] * (nd - 1), bc_state=None)
+    R2, _ = O.rhs(_cfgx(d2), O.prim2con_batch(1, 0.0, W2))
+    for row in range(int(np.prod(nel[1:])) if nd > 1 else 1):
+        base2, base = row * nel2[0] * nn, row * nel[0] * nn
+        np.testing.assert_allclose(R[:, base:base + nel[0] * nn], R2[:, base2 + nn:base2 + nn + nel[0] * nn],
+                                   rtol=1e-12, atol=1e-12)
+    Wu = np.repeat(np.array(ghostL)[:, None], W.shape[1], axis=1)
+    Ru, _ = O.rhs(_cfgx(dict(d, bc_state={(0, 0): ghostL, (0, 1): ghostL})), O.prim2con_batch(1, 0.0, Wu))
+    assert np.max(np.abs(Ru)) < 1e-11
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_paper_riemann_problems_stay_admissible_and_conserve_up_to_the_boundary_flux(k):
+    """PAPER.md Eq. 85-89 with HLLC, p = 2, the physicality operator after every stage (no shock
+    limiter: oscillatory but admissible, :551): finite, admissible at every node, and -- Dirichlet
+    states equal to the untouched far field -- the mass in the domain changes only through the known
+    boundary fluxes (tests 1-4: none until a wave arrives; test 5: inflow at x = 0, none at the wall)."""
+    d, W, t_end = I.paper_riemann1d(k, ne=64, p=2, riemann=I.RIEMANN_HLLC)
+    U = O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy())
+    cfg = _cfgx(d)
+    U1, t, cnt = O.step(cfg, U, -0.2, 40)
+    assert np.isfinite(U1).all() and cnt[1] == 0 and cnt[2] == 0
+    for i in range(U1.shape[1]):
+        assert O.admissible(U1[:, i])
+    w = np.tile(_node_weights(1, 3), 64) * (1.0 / 64) / 2.0
+    mass0, mass1 = (w * U[0]).sum(), (w * U1[0]).sum()
+    inflow = U[0, 0] * (W[1, 0] / np.sqrt(1 + W[1, 0] ** 2 + W[2, 0] ** 2)) * t     # D v_x at x = 0
+    outflow = 0.0 if k == 5 else U[0, -1] * float(W[1, -1] / np.sqrt(1 + W[1, -1] ** 2 + W[2, -1] ** 2)) * t
+    assert abs((mass1 - mass0) - (float(inflow) - outflow)) <= 1e-10 * mass0

@@ -368,3 +368,76 @@ def test_con2prim_rejects_inadmissible_states(eos, G):
               [1.0, 0.1, 0, 0, float("nan")]):
         W, st, _ = O.con2prim(eos, G, U)
         assert st == 1 and np.all(np.isnan(W))
+
+
+# ------------------------------------------------------------------------------------------------
+# HLLC interface flux (SURVEY.md 8(f).1; PAPER.md:126, :161 ref [34]) -- pins that do not restate it
+# ------------------------------------------------------------------------------------------------
+def _random_pair(rng, eos):
+    def one():
+        rho, P = 10.0 ** rng.uniform(-2, 1), 10.0 ** rng.uniform(-3, 1)
+        v = rng.uniform(-0.6, 0.6, 3)
+        g = 1.0 / np.sqrt(1.0 - v @ v)
+        return np.array([rho, *(g * v), P])
+    return one(), one()
+
+
+@pytest.mark.parametrize("eos,G", [(0, 5.0 / 3.0), (0, 4.0 / 3.0), (1, 0.0)])
+def test_hllc_star_states_satisfy_the_jump_conditions_of_all_three_waves(eos, G):
+    """Rankine-Hugoniot across lambda_L, lambda* and lambda_R, the integral (consistency) relation, the
+    contact conditions m* = (E* + p*) lambda* with ONE p* on both sides, and lambda_L <= lambda* <= lambda_R:
+    a dropped term or wrong sign in any star-state formula breaks one of them."""
+    rng = np.random.default_rng(3)
+    for _ in range(400):
+        WL, WR = _random_pair(rng, eos)
+        for d in range(3):
+            F, ls, UsL, UsR = O.hllc(eos, G, WL, WR, d)
+            lmL, lpL = O.wavespeeds(eos, G, WL, d)
+            lmR, lpR = O.wavespeeds(eos, G, WR, d)
+            lL, lR = min(lmL, lmR), max(lpL, lpR)
+            UL, UR = O.prim2con(eos, G, WL), O.prim2con(eos, G, WR)
+            FL, FR = O.flux(eos, G, WL, d), O.flux(eos, G, WR, d)
+            assert lL - 1e-14 <= ls <= lR + 1e-14
+            Uh = (lR * UR - lL * UL + FL - FR) / (lR - lL)
+            sc = np.abs(UL) + np.abs(UR) + 1e-300
+            assert np.max(np.abs((ls - lL) * UsL + (lR - ls) * UsR - (lR - lL) * Uh) / sc) < 1e-12
+            FsL, FsR = FL + lL * (UsL - UL), FR + lR * (UsR - UR)          # RH across the outer waves
+            assert np.max(np.abs(FsR - FsL - ls * (UsR - UsL)) / sc) < 1e-12   # RH across the contact
+            # one pressure on both sides of the contact, from either side's normal-momentum flux:
+            # F*_m = m* lambda* + p*  and  F*_E = m* ;  m* = (E* + p*) lambda*
+            m = 1 + d
+            pL, pR = FsL[m] - UsL[m] * ls, FsR[m] - UsR[m] * ls
+            assert abs(pL - pR) <= 1e-11 * max(abs(pL), 1e-3)
+            for Us, p in ((UsL, pL), (UsR, pR)):
+                assert abs(Us[m] - (Us[4] + p) * ls) <= 1e-11 * max(abs(Us[4]), 1e-3)
+
+
+def test_hllc_is_consistent_upwinds_and_mirrors():
+    rng = np.random.default_rng(5)
+    for eos, G in ((0, 5.0 / 3.0), (1, 0.0)):
+        for _ in range(50):
+            WL, WR = _random_pair(rng, eos)
+            for d in range(3):
+                F, _, _, _ = O.hllc(eos, G, WL, WL, d)                     # F(W, W) = F(W)
+                np.testing.assert_allclose(F, O.flux(eos, G, WL, d), rtol=1e-12, atol=1e-14)
+                Fm, _, _, _ = O.hllc(eos, G, WR * [1, -1, -1, -1, 1], WL * [1, -1, -1, -1, 1], d)
+                F, _, _, _ = O.hllc(eos, G, WL, WR, d)                     # mirror image
+                np.testing.assert_allclose(Fm, -F * [1, -1, -1, -1, 1], rtol=1e-11, atol=1e-13)
+        Ws = np.array([1.0, 3.0, 0.2, 0.0, 0.5])                           # supersonic to the right
+        F, _, _, _ = O.hllc(eos, G, Ws, Ws * [0.5, 1, 1, 1, 0.7], 0)
+        np.testing.assert_allclose(F, O.flux(eos, G, Ws, 0), rtol=1e-14)
+
+
+@pytest.mark.parametrize("eos,G", [(0, 5.0 / 3.0), (1, 0.0)])
+def test_hllc_preserves_an_isolated_contact_exactly_while_hll_smears_it(eos, G):
+    """Equal velocity and pressure, a density jump: the exact flux at the interface is the upwind one.
+    HLLC returns it to rounding (the point of the third wave); the two-wave HLL flux does not."""
+    for vx in (0.3, -0.45):
+        g = 1.0 / np.sqrt(1.0 - vx * vx - 0.04)
+        WL = np.array([1.0, g * vx, g * 0.2, 0.0, 0.7])
+        WR = np.array([0.05, g * vx, g * 0.2, 0.0, 0.7])
+        exact = O.flux(eos, G, WL if vx > 0 else WR, 0)
+        F, ls, _, _ = O.hllc(eos, G, WL, WR, 0)
+        assert abs(ls - vx) < 1e-13
+        np.testing.assert_allclose(F, exact, rtol=1e-12, atol=1e-14)
+        assert np.max(np.abs(O.hll(eos, G, WL, WR, 0) - exact)) > 1e-3

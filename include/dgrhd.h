@@ -37,8 +37,17 @@ typedef struct dgrhd_ctx dgrhd_ctx;          /* opaque, owned by the library, fr
 
 enum { DGRHD_EOS_IDEAL = 0,                  /* h = 1 + Gamma/(Gamma-1) Theta   (Eq. 8)  */
        DGRHD_EOS_TAUB_MATTHEWS = 1 };        /* h = 5/2 Theta + 3/2 sqrt(Theta^2+4/9)  (:89 Eq. 10)  */
+/* Boundary conditions.  bc[d] = lo + 256*hi (DGRHD_BC_PAIR): lo is the
+ * condition at the low end of axis d, hi at the high end; hi = 0 means "the same as lo" (periodic is
+ * always both ends), so a plain DGRHD_BC_* value sets both ends. */
 enum { DGRHD_BC_PERIODIC = 0,                /* wrap                                                  */
-       DGRHD_BC_OUTFLOW = 1 };               /* transmissive: ghost face state = own face state (:621)*/
+       DGRHD_BC_OUTFLOW = 1,                 /* transmissive: ghost face state = own face state (:621)*/
+       DGRHD_BC_REFLECT = 2,                 /* wall: ghost = own state, normal velocity reversed (:541)*/
+       DGRHD_BC_DIRICHLET = 3 };             /* ghost = the fixed primitive state bc_state[d][side] (:541)*/
+#define DGRHD_BC_PAIR(lo, hi) ((lo) + 256 * (((hi) == (lo)) ? 0 : (hi)))
+/* Interface (Riemann) flux: the two-wave HLL flux (reading R9) or the
+ * three-wave HLLC flux of Mignone & Bodo (ref [34]); both with lambda_L, lambda_R of Eq. 23-24. */
+enum { DGRHD_RIEMANN_HLL = 0, DGRHD_RIEMANN_HLLC = 1 };
 enum { DGRHD_OK = 0, DGRHD_EINVAL = 1, DGRHD_ENOMEM = 2, DGRHD_ECUDA = 3, DGRHD_ESTATE = 4 };
 
 /* Problem statement: mesh, order, EOS. */
@@ -46,13 +55,15 @@ typedef struct {
   int     ndim;            /* 1, 2 or 3                                                            */
   int64_t nelem[3];        /* elements per axis (unused axes must be 1)                            */
   double  xmin[3], xmax[3];/* domain; uniform Cartesian mesh, h_d = (xmax_d - xmin_d)/nelem_d     */
-  int     bc[3];           /* DGRHD_BC_* per axis (both ends of the axis)                          */
+  int     bc[3];           /* DGRHD_BC_* per axis, or DGRHD_BC_PAIR(lo, hi) for different ends             */
   int     order_p;         /* polynomial order 0..4; N = p+1 nodes per direction                  */
   int     eos;             /* DGRHD_EOS_*                                                          */
   double  gamma_ad;        /* adiabatic index Gamma (ideal EOS, > 1); ignored for Taub-Matthews    */
   int     rk_stages;       /* 1 (RK1), 2 (SSPRK2) or 3 (SSPRK3), Shu-Osher form */
   double  eps_q, delta_s;  /* safety knobs of the physicality operator (reading R13c);
                               0,0 = the paper verbatim; defaults used by the tests: 1e-12, 1e-10   */
+  int     riemann;         /* DGRHD_RIEMANN_*                                                       */
+  double  bc_state[3][2][5]; /* Dirichlet ghost primitives [axis][end] = rho, ux, uy, uz, P          */
 } dgrhd_config;
 
 /* Bytes of device workspace dgrhd_create needs for this configuration (0 if cfg is invalid). */

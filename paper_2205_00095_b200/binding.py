@@ -10,7 +10,8 @@ import os
 import torch
 
 EOS_IDEAL, EOS_TAUB_MATTHEWS = 0, 1
-BC_PERIODIC, BC_OUTFLOW = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_DIRICHLET = 0, 1, 2, 3
+RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
 OPT_CUDA_GRAPH = 0
 
@@ -29,20 +30,33 @@ class Config(C.Structure):
     _fields_ = [("ndim", C.c_int), ("nelem", C.c_int64 * 3), ("xmin", C.c_double * 3),
                 ("xmax", C.c_double * 3), ("bc", C.c_int * 3), ("order_p", C.c_int),
                 ("eos", C.c_int), ("gamma_ad", C.c_double), ("rk_stages", C.c_int),
-                ("eps_q", C.c_double), ("delta_s", C.c_double)]
+                ("eps_q", C.c_double), ("delta_s", C.c_double), ("riemann", C.c_int),
+                ("bc_state", C.c_double * 5 * 2 * 3)]
+
+
+def _bc_code(b):
+    """int (both ends) or (lo, hi) -> DGRHD_BC_PAIR(lo, hi)."""
+    if isinstance(b, (tuple, list)):
+        lo, hi = int(b[0]), int(b[1])
+        return lo + 256 * (hi if hi != lo else 0)
+    return int(b)
 
 
 def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3, eps_q=1e-12,
-                delta_s=1e-10):
+                delta_s=1e-10, riemann=0, bc_state=None):
     c = Config()
     c.ndim = ndim
     for d in range(3):
         c.nelem[d] = int(nelem[d]) if d < ndim else 1
         c.xmin[d] = float(xmin[d]) if d < ndim else 0.0
         c.xmax[d] = float(xmax[d]) if d < ndim else 1.0
-        c.bc[d] = int(bc[d]) if d < ndim else 0
+        c.bc[d] = _bc_code(bc[d]) if d < ndim else 0
     c.order_p, c.eos, c.gamma_ad, c.rk_stages = order_p, eos, gamma_ad, rk_stages
     c.eps_q, c.delta_s = eps_q, delta_s
+    c.riemann = int(riemann)
+    for (d, side), W in (bc_state or {}).items():      # {(axis, end): [rho, ux, uy, uz, P]}
+        for v in range(5):
+            c.bc_state[d][side][v] = float(W[v])
     return c
 
 

@@ -1,9 +1,9 @@
 """Build libdgrhd.so (the C-ABI CUDA library of include/dgrhd.h) in-tree for sm_100a.
 
-    python -m paper_2205_00095_b200.build [--force]
+    python -m paper_2205_00095_b200.build [--force] [-v] [--debug-asserts]
 
-nvcc cross-compiles without a GPU.  The fused stage kernel is instantiated once per (ndim, EOS)
-pair in its own translation unit (csrc/stage_inst.cu) so the objects build in parallel.
+nvcc cross-compiles without a GPU.  The fused stage kernel is instantiated once per (ndim, EOS,
+Riemann flux) triple in its own translation unit (csrc/stage_inst.cu) so the objects build in parallel.
 """
 import os
 import subprocess
@@ -33,8 +33,12 @@ def _nvcc():
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, debug_asserts: bool = False) -> str:
+    """debug_asserts: compile with -DDG_DEBUG_ASSERTS (every shared-memory slot index and halo offset of
+    the fused kernel is bounds-checked and a failed check traps): the stand-in for compute-sanitizer,
+    which is closed on this GPU pool.  Always rebuilds; rebuild with force=True afterwards."""
     deps = _sources()
+    force = force or debug_asserts
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in deps)):
         return LIB
@@ -42,14 +46,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
     jobs = [([nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, "dgrhd.cu"), "-o",
               os.path.join(OBJ, "dgrhd.o")], os.path.join(OBJ, "dgrhd.o"))]
-    for nd in (1, 2, 3):
+    for nd in (3, 2, 1):                                     # the slowest translation units first
         for eos in (0, 1):
-            o = os.path.join(OBJ, f"stage_{nd}_{eos}.o")
-            jobs.append(([nvcc, *NVCC_FLAGS, f"-DDG_INST_ND={nd}", f"-DDG_INST_EOS={eos}", "-c",
-                          os.path.join(CSRC, "stage_inst.cu"), "-o", o], o))
-    extra = os.environ.get("DGRHD_NVCC_EXTRA", "").split()      # kernel-tuning experiments only
-    for j in jobs:
-        j[0][1:1] = extra
+            for rs in (0, 1):                                    # HLL, HLLC
+                o = os.path.join(OBJ, f"stage_{nd}_{eos}{rs}.o")
+                jobs.append(([nvcc, *NVCC_FLAGS, f"-DDG_INST_ND={nd}", f"-DDG_INST_EOS={eos}",
+                              f"-DDG_INST_RS={rs}", "-c", os.path.join(CSRC, "stage_inst.cu"), "-o", o], o))
+    if debug_asserts:                                            # bounds / ownership checks in the kernels
+        for j in jobs:
+            j[0].insert(1, "-DDG_DEBUG_ASSERTS")
     if verbose:
         for j in jobs:
             j[0].insert(1, "-Xptxas=-v")
@@ -73,4 +78,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, debug_asserts="--debug-asserts" in sys.argv))

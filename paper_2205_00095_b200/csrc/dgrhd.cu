@@ -15,10 +15,11 @@
 #include "flat_kernels.cuh"
 
 // launchers of the fused stage kernel, one translation unit per (ndim, EOS): stage_inst.cu
-#define DG_DECL(nd, eos)                                                                   \
-  cudaError_t dg_launch_stage_##nd##_##eos(int N, const StageArgs& a, cudaStream_t st); \
-  cudaError_t dg_prepare_stage_##nd##_##eos(int N);
-DG_DECL(1, 0) DG_DECL(1, 1) DG_DECL(2, 0) DG_DECL(2, 1) DG_DECL(3, 0) DG_DECL(3, 1)
+#define DG_DECL(nd, eos, rs)                                                                      \
+  cudaError_t dg_launch_stage_##nd##_##eos##rs(int N, const StageArgs& a, cudaStream_t st); \
+  cudaError_t dg_prepare_stage_##nd##_##eos##rs(int N);
+DG_DECL(1, 0, 0) DG_DECL(1, 1, 0) DG_DECL(2, 0, 0) DG_DECL(2, 1, 0) DG_DECL(3, 0, 0) DG_DECL(3, 1, 0)
+DG_DECL(1, 0, 1) DG_DECL(1, 1, 1) DG_DECL(2, 0, 1) DG_DECL(2, 1, 1) DG_DECL(3, 0, 1) DG_DECL(3, 1, 1)
 #undef DG_DECL
 
 namespace {
@@ -51,8 +52,17 @@ bool valid_cfg(const dgrhd_config* c) {
     if (c->nelem[d] < 1 || c->nelem[d] > 2147483647LL) return false;
     if (d >= c->ndim && c->nelem[d] != 1) return false;
     if (d < c->ndim && !(c->xmax[d] > c->xmin[d])) return false;
-    if (d < c->ndim && c->bc[d] != DGRHD_BC_PERIODIC && c->bc[d] != DGRHD_BC_OUTFLOW) return false;
+    if (d < c->ndim) {                       // bc[d] = lo + 256*hi, hi = 0: same as lo
+      const int lo = c->bc[d] & 255, hi = (c->bc[d] >> 8) & 255;
+      if (c->bc[d] < 0 || c->bc[d] > 0xffff || lo > DGRHD_BC_DIRICHLET || hi > DGRHD_BC_DIRICHLET) return false;
+      if (lo == DGRHD_BC_PERIODIC && hi != 0) return false;     // periodic is both ends
+      for (int sd = 0; sd < 2; ++sd) {
+        const int k = (sd && hi) ? hi : lo;
+        if (k == DGRHD_BC_DIRICHLET && !(c->bc_state[d][sd][0] > 0.0 && c->bc_state[d][sd][4] > 0.0)) return false;
+      }
+    }
   }
+  if (c->riemann != DGRHD_RIEMANN_HLL && c->riemann != DGRHD_RIEMANN_HLLC) return false;
   if (c->order_p < 0 || c->order_p > 4) return false;
   if (c->eos != DGRHD_EOS_IDEAL && c->eos != DGRHD_EOS_TAUB_MATTHEWS) return false;
   if (c->eos == DGRHD_EOS_IDEAL && !(c->gamma_ad > 1.0)) return false;
@@ -129,30 +139,30 @@ static inline bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; 
 // ------------------------------------------------------------------------------------------------
 // kernel dispatch helpers
 // ------------------------------------------------------------------------------------------------
-static cudaError_t launch_stage(dgrhd_ctx* c, const StageArgs& a) {
-  const int key = c->cfg.ndim * 2 + c->cfg.eos;
-  switch (key) {
-    case 2: return dg_launch_stage_1_0(c->N, a, c->stream);
-    case 3: return dg_launch_stage_1_1(c->N, a, c->stream);
-    case 4: return dg_launch_stage_2_0(c->N, a, c->stream);
-    case 5: return dg_launch_stage_2_1(c->N, a, c->stream);
-    case 6: return dg_launch_stage_3_0(c->N, a, c->stream);
-    case 7: return dg_launch_stage_3_1(c->N, a, c->stream);
-  }
+#define DG_CASES(FN, ARGS)                                                         \
+  switch (c->cfg.ndim * 4 + c->cfg.eos * 2 + c->cfg.riemann) {                     \
+    case 4: return dg_##FN##_stage_1_00 ARGS;  case 5: return dg_##FN##_stage_1_01 ARGS;   \
+    case 6: return dg_##FN##_stage_1_10 ARGS;  case 7: return dg_##FN##_stage_1_11 ARGS;   \
+    case 8: return dg_##FN##_stage_2_00 ARGS;  case 9: return dg_##FN##_stage_2_01 ARGS;   \
+    case 10: return dg_##FN##_stage_2_10 ARGS; case 11: return dg_##FN##_stage_2_11 ARGS;  \
+    case 12: return dg_##FN##_stage_3_00 ARGS; case 13: return dg_##FN##_stage_3_01 ARGS;  \
+    case 14: return dg_##FN##_stage_3_10 ARGS; case 15: return dg_##FN##_stage_3_11 ARGS;  \
+  }                                                                                \
   return cudaErrorInvalidValue;
-}
 
-static cudaError_t prepare_stage(dgrhd_ctx* c) {
-  const int key = c->cfg.ndim * 2 + c->cfg.eos;
-  switch (key) {
-    case 2: return dg_prepare_stage_1_0(c->N);
-    case 3: return dg_prepare_stage_1_1(c->N);
-    case 4: return dg_prepare_stage_2_0(c->N);
-    case 5: return dg_prepare_stage_2_1(c->N);
-    case 6: return dg_prepare_stage_3_0(c->N);
-    case 7: return dg_prepare_stage_3_1(c->N);
-  }
-  return cudaErrorInvalidValue;
+static cudaError_t launch_stage(dgrhd_ctx* c, const StageArgs& a) { DG_CASES(launch, (c->N, a, c->stream)) }
+static cudaError_t prepare_stage(dgrhd_ctx* c) { DG_CASES(prepare, (c->N)) }
+#undef DG_CASES
+
+// Eq. 4 on the host, for the Dirichlet ghost states: U = [gamma rho, gamma rho h u, gamma^2 rho h - P],
+// rho h by Eq. 8 (ideal) or Eq. 10 (Taub-Matthews)
+static void host_prim2con(int eos, double G, const double W[5], double U[5]) {
+  const double g2 = 1.0 + W[1] * W[1] + W[2] * W[2] + W[3] * W[3], g = std::sqrt(g2);
+  const double rh = (eos == DGRHD_EOS_IDEAL) ? W[0] + G / (G - 1.0) * W[4]
+                                             : 2.5 * W[4] + 1.5 * std::sqrt(W[4] * W[4] + 4.0 / 9.0 * W[0] * W[0]);
+  U[0] = g * W[0];
+  for (int k = 1; k <= 3; ++k) U[k] = g * rh * W[k];
+  U[4] = g2 * rh - W[4];
 }
 
 // P = P(U) over a state (+ all primitives when W != NULL, + failure counts, + CFL maximum when
@@ -248,12 +258,21 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
       const long long step = es[d] * NN, layer = (long long)(N - 1) * sn;
       a.hoff[d][0] = (int)(-step + layer);                 // minus side: neighbour e-1, node layer N-1
       a.hoff[d][1] = (int)(step - layer);                  // plus side:  neighbour e+1, node layer 0
-      if (d < c->cfg.ndim && c->cfg.bc[d] == DGRHD_BC_PERIODIC) {
+      const int lo = c->cfg.bc[d] & 255, hi = (c->cfg.bc[d] >> 8) & 255;
+      if (d < c->cfg.ndim && lo == DGRHD_BC_PERIODIC) {
         a.hfix[d][0] = (int)(c->cfg.nelem[d] * step);      // e-1 -> e-1+ne
         a.hfix[d][1] = (int)(-c->cfg.nelem[d] * step);
-      } else {                                             // own node: total offset 0
-        a.hfix[d][0] = -a.hoff[d][0];
-        a.hfix[d][1] = -a.hoff[d][1];
+      } else {                                             // own node: total offset 0; the ghost state
+        a.hfix[d][0] = -a.hoff[d][0];                      // is made from it (outflow: as is, wall:
+        a.hfix[d][1] = -a.hoff[d][1];                      // normal momentum reversed) or replaced
+        for (int sd = 0; sd < 2 && d < c->cfg.ndim; ++sd) {
+          const int k = (sd && hi) ? hi : lo;
+          a.bcm[d][sd] = (k == DGRHD_BC_REFLECT || k == DGRHD_BC_DIRICHLET) ? k : 0;
+          if (k == DGRHD_BC_DIRICHLET) {
+            host_prim2con(c->cfg.eos, c->cfg.gamma_ad, c->cfg.bc_state[d][sd], a.bcU[d][sd]);
+            a.bcU[d][sd][5] = c->cfg.bc_state[d][sd][4];
+          }
+        }
       }
     }
   }

@@ -22,8 +22,9 @@
 //      interpolation of :132-134 is a gather, reading R1; periodic wrap / outflow copy, R12) -> records
 //      in shared memory: U, P and r = 1/(E+P) (v = M r; the fraction sigma = num/den of Eq. 22 is
 //      re-derived at the face points);
-//   2. HLL interface flux (Eq. 21-24, reading R9) at every face point of the tile, once each, spread
-//      over the block's threads; volume quadrature (Eq. 17) over the diagonal mass matrix, F_d =
+//   2. interface flux -- HLL (Eq. 21-24, reading R9) or HLLC (ref [34]) -- at every face point of the
+//      tile, once each, spread over the block's threads; ghost states at the mesh boundary: outflow
+//      copy, reflecting wall or fixed (Dirichlet) state; volume quadrature (Eq. 17) over the diagonal mass matrix, F_d =
 //      U v_d + P e_d (Eq. 2) formed on the fly from the records;
 //   3. surface lift (Eq. 18).  MODE_RHS stops here and writes R = L(U).  MODE_STAGE continues:
 //   4. SSP-RK combine  U_out = a U0 + b (U_s + dt R)   (:147-152, reading R10), dt from device memory;
@@ -39,6 +40,10 @@
 #define DG_MODE_STAGE 1
 #define DG_BC_PERIODIC 0
 #define DG_BC_OUTFLOW 1
+#define DG_BC_REFLECT 2
+#define DG_BC_DIRICHLET 3
+#define DG_RS_HLL 0
+#define DG_RS_HLLC 1
 #define DG_NSLOT 32          // counter / CFL-maximum slots (spread same-address atomics), 128 B apart
 #define DG_SLOT_STRIDE 16    // in 8-byte words
 
@@ -132,6 +137,9 @@ struct StageArgs {
   double wsum;            // sum of the tensor weights
   int mode;               // DG_MODE_RHS / DG_MODE_STAGE
   int hoff[3][2], hfix[3][2];   // halo: global-index offset of the facing node (minus, plus side)
+  int bcm[3][2];          // at a mesh boundary [axis][end]: 0 ghost = halo value as loaded (periodic wrap /
+                          // outflow copy), DG_BC_REFLECT normal momentum reversed, DG_BC_DIRICHLET fixed state
+  double bcU[3][2][6];    // Dirichlet ghost state: U (Eq. 4 of the given primitives) and P
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -341,6 +349,62 @@ DG_INL void dg_hll_point(const double UL[5], double vL, double PL, double numL, 
   for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
 }
 
+// HLLC flux ("HLL and HLLC variants ... Mignone and Bodo [34]"; formulas only cited)
+// from the same inputs: lambda_L, lambda_R of Eq. 23-24; HLL state and flux U^hll, F^hll; the contact
+// speed lambda* = minus-sign root of  F_E^hll l^2 - (E^hll + F_m^hll) l + m^hll = 0  (m: momentum
+// normal to the face), written as 2c / (-b + sqrt(b^2 - 4ac)), which stays finite as F_E^hll -> 0;
+// p* = -F_E^hll l* + F_m^hll; the star state of the side the contact has not passed,
+//   D* = D (lK - v)/(lK - l*), m_t* = m_t (lK - v)/(lK - l*), m* = (m (lK - v) + p* - p)/(lK - l*),
+//   E* = (E (lK - v) + p* l* - p v)/(lK - l*),  and  F = F_K + lK (U*_K - U_K).
+template <int D>
+DG_INL void dg_hllc_point(const double UL[5], double vL, double PL, double numL, double denL,
+                          const double UR[5], double vR, double PR, double numR, double denR,
+                          double* pF, int fstride) {
+  double nmL, npL, dL, nmR, npR, dR;
+  dg_speeds_frac(vL, numL, denL, nmL, npL, dL);
+  dg_speeds_frac(vR, numR, denR, nmR, npR, dR);
+  const double rdL = dg_rcp(dL), rdR = dg_rcp(dR);
+  const double lL = fmin(nmL * rdL, nmR * rdR), lR = fmax(npL * rdL, npR * rdR);   // Eq. 23-24
+  constexpr int m = 1 + D;
+  double FL[5], FR[5];
+#pragma unroll
+  for (int v = 0; v < 4; ++v) { FL[v] = UL[v] * vL; FR[v] = UR[v] * vR; }
+  FL[m] += PL; FR[m] += PR;
+  FL[4] = UL[m]; FR[4] = UR[m];                                     // (E + P) v_n = M_n
+  double f[5];
+  if (lL >= 0.0) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) f[v] = FL[v];
+  } else if (lR <= 0.0) {
+#pragma unroll
+    for (int v = 0; v < 5; ++v) f[v] = FR[v];
+  } else {
+    const double inv = dg_rcp(lR - lL);
+    const double Um = (lR * UR[m] - lL * UL[m] + FL[m] - FR[m]) * inv;
+    const double Ue = (lR * UR[4] - lL * UL[4] + FL[4] - FR[4]) * inv;
+    const double Fm = (lR * FL[m] - lL * FR[m] + lL * lR * (UR[m] - UL[m])) * inv;
+    const double Fe = (lR * FL[4] - lL * FR[4] + lL * lR * (UR[4] - UL[4])) * inv;
+    const double b = -(Ue + Fm);
+    const double disc = dg_sqrt(fmax(fma(b, b, -4.0 * Fe * Um), 0.0));
+    const double ls = 2.0 * Um * dg_rcp(disc - b);
+    const double ps = fma(-Fe, ls, Fm);
+    const bool left = (ls >= 0.0);
+    const double lK = left ? lL : lR, vK = left ? vL : vR, PK = left ? PL : PR;
+    const double den = dg_rcp(lK - ls);
+    const double w = lK - vK, fac = w * den;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const double Uk = left ? UL[v] : UR[v], Fk = left ? FL[v] : FR[v];
+      double Us = Uk * fac;
+      if (v == m) Us = (Uk * w + ps - PK) * den;
+      if (v == 4) Us = (Uk * w + ps * ls - PK * vK) * den;
+      f[v] = fma(lK, Us - Uk, Fk);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < 5; ++v) pF[v * fstride] = f[v];
+}
+
 // Where the two sides of face point fl of direction D live: slots of the record rows -- a tile node
 // (< NS) or a halo point (>= NS: rows U | P only; r is derived at use, each halo point is used by
 // exactly one face point) -- and where its flux goes: the halo slot of a boundary plane, else the
@@ -377,28 +441,39 @@ DG_INL bool dg_face_sides(int fl, const int teff[3], FaceSides& fs) {
   return true;
 }
 
+// bmode (block-uniform): what stands behind a halo point that lies outside the mesh (StageArgs::bcm)
 template <int ND, int N, int EOS, int D>
-DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, double U[5], double& vn,
-                         double& P, double& num, double& den) {
+DG_INL void dg_load_side(const EosPar& eos, const double* x, bool halo, int bmode, const double* bcU,
+                         double U[5], double& vn, double& P, double& num, double& den) {
   constexpr int S = TileShape<ND, N>::RS;
 #pragma unroll
   for (int v = 0; v < 5; ++v) U[v] = x[v * S];
   P = x[5 * S];
   double r;
-  if (halo) r = dg_rcp(U[4] + P);
-  else r = x[6 * S];
+  if (halo) {
+    if (bmode == DG_BC_REFLECT) U[1 + D] = -U[1 + D];               // wall
+    if (bmode == DG_BC_DIRICHLET) {                                 // fixed state
+#pragma unroll
+      for (int v = 0; v < 5; ++v) U[v] = bcU[v];
+      P = bcU[5];
+    }
+    r = dg_rcp(U[4] + P);
+  } else {
+    r = x[6 * S];
+  }
   vn = U[1 + D] * r;
   dg_sigma_r<EOS>(eos, U, P, r, num, den);
 }
 
-template <int ND, int N, int EOS, int D>
-DG_INL void dg_face_point(const EosPar& eos, double* sm, int fl, const int teff[3]) {
+template <int ND, int N, int EOS, int RSOL, int D>
+DG_INL void dg_face_point(const StageArgs& a, double* sm, int fl, const int teff[3], int bm0, int bm1) {
   FaceSides fs;
   if (!dg_face_sides<ND, N, D>(fl, teff, fs)) return;
   double UL[5], UR[5], vL, vR, PL, PR, numL, denL, numR, denR;
-  dg_load_side<ND, N, EOS, D>(eos, sm + fs.sl, fs.hl, UL, vL, PL, numL, denL);
-  dg_load_side<ND, N, EOS, D>(eos, sm + fs.sr, fs.hr, UR, vR, PR, numR, denR);
-  dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, sm + fs.of, fs.fstride);
+  dg_load_side<ND, N, EOS, D>(a.eos, sm + fs.sl, fs.hl, bm0, a.bcU[D][0], UL, vL, PL, numL, denL);
+  dg_load_side<ND, N, EOS, D>(a.eos, sm + fs.sr, fs.hr, bm1, a.bcU[D][1], UR, vR, PR, numR, denR);
+  if (RSOL == DG_RS_HLLC) dg_hllc_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, sm + fs.of, fs.fstride);
+  else dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, sm + fs.of, fs.fstride);
 }
 
 // Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
@@ -497,7 +572,7 @@ DG_INL void dg_lift_seg(const double* sm, int id, int lcD, int teffD, int fp0, d
   }
 }
 
-template <int ND, int N, int EOS>
+template <int ND, int N, int EOS, int RSOL>
 __global__ void __launch_bounds__(TileShape<ND, N>::NT, TileShape<ND, N>::MINB)
 dg_stage_kernel(const __grid_constant__ StageArgs a) {
   using TS = TileShape<ND, N>;
@@ -646,10 +721,18 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   __syncthreads();
 
   // 2. interface flux at every face point of the tile, once each, spread over all threads
+  int bm[3][2];                                     // ghost-state rule where the tile touches the mesh boundary
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    bm[d][0] = (org[d] == 0) ? a.bcm[d][0] : 0;
+    bm[d][1] = (org[d] + teff[d] == a.ne[d]) ? a.bcm[d][1] : 0;
+  }
   for (int f = t; f < TS::NFACE; f += NT) {
-    if (ND == 1 || f < TS::FOFF(1)) dg_face_point<ND, N, EOS, 0>(a.eos, sm, f, teff);
-    else if (ND == 2 || f < TS::FOFF(2)) dg_face_point<ND, N, EOS, (ND > 1 ? 1 : 0)>(a.eos, sm, f - TS::FOFF(1), teff);
-    else dg_face_point<ND, N, EOS, (ND > 2 ? 2 : 0)>(a.eos, sm, f - TS::FOFF(2), teff);
+    if (ND == 1 || f < TS::FOFF(1)) dg_face_point<ND, N, EOS, RSOL, 0>(a, sm, f, teff, bm[0][0], bm[0][1]);
+    else if (ND == 2 || f < TS::FOFF(2))
+      dg_face_point<ND, N, EOS, RSOL, (ND > 1 ? 1 : 0)>(a, sm, f - TS::FOFF(1), teff, bm[ND > 1 ? 1 : 0][0], bm[ND > 1 ? 1 : 0][1]);
+    else
+      dg_face_point<ND, N, EOS, RSOL, (ND > 2 ? 2 : 0)>(a, sm, f - TS::FOFF(2), teff, bm[ND > 2 ? 2 : 0][0], bm[ND > 2 ? 2 : 0][1]);
   }
   //    volume quadrature: reads the records only, so it needs no barrier here
   if (active && N > 1) {

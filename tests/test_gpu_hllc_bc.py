@@ -1,0 +1,105 @@
+"""SURVEY.md 8(f) rows built in round 2, CUDA path against the oracle:
+  f1  HLLC interface flux (PAPER.md:126, :161 ref [34]): residual parity at 1e-11 on the RHS_CASES meshes;
+  f4  Dirichlet and reflecting boundaries, per axis end, and the paper's five 1D
+      Riemann problems (Eq. 85-89) with HLLC and the physicality operator.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_2205_00095_b200 import inputs as I
+
+from _util import B, gcfg, mesh, ocfg, relmax, smooth_prims, to_dev
+from test_gpu_parity import RHS_CASES
+
+pytestmark = pytest.mark.gpu
+
+
+def rhs_both(d, U):
+    Ro, _ = O.rhs(ocfg(d), U)
+    ctx = B().Context(gcfg(d))
+    Rg = ctx.dgrhd_rhs(to_dev(U)).cpu().numpy()
+    assert ctx.dgrhd_get_counters()["n_c2p_fail"] == 0 and np.isfinite(Rg).all()
+    err = relmax(Rg, Ro)
+    active = np.max(np.abs(Ro), axis=1) > 1e-9
+    return err[active].max(), np.max(np.abs(Rg - Ro)[~active], initial=0.0)
+
+
+@pytest.mark.parametrize("nd,nelem,p,eos,G,bc", RHS_CASES)
+def test_hllc_rhs_matches_oracle(nd, nelem, p, eos, G, bc):
+    d = mesh(nd, nelem, p, eos, G, bc, riemann=I.RIEMANN_HLLC)
+    W = smooth_prims(d, seed=nd * 10 + p)
+    e1, e0 = rhs_both(d, O.prim2con_batch(eos, G, W))
+    assert e1 <= 1e-11 and e0 <= 1e-11
+
+
+def test_hllc_takes_every_branch_on_jumps_and_supersonic_faces():
+    """Config 1's jumps over several seeds (star states on both sides of the contact) and flows faster
+    than sound in both directions (the two upwind branches)."""
+    for seed in range(6):
+        d, W = I.riemann1d(seed)
+        d = dict(d, riemann=I.RIEMANN_HLLC)
+        e1, _ = rhs_both(d, O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy()))
+        assert e1 <= 1e-11, (seed, e1)
+    d = mesh(1, [40], 2, 0, 5 / 3, [1], riemann=I.RIEMANN_HLLC)
+    W = smooth_prims(d, 3, amp=0.1)
+    for sgn in (+1.0, -1.0):
+        Wb = W.copy()
+        Wb[1] = sgn * 3.0 + 0.1 * W[1]
+        e1, _ = rhs_both(d, O.prim2con_batch(0, 5 / 3, Wb))
+        assert e1 <= 1e-11
+
+
+GHOST = {(0, 0): [2.0, 0.3, -0.1, 0.05, 1.5], (0, 1): [0.4, -0.2, 0.2, 0.0, 0.3],
+         (1, 0): [1.0, 0.0, 0.4, 0.0, 1.0], (1, 1): [0.7, 0.1, -0.3, 0.2, 0.8],
+         (2, 0): [1.5, 0.0, 0.0, -0.2, 0.5], (2, 1): [0.9, 0.2, 0.1, 0.3, 2.0]}
+BC_CASES = [
+    (1, [67], 2, 0, 5 / 3, [(I.BC_DIRICHLET, I.BC_REFLECT)]),
+    (1, [5], 3, 1, 0.0, [(I.BC_REFLECT, I.BC_DIRICHLET)]),
+    (1, [1], 2, 0, 5 / 3, [I.BC_DIRICHLET]),
+    (2, [21, 10], 2, 1, 0.0, [I.BC_DIRICHLET, (I.BC_OUTFLOW, I.BC_REFLECT)]),
+    (2, [9, 7], 3, 0, 5 / 3, [I.BC_PERIODIC, I.BC_REFLECT]),
+    (2, [11, 5], 1, 0, 4 / 3, [(I.BC_REFLECT, I.BC_OUTFLOW), I.BC_DIRICHLET]),
+    (3, [5, 3, 3], 3, 0, 5 / 3, [I.BC_REFLECT, I.BC_DIRICHLET, (I.BC_DIRICHLET, I.BC_OUTFLOW)]),
+    (3, [6, 5, 3], 2, 1, 0.0, [I.BC_DIRICHLET, I.BC_PERIODIC, I.BC_REFLECT]),
+    (3, [3, 2, 2], 4, 0, 5 / 3, [(I.BC_OUTFLOW, I.BC_DIRICHLET), I.BC_REFLECT, I.BC_PERIODIC]),
+]
+
+
+@pytest.mark.parametrize("riemann", [I.RIEMANN_HLL, I.RIEMANN_HLLC])
+@pytest.mark.parametrize("nd,nelem,p,eos,G,bc", BC_CASES)
+def test_dirichlet_and_reflecting_boundaries_match_oracle(nd, nelem, p, eos, G, bc, riemann):
+    d = mesh(nd, nelem, p, eos, G, bc, riemann=riemann, bc_state={k: v for k, v in GHOST.items() if k[0] < nd})
+    W = smooth_prims(d, seed=31 + nd + p)
+    e1, e0 = rhs_both(d, O.prim2con_batch(eos, G, W))
+    assert e1 <= 1e-11 and e0 <= 1e-11
+
+
+def test_bad_boundary_configurations_are_rejected():
+    b = B()
+    d = mesh(1, [8], 2, 0, 5 / 3, [(I.BC_PERIODIC, I.BC_OUTFLOW)])                 # periodic at one end only
+    assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
+    d = mesh(1, [8], 2, 0, 5 / 3, [I.BC_DIRICHLET])                               # no ghost state given
+    assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
+    d = mesh(1, [8], 2, 0, 5 / 3, [1], riemann=7)
+    assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
+def test_paper_riemann_problems_forty_steps_match_oracle(k):
+    """PAPER.md Eq. 85-89 with the paper's boundaries (Dirichlet; test 5: a wall at x = 1), HLLC, p = 2,
+    the physicality operator active (no shock limiter, :551): 40 SSPRK3 steps at CFL 0.2."""
+    d, W, _ = I.paper_riemann1d(k, ne=128, p=2, riemann=I.RIEMANN_HLLC)
+    U = O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy())
+    Uo, to, cnt_o = O.step(ocfg(d), U, -0.2, 40)
+    ctx = B().Context(gcfg(d))
+    ctx.dgrhd_set_state(to_dev(U))
+    tg = ctx.dgrhd_step(-0.2, 40, t=0.0)
+    Ug = ctx.dgrhd_get_state().cpu().numpy()
+    c = ctx.dgrhd_get_counters()
+    err = relmax(Ug, Uo)[[0, 1, 2, 4]]
+    print(f"paper Riemann problem {k}: max-norm rel. diff {err.max():.2e}, activations {cnt_o[0]} / {c['n_flagged']}")
+    assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to
+    assert c["n_bad_mean"] == cnt_o[1] == 0 and c["n_c2p_fail"] == cnt_o[2] == 0
+    assert err.max() <= 1e-8
+    assert abs(c["n_flagged"] - cnt_o[0]) <= max(2, cnt_o[0] // 50)

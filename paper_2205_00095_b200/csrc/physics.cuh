@@ -158,13 +158,14 @@ DG_INL bool dg_admissible(const double U[5], double one_minus_eps) {
   m2 = __dadd_rn(m2, __dmul_rn(U[2], U[2]));
   m2 = __dadd_rn(m2, __dmul_rn(U[3], U[3]));
   const double Es = __dmul_rn(one_minus_eps, U[4]);
-  if (!(U[0] > 0.0) || !(Es > 0.0)) return false;
   // The decision Es > sqrt(m2) is taken without the square root wherever Es^2 and m2 differ by
-  // more than 1e-12 relative (>> the 2-ulp rounding of Es*Es); only marginal states pay for the
-  // correctly rounded sqrt, so the result is identical to the reference expression in every case.
+  // more than 1e-12 relative (>> the 2-ulp rounding of Es*Es) and Es^2 is safely normal: one test for
+  // the common, clearly admissible case; only marginal or inadmissible states take the exact path, so
+  // the result is identical to the reference expression in every case.
   const double t = __dmul_rn(Es, Es);
+  if ((U[0] > 0.0) & (Es > 0.0) & (t > __dmul_rn(m2, 1.0 + 1e-12)) & (t > 1e-280) & (t < 1e300)) return true;
+  if (!(U[0] > 0.0) || !(Es > 0.0)) return false;
   if (!(t > 1e-280 && t < 1e300)) return Es > __dsqrt_rn(m2);   // outside the safely normal range
-  if (t > __dmul_rn(m2, 1.0 + 1e-12)) return true;
   if (!(t >= __dmul_rn(m2, 1.0 - 1e-12))) return false;
   return Es > __dsqrt_rn(m2);
 }
@@ -396,10 +397,11 @@ DG_INL void dg_con2prim_n(const EosPar& e, const double (*U)[5], double (*W)[5],
   }
 #pragma unroll
   for (int s = 0; s < NS; ++s) {
-    // an inadmissible state is replaced by a harmless one for the solver; its outputs are NaN
-    D[s] = adm[s] ? U[s][0] : 1.0;
-    E[s] = adm[s] ? U[s][4] : 2.0;
-    Mabs[s] = adm[s] ? dg_sqrt_p(fma(U[s][1], U[s][1], fma(U[s][2], U[s][2], U[s][3] * U[s][3]))) : 0.0;
+    // (an inadmissible state goes through the solver too -- every loop is bounded and nothing traps --
+    // and its outputs are replaced by NaN below)
+    D[s] = U[s][0];
+    E[s] = U[s][4];
+    Mabs[s] = dg_sqrt_p(fma(U[s][1], U[s][1], fma(U[s][2], U[s][2], U[s][3] * U[s][3])));
   }
   if (EOS == DG_EOS_IDEAL) {
     double w[NS];

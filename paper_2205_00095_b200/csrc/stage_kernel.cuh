@@ -81,6 +81,18 @@ struct TileShape {
   __host__ __device__ static constexpr int T(int d) { return d == 0 ? TX : (d == 1 ? TY : TZ); }
   __host__ __device__ static constexpr int SE(int d) { return d == 0 ? 1 : (d == 1 ? TX : TX * TY); }
   __host__ __device__ static constexpr int SS(int d) { return d == 0 ? 1 : (d == 1 ? N : PK); }
+  // Slot of the segment h of line (j,k) of tile element le, and of node (i,j,k).  For the 64-node
+  // hexahedron (two 16-byte segments per line) the eight segments of a k-plane are rotated by k
+  // positions: the line loads of the volume terms stay conflict-free, and the face points -- which
+  // read nodes of one parity of i only, at stride-4 addresses in the natural order (4-way bank
+  // conflicts) -- spread over all banks that parity can reach (2-way for x and y faces, none for z).
+  static constexpr bool SWZ = (ND == 3 && N == 4);
+  __host__ __device__ static constexpr int seg_slot(int le, int h, int j, int k) {
+    return SWZ ? le * ES + 16 * k + 2 * ((2 * j + h + k) & 7) : le * ES + h * SEG + N * j + PK * k;
+  }
+  __host__ __device__ static constexpr int node_slot(int le, int i, int j, int k) {
+    return SWZ ? seg_slot(le, i >> 1, j, k) + (i & 1) : le * ES + i + N * j + PK * k;
+  }
   __host__ __device__ static constexpr int FP(int d) { return NE / T(d) * NF1; }   // points per face plane
   __host__ __device__ static constexpr int HOFF(int d) { return d <= 0 ? 0 : HOFF(d - 1) + 2 * FP(d - 1); }
   __host__ __device__ static constexpr int FOFF(int d) {
@@ -425,13 +437,16 @@ DG_INL bool dg_face_sides(int fl, const int teff[3], FaceSides& fs) {
   const int la = te % TS::T(A), lb = te / TS::T(A);
   const int ca = tn % N, cb = tn / N;
   if (p > teff[D] || la >= teff[A] || lb >= teff[B]) return false;
-  const int tnode = ca * TS::SS(A) + cb * TS::SS(B);
   const int telem = la * TS::SE(A) + lb * TS::SE(B);
+  // node coordinates of the two sides: the transverse ones are (ca, cb); along D the left side is the
+  // last node of element p-1, the right side the first node of element p
+  int cl[3], cr[3];
+  cl[A] = cr[A] = ca; cl[B] = cr[B] = cb; cl[D] = N - 1; cr[D] = 0;
   fs.hl = (p < 1);
   fs.hr = (p >= teff[D]);
   const int hl_slot = TS::NS + TS::HOFF(D) + fp, hr_slot = hl_slot + FPD;
-  fs.sl = fs.hl ? hl_slot : (telem + (p - 1) * TS::SE(D)) * TS::ES + tnode + (N - 1) * TS::SS(D);
-  fs.sr = fs.hr ? hr_slot : (telem + p * TS::SE(D)) * TS::ES + tnode;
+  fs.sl = fs.hl ? hl_slot : TS::node_slot(telem + (p - 1) * TS::SE(D), cl[0], (ND >= 2) ? cl[1] : 0, (ND >= 3) ? cl[2] : 0);
+  fs.sr = fs.hr ? hr_slot : TS::node_slot(telem + p * TS::SE(D), cr[0], (ND >= 2) ? cr[1] : 0, (ND >= 3) ? cr[2] : 0);
   DG_ASSERT(fs.sl >= 0 && fs.sl < TS::RS && fs.sr >= 0 && fs.sr < TS::RS);
   DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
   const int oi = TS::O_FH + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
@@ -476,17 +491,17 @@ DG_INL void dg_face_point(const StageArgs& a, double* sm, int fl, const int teff
   else dg_hll_point<D>(UL, vL, PL, numL, denL, UR, vR, PR, numR, denR, sm + fs.of, fs.fstride);
 }
 
-// Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread (Eq. 17 over the
-// diagonal mass matrix): for each q the segment at index q along D -- SEG adjacent slots -- is read
-// with vector loads and F_D = [D v_D, M v_D + P e_D, M_D], v_D = M_D r, is formed on the fly.
+// Volume term of direction D = 1 (y) or 2 (z) for the SEG nodes of this thread, segment h of line (j,k)
+// of tile element le (Eq. 17 over the diagonal mass matrix): for each q the segment at index q along D
+// -- SEG adjacent slots -- is read with vector loads and F_D = [D v_D, M v_D + P e_D, M_D], v_D = M_D r, is formed on the fly.
 // dh: (2/h_D) Dhat[id][q] of this thread's index id along D.
 template <int ND, int N, int D>
-DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double (*R)[5]) {
+DG_INL void dg_volume_seg(const double* X, const double* dh, int le, int h, int j, int k, double (*R)[5]) {
   using TS = TileShape<ND, N>;
   constexpr int S = TS::RS, SEG = TS::SEG;
 #pragma unroll
   for (int q = 0; q < N; ++q) {
-    const double* x = X + s_line0 + q * TS::SS(D);
+    const double* x = X + ((D == 1) ? TS::seg_slot(le, h, q, k) : TS::seg_slot(le, h, j, q));
     const double c = dh[q];
     double u[4][SEG], Pq[SEG], rq[SEG];
 #pragma unroll
@@ -508,14 +523,18 @@ DG_INL void dg_volume_seg(const double* X, const double* dh, int s_line0, double
 // Volume term of direction x for a thread that owns only a segment of its line: the whole line's
 // records (N adjacent slots) are read once; dh: rows (2/h_x) Dhat[i0+m][.] of the thread's nodes.
 template <int ND, int N>
-DG_INL void dg_volume_x_seg(const double* X, const double* dh, int s_line, double (*R)[5]) {
+DG_INL void dg_volume_x_seg(const double* X, const double* dh, int le, int j, int k, double (*R)[5]) {
   using TS = TileShape<ND, N>;
-  constexpr int S = TS::RS, SEG = TS::SEG;
+  constexpr int S = TS::RS, SEG = TS::SEG, NSEG = TS::NSEG;
   double u[4][N], Pq[N], rq[N], c[SEG][N];
 #pragma unroll
-  for (int v = 0; v < 4; ++v) dg_ld_line<N>(X + s_line + v * S, u[v]);
-  dg_ld_line<N>(X + s_line + 5 * S, Pq);
-  dg_ld_line<N>(X + s_line + 6 * S, rq);
+  for (int g = 0; g < NSEG; ++g) {
+    const double* x = X + TS::seg_slot(le, g, j, k);
+#pragma unroll
+    for (int v = 0; v < 4; ++v) dg_ld_line<SEG>(x + v * S, u[v] + g * SEG);
+    dg_ld_line<SEG>(x + 5 * S, Pq + g * SEG);
+    dg_ld_line<SEG>(x + 6 * S, rq + g * SEG);
+  }
 #pragma unroll
   for (int m = 0; m < SEG; ++m) dg_ld_line<N>(dh + m * N, c[m]);
 #pragma unroll
@@ -597,8 +616,7 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
   const int lc[3] = {le % TS::TX, (le / TS::TX) % TS::TY, le / (TS::TX * TS::TY)};
   const bool active = (ew < TS::EPW) && (le < TS::NE) && lc[0] < teff[0] && lc[1] < teff[1] && lc[2] < teff[2];
-  const int sl0 = le * TS::ES + N * j + TS::PK * k;                  // slot of node i = 0 of the line
-  const int s0 = sl0 + i0;                                           // slot of the thread's first node
+  const int s0 = TS::seg_slot(le, h, j, k);                          // slot of the thread's first node
   int g0 = 0;                                                        // its global index; ndof < 2^31
   if (active) g0 = ((org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]))) * NN + N * ln + i0;
   const bool xlo = (h == 0), xhi = (h == NSEG - 1);                  // the segment holds node i = 0 / N-1
@@ -736,9 +754,9 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   }
   //    volume quadrature: reads the records only, so it needs no barrier here
   if (active && N > 1) {
-    if constexpr (NSEG > 1) dg_volume_x_seg<ND, N>(X, sDx + i0 * N, sl0, R);
-    if constexpr (ND >= 2) dg_volume_seg<ND, N, 1>(X, sDy + j * N, le * TS::ES + i0 + TS::PK * k, R);
-    if constexpr (ND >= 3) dg_volume_seg<ND, N, 2>(X, sDz + k * N, le * TS::ES + i0 + N * j, R);
+    if constexpr (NSEG > 1) dg_volume_x_seg<ND, N>(X, sDx + i0 * N, le, j, k, R);
+    if constexpr (ND >= 2) dg_volume_seg<ND, N, 1>(X, sDy + j * N, le, h, j, k, R);
+    if constexpr (ND >= 3) dg_volume_seg<ND, N, 2>(X, sDz + k * N, le, h, j, k, R);
   }
   // U0 is requested before the barrier: its (L2) latency overlaps the wait and the lift
   double U0r[5][SEG];

@@ -110,14 +110,12 @@ struct TileShape {
   // r = 1/(E+P): v = M r); a row holds the NS node slots of the tile followed by its NHP halo points
   // (rows 0..5 only), so that a face point addresses either kind of side with the same row stride.
   // Shared-memory bandwidth is a co-equal bound of this kernel, so the records hold only what cannot
-  // be re-derived in a few flops.  The interface flux of a face point on the tile's boundary
-  // overwrites rows 0..4 of the halo point it was computed from (read and written by the same
-  // thread); Fhat holds the interior planes only.
+  // be re-derived in a few flops.
   static constexpr int NREC = 7;
   static constexpr int RS = NS + NHP;                // row stride
   static constexpr int O_X = 0;
-  static constexpr int O_FH = O_X + NREC * RS;       // Fhat  [dir][interior plane][5][FP]
-  static constexpr int O_D = O_FH + (5 * NFACEI + 1) / 2 * 2;  // (2/h_d) Dhat[i][q] for d = x, y, z
+  static constexpr int O_FH = O_X + NREC * RS;       // Fhat  [dir][plane][5][FP]
+  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = x, y, z
   static constexpr int SMEM_BYTES = (O_D + 3 * 26) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
   static constexpr int REG_FLOOR = (SEG <= 1) ? 64 : ((SEG >= 6) ? 240 : 40 * SEG);   // registers per thread to leave
@@ -419,8 +417,8 @@ DG_INL void dg_hllc_point(const double UL[5], double vL, double PL, double numL,
 
 // Where the two sides of face point fl of direction D live: slots of the record rows -- a tile node
 // (< NS) or a halo point (>= NS: rows U | P only; r is derived at use, each halo point is used by
-// exactly one face point) -- and where its flux goes: the halo slot of a boundary plane, else the
-// interior-plane array.  Returns false for face points outside a ragged tile.
+// exactly one face point) -- and where its flux goes.  Returns false for face points outside a
+// ragged tile.
 struct FaceSides {
   int sl, sr;        // record slots of the left / right side
   bool hl, hr;       // side is a halo point
@@ -449,10 +447,9 @@ DG_INL bool dg_face_sides(int fl, const int teff[3], FaceSides& fs) {
   fs.sr = fs.hr ? hr_slot : TS::node_slot(telem + p * TS::SE(D), cr[0], (ND >= 2) ? cr[1] : 0, (ND >= 3) ? cr[2] : 0);
   DG_ASSERT(fs.sl >= 0 && fs.sl < TS::RS && fs.sr >= 0 && fs.sr < TS::RS);
   DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
-  const int oi = TS::O_FH + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp;
-  fs.of = fs.hl ? hl_slot : (fs.hr ? hr_slot : oi);
-  fs.fstride = (fs.hl || fs.hr) ? TS::RS : FPD;
-  DG_ASSERT(fs.hl || fs.hr || (p >= 1 && 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACEI));
+  fs.of = TS::O_FH + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
+  fs.fstride = FPD;
+  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
   return true;
 }
 
@@ -551,17 +548,13 @@ DG_INL void dg_volume_x_seg(const double* X, const double* dh, int le, int j, in
   }
 }
 
-// Flux of face plane p of direction D at face point fp: in the halo slot for the tile's boundary
-// planes (p == 0, p == teffD), else in the interior-plane array.  Returns the offset from the start
-// of shared memory; stride: the distance between the flux components.
+// Flux of face plane p of direction D at face point fp: offset from the start of shared memory;
+// stride: the distance between the flux components.
 template <int ND, int N, int D>
 DG_INL int dg_flux_off(int p, int teffD, int fp, int& stride) {
   using TS = TileShape<ND, N>;
-  constexpr int FPD = TS::FP(D);
-  const bool lo = (p == 0), hi = (p == teffD);
-  stride = (lo || hi) ? TS::RS : FPD;
-  const int oh = TS::NS + TS::HOFF(D) + fp;
-  return lo ? oh : (hi ? oh + FPD : TS::O_FH + 5 * TS::FOFFI(D) + (p - 1) * 5 * FPD + fp);
+  stride = TS::FP(D);
+  return TS::O_FH + 5 * TS::FOFF(D) + p * 5 * TS::FP(D) + fp;
 }
 
 // Lift of the interface flux of direction D = 1 or 2 onto the thread's nodes (Eq. 18): the segment

@@ -142,6 +142,16 @@ int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[6], int reset);
 int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const double* U_dev, double* W_dev,
                          int* status_dev, void* cuda_stream);
 
+/* The paper's comparison variants of the recovery ("four algorithms in all", the study of
+ * section 3.3, :405-449), same layout and status codes as dgrhd_con2prim_batch:
+ *   DGRHD_C2P_DEFAULT    the hot-path solvers (ideal: Newton on Eq. 59; Taub-Matthews: analytic cubic)
+ *   DGRHD_C2P_ALTERNATE  ideal EOS by the analytic quartic in beta (Eq. 39-57, after Ryu et al.);
+ *                        Taub-Matthews by Brent's method on Eq. 61, bracket gamma in [1,200] expanded
+ *                        if needed, at most max_iter iterations (>= 1; the paper's Fig. 2 uses 25, 50) */
+enum { DGRHD_C2P_DEFAULT = 0, DGRHD_C2P_ALTERNATE = 1 };
+int dgrhd_con2prim_batch_variant(int eos, int variant, double gamma_ad, int64_t n, const double* U_dev,
+                                 double* W_dev, int* status_dev, int max_iter, void* cuda_stream);
+
 /* Number of Taub-Matthews recoveries of the context-free batch calls (all streams of the current
  * device) that took the double-precision fallback since the last reset (see n_tm_fallback above).
  * Synchronises cuda_stream. */

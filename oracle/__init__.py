@@ -166,6 +166,24 @@ def con2prim_batch(eos, G, U):
     return W, st
 
 
+def con2prim_variant(eos, variant, G, U, max_iter=50):
+    """variant 1: ideal EOS analytic quartic / Taub-Matthews Brent.  Returns (W, status, iterations)."""
+    W = np.zeros(5)
+    nit = C.c_int()
+    st = lib().orc_con2prim_variant(C.c_int(eos), C.c_int(variant), C.c_double(G), _p(_v5(U)), _p(W),
+                                    C.c_int(max_iter), C.byref(nit))
+    return W, int(st), nit.value
+
+
+def con2prim_variant_batch(eos, variant, G, U, max_iter=50):
+    U = np.ascontiguousarray(U, dtype=np.float64)
+    W = np.empty_like(U)
+    st = np.zeros(U.shape[1], dtype=np.int32)
+    lib().orc_con2prim_variant_batch(C.c_int(eos), C.c_int(variant), C.c_double(G), C.c_int64(U.shape[1]),
+                                     _p(U), _p(W), st.ctypes.data_as(C.POINTER(C.c_int)), C.c_int(max_iter))
+    return W, st
+
+
 def admissible(U, eps=0.0):
     return bool(lib().orc_admissible(_p(_v5(U)), C.c_double(eps)))
 

@@ -337,6 +337,153 @@ static int con2prim_tm(const double U[5], double Wp[5]) {
   return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * The paper's two comparison variants of con2prim ("four algorithms in all"; the
+ * section 3.3 study, :405-449).  SURVEY.md 8(f).3.
+ *
+ * (1) Ideal EOS, ANALYTIC route (:269-323, Eq. 39-57, after Ryu et al. [15]): the physical root of
+ *   beta^4 + a3 beta^3 + a2 beta^2 + a1 beta + a0 = 0     (Eq. 39; the beta^3 term is missing in the
+ *   extracted text -- with it the true beta is a root to 1e-50, reading R17)
+ * with a0..a3 of Eq. 40-43, by Ferrari's factorisation: x = real root of the resolvent cubic
+ * x^3 + i1 x^2 + i2 x + i3 (Eq. 51-53; Eq. 48 reads 9 i1 i2, Eq. 49 uses i1^2 = a2^2), trigonometric
+ * form for T < 0 -- 2 sqrt(-S) cos(acos(R / sqrt(-S^3)) / 3) - i1/3, which is what the garbled
+ * Eq. 47 encodes ((R^2 - T)^(1/6) = sqrt(-S)) -- else Cardano; B, C of Eq. 45-46; beta by Eq. 44;
+ * finishing Eq. 55-57.
+ * ------------------------------------------------------------------------------------------ */
+static int con2prim_ideal_analytic(double G, const double U[5], double W[5]) {
+  double D = U[0], E = U[4];
+  double Mabs = sqrt(U[1] * U[1] + U[2] * U[2] + U[3] * U[3]);
+  double xi = Mabs / D, eta = E / D;                                   /* Eq. 38 */
+  double beta;
+  if (xi == 0.0) {
+    beta = 0.0;
+  } else {
+    double g1 = G - 1.0, den = g1 * g1 * (xi * xi + 1.0);
+    double a3 = -2.0 * G * g1 * xi * eta / den;                        /* Eq. 40 */
+    double a2 = (G * G * eta * eta + 2.0 * g1 * xi * xi - g1 * g1) / den;   /* Eq. 41 */
+    double a1 = -2.0 * G * xi * eta / den;                             /* Eq. 42 */
+    double a0 = xi * xi / den;                                         /* Eq. 43 */
+    double i1 = -a2;                                                   /* Eq. 51 */
+    double i2 = a3 * a1 - 4.0 * a0;                                    /* Eq. 52 */
+    double i3 = 4.0 * a2 * a0 - a1 * a1 - a3 * a3 * a0;                /* Eq. 53 */
+    double R = (9.0 * i1 * i2 - 27.0 * i3 - 2.0 * i1 * i1 * i1) / 54.0;   /* Eq. 48 */
+    double S = (3.0 * i2 - i1 * i1) / 9.0;                             /* Eq. 49 */
+    double T = R * R + S * S * S;                                      /* Eq. 50 */
+    double x;
+    if (T < 0.0) {                                                     /* Eq. 47 */
+      double arg = R / sqrt(-(S * S * S));
+      if (arg > 1.0) arg = 1.0;
+      if (arg < -1.0) arg = -1.0;
+      x = 2.0 * sqrt(-S) * cos(acos(arg) / 3.0) - i1 / 3.0;
+    } else {
+      double sT = sqrt(T);
+      x = cbrt(R + sT) + cbrt(R - sT) - i1 / 3.0;
+    }
+    double B = 0.5 * (a3 + sqrt(a3 * a3 - 4.0 * a2 + 4.0 * x));        /* Eq. 45 */
+    double C = 0.5 * (x - sqrt(x * x - 4.0 * a0));                     /* Eq. 46 */
+    beta = 0.5 * (-B + sqrt(B * B - 4.0 * C));                         /* Eq. 44 */
+  }
+  double rho = D * sqrt(1.0 - beta * beta);                            /* Eq. 55 */
+  double g = 1.0 / sqrt(1.0 - beta * beta);
+  double nx = 0.0, ny = 0.0, nz = 0.0;
+  if (Mabs > 0.0) { nx = U[1] / Mabs; ny = U[2] / Mabs; nz = U[3] / Mabs; }
+  W[0] = rho;
+  W[1] = g * beta * nx;                                                /* u = gamma v, v = beta M/|M| (Eq. 56) */
+  W[2] = g * beta * ny;
+  W[3] = g * beta * nz;
+  W[4] = (G - 1.0) * (E - beta * Mabs - rho);                          /* Eq. 57 */
+  if (!(beta >= 0.0 && beta < 1.0) || !finite5(W) || !(W[4] > 0.0)) return 2;
+  return 0;
+}
+
+/* (2) Taub-Matthews, ITERATIVE route (:392): Brent's method [36] on the cubic of Eq. 61 in
+ * W = gamma^2 - 1, bracketed by gamma in [1, 200] and re-bracketed upwards (gamma -> 10 gamma) while
+ * the root is not inside; at most max_iter iterations (the paper's Fig. 2 uses 25 and 50), stopped
+ * early when the bracket has shrunk to 4 ulp.  Finishing Eq. 74-75. */
+static double tm_cubic(double W, double c1, double c2, double c3) { return ((W + c1) * W + c2) * W + c3; }
+
+static int con2prim_tm_brent(const double U[5], double Wp[5], int max_iter, int *niter_out) {
+  double D = U[0], E = U[4];
+  double Mabs = sqrt(U[1] * U[1] + U[2] * U[2] + U[3] * U[3]);
+  double xi = Mabs / D, eta = E / D;
+  double x2 = xi * xi, e2 = eta * eta;
+  double dif = (eta - xi) * (eta + xi), den = dif * dif;
+  double sum = e2 + x2, br = 4.0 * sum - (x2 + 1.0);
+  double c1 = (sum * br - 14.0 * x2 * e2) / (2.0 * den);
+  double c2 = (br * br - 57.0 * x2 * e2) / (16.0 * den);
+  double c3 = -9.0 * x2 * e2 / (16.0 * den);
+  double a = 0.0, b = 200.0 * 200.0 - 1.0;
+  double fa = tm_cubic(a, c1, c2, c3), fb = tm_cubic(b, c1, c2, c3);
+  for (int k = 0; k < 40 && fb < 0.0; ++k) { b = 100.0 * (b + 1.0) - 1.0; fb = tm_cubic(b, c1, c2, c3); }
+  int it = 0;
+  double Wv;
+  if (fa == 0.0) Wv = a;
+  else if (!(fa < 0.0 && fb >= 0.0)) Wv = NAN;
+  else {
+    /* Brent's method: a = contrapoint, b = best estimate, c = previous b */
+    double c = a, fc = fa, d = b - a, e = d;
+    for (it = 0; it < max_iter; ++it) {
+      if ((fb > 0.0 && fc > 0.0) || (fb < 0.0 && fc < 0.0)) { c = a; fc = fa; d = b - a; e = d; }
+      if (fabs(fc) < fabs(fb)) { a = b; b = c; c = a; fa = fb; fb = fc; fc = fa; }
+      double tol = 2.0 * 2.220446049250313e-16 * fabs(b), m = 0.5 * (c - b);
+      if (fabs(m) <= tol || fb == 0.0) break;
+      if (fabs(e) >= tol && fabs(fa) > fabs(fb)) {
+        double p, q, s = fb / fa;
+        if (a == c) { p = 2.0 * m * s; q = 1.0 - s; }                   /* secant */
+        else {                                                          /* inverse quadratic */
+          double qq = fa / fc, r = fb / fc;
+          p = s * (2.0 * m * qq * (qq - r) - (b - a) * (r - 1.0));
+          q = (qq - 1.0) * (r - 1.0) * (s - 1.0);
+        }
+        if (p > 0.0) q = -q; else p = -p;
+        if (2.0 * p < fmin(3.0 * m * q - fabs(tol * q), fabs(e * q))) { e = d; d = p / q; }
+        else { d = m; e = m; }
+      } else { d = m; e = m; }
+      a = b; fa = fb;
+      b += (fabs(d) > tol) ? d : (m > 0.0 ? tol : -tol);
+      fb = tm_cubic(b, c1, c2, c3);
+    }
+    Wv = b;
+  }
+  if (niter_out) *niter_out = it;
+  if (Wv < 0.0) Wv = 0.0;
+  double g = sqrt(Wv + 1.0), beta = sqrt(Wv / (Wv + 1.0));             /* Eq. 74 */
+  double rho = D / g;
+  double nx = 0.0, ny = 0.0, nz = 0.0;
+  if (Mabs > 0.0) { nx = U[1] / Mabs; ny = U[2] / Mabs; nz = U[3] / Mabs; }
+  double ug = sqrt(Wv);
+  double X = E - beta * Mabs;
+  Wp[0] = rho; Wp[1] = ug * nx; Wp[2] = ug * ny; Wp[3] = ug * nz;
+  Wp[4] = (X - rho) * (X + rho) / (3.0 * X);                            /* Eq. 75 */
+  if (!finite5(Wp) || !(Wp[4] > 0.0)) return 2;
+  return 0;
+}
+
+/* variant = 0: the hot-path solvers (orc_con2prim); 1: ideal analytic / Taub-Matthews Brent */
+int orc_con2prim_variant(int eos, int variant, double G, const double U[5], double W[5], int max_iter,
+                         int *niter_out) {
+  if (niter_out) *niter_out = 0;
+  if (variant == 0) return orc_con2prim(eos, G, U, W, niter_out);
+  if (!orc_admissible(U, 0.0)) {
+    for (int v = 0; v < 5; ++v) W[v] = NAN;
+    return 1;
+  }
+  if (eos == ORC_EOS_IDEAL) return con2prim_ideal_analytic(G, U, W);
+  return con2prim_tm_brent(U, W, max_iter, niter_out);
+}
+
+void orc_con2prim_variant_batch(int eos, int variant, double G, int64_t n, const double *U, double *W,
+                                int *status, int max_iter) {
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < n; ++i) {
+    double u[5], w[5];
+    for (int v = 0; v < 5; ++v) u[v] = U[v * n + i];
+    int st = orc_con2prim_variant(eos, variant, G, u, w, max_iter, 0);
+    for (int v = 0; v < 5; ++v) W[v * n + i] = w[v];
+    if (status) status[i] = st;
+  }
+}
+
 int orc_con2prim(int eos, double G, const double U[5], double W[5], int *niter_out) {
   if (niter_out) *niter_out = 0;
   if (!orc_admissible(U, 0.0)) {            /* Eq. 25: the solvers are specified on admissible U */

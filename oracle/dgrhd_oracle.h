@@ -61,6 +61,13 @@ int    orc_con2prim(int eos, double G, const double U[5], double W[5], int *nite
 /* ideal EOS Newton with a caller-fixed iteration count and no stopping test (Fig. 2 protocol) */
 int    orc_con2prim_ideal_fixed(double G, const double U[5], double W[5], int niter);
 
+/* the paper's comparison variants (section 3.3): variant 0 = orc_con2prim; 1 = ideal EOS by the analytic
+ * quartic (Eq. 39-57) / Taub-Matthews by Brent's method on Eq. 61 with at most max_iter iterations */
+int    orc_con2prim_variant(int eos, int variant, double G, const double U[5], double W[5], int max_iter,
+                            int *niter_out);
+void   orc_con2prim_variant_batch(int eos, int variant, double G, int64_t n, const double *U, double *W,
+                                  int *status, int max_iter);
+
 void   orc_prim2con_batch(int eos, double G, int64_t n, const double *W, double *U);
 void   orc_con2prim_batch(int eos, double G, int64_t n, const double *U, double *W, int *status);
 

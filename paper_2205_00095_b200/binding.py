@@ -14,6 +14,7 @@ BC_PERIODIC, BC_OUTFLOW, BC_REFLECT, BC_DIRICHLET = 0, 1, 2, 3
 RIEMANN_HLL, RIEMANN_HLLC = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
 OPT_CUDA_GRAPH = 0
+C2P_DEFAULT, C2P_ALTERNATE = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdgrhd.so")
@@ -66,7 +67,7 @@ _vp, _dp, _i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
 EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_state",
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
-           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64",
+           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64", "dgrhd_con2prim_batch_variant",
            "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
 
 
@@ -93,6 +94,8 @@ def lib():
         L.dgrhd_get_counters.argtypes = [_vp, _i64p, C.c_int]
         L.dgrhd_con2prim_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp, _vp]
         L.dgrhd_tm_fallback_count.argtypes = [_i64p, C.c_int, _vp]
+        L.dgrhd_con2prim_batch_variant.argtypes = [C.c_int, C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp,
+                                                   C.c_int, _vp]
         L.dgrhd_probe_fp64.argtypes = [_vp, _dp, _dp, _vp]
         L.dgrhd_prim2con_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp]
         L.dgrhd_con2prim_batch_host.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp,
@@ -235,6 +238,13 @@ def dgrhd_con2prim_batch(eos, gamma_ad, U, W=None, status=None):
     W = torch.empty_like(U) if W is None else W
     _check(lib().dgrhd_con2prim_batch(eos, gamma_ad, U.shape[1], _ptr(U, 5), _ptr(W, 5),
                                       _ptr(status), _stream()))
+    return W
+
+
+def dgrhd_con2prim_batch_variant(eos, variant, gamma_ad, U, W=None, status=None, max_iter=50):
+    W = torch.empty_like(U) if W is None else W
+    _check(lib().dgrhd_con2prim_batch_variant(eos, variant, gamma_ad, U.shape[1], _ptr(U, 5), _ptr(W, 5),
+                                              _ptr(status), max_iter, _stream()))
     return W
 
 

@@ -634,6 +634,22 @@ extern "C" int dgrhd_con2prim_batch(int eos, double gamma_ad, int64_t n, const d
   return DGRHD_OK;
 }
 
+extern "C" int dgrhd_con2prim_batch_variant(int eos, int variant, double gamma_ad, int64_t n, const double* U_dev,
+                                            double* W_dev, int* status_dev, int max_iter, void* cuda_stream) {
+  if (variant == DGRHD_C2P_DEFAULT) return dgrhd_con2prim_batch(eos, gamma_ad, n, U_dev, W_dev, status_dev, cuda_stream);
+  if (variant != DGRHD_C2P_ALTERNATE) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_variant: unknown variant %d", variant);
+  int r = check_batch("dgrhd_con2prim_batch_variant", eos, gamma_ad, n, U_dev, W_dev);
+  if (r != DGRHD_OK || n == 0) return r;
+  if (max_iter < 1) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_variant: max_iter must be >= 1");
+  const EosPar e = make_eos(eos, gamma_ad);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
+  if (eos == DGRHD_EOS_IDEAL) dg_c2p_variant_kernel<0><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e, max_iter);
+  else dg_c2p_variant_kernel<1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e, max_iter);
+  DG_CUDA(nullptr, cudaGetLastError());
+  return DGRHD_OK;
+}
+
 extern "C" int dgrhd_tm_fallback_count(int64_t* out_host, int reset, void* cuda_stream) {
   if (!out_host) return fail(nullptr, DGRHD_EINVAL, "dgrhd_tm_fallback_count: NULL argument");
   cudaStream_t st = (cudaStream_t)cuda_stream;

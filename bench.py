@@ -193,22 +193,29 @@ def run_reference(a):
 # ------------------------------------------------------------------------------------------------
 # CUDA leg
 # ------------------------------------------------------------------------------------------------
-def time_c2p(b, torch, eos, G, n):
+def time_c2p(b, torch, eos, G, n, variant=0):
     """con2prim states/s on configs[2]'s 2^26-state batch (device-resident), median of 5; also the
-    number of Taub-Matthews fallbacks of one pass."""
+    number of Taub-Matthews fallbacks of one pass.  variant 1: the paper's comparison solvers."""
     from paper_2205_00095_b200 import inputs as I
     W = I.c2p_states(0, n, device="cuda")
     U = b.dgrhd_prim2con_batch(eos, G, W)
     del W
     out = torch.empty_like(U)
+
+    def call():
+        if variant:
+            b.dgrhd_con2prim_batch_variant(eos, variant, G, U, out, max_iter=50)
+        else:
+            b.dgrhd_con2prim_batch(eos, G, U, out)
+
     for _ in range(3):
-        b.dgrhd_con2prim_batch(eos, G, U, out)
+        call()
     b.dgrhd_tm_fallback_count(reset=True)
     ts = []
     for _ in range(5):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        b.dgrhd_con2prim_batch(eos, G, U, out)
+        call()
         e1.record()
         e1.synchronize()
         ts.append(e0.elapsed_time(e1) * 1e-3)
@@ -219,7 +226,12 @@ def time_c2p(b, torch, eos, G, n):
 def c2p_leg(b, torch, n, peak, peak_src):
     ideal, _ = time_c2p(b, torch, 0, 4.0 / 3.0, n)
     tm, nfall = time_c2p(b, torch, 1, 0.0, n)
+    # the paper's section-3.3 comparison on this GPU: its other two algorithms on the same batch
+    ideal_an, _ = time_c2p(b, torch, 0, 4.0 / 3.0, n, variant=1)
+    tm_brent, _ = time_c2p(b, torch, 1, 0.0, n, variant=1)
     return {"unit": "states/s", "n": n, "ideal_gamma_4_3": ideal, "taub_matthews": tm,
+            "comparison_variants": {"ideal_analytic_quartic": ideal_an, "taub_matthews_brent_50_iterations": tm_brent,
+                                    "what": "PAPER.md section 3.3 (:405-449): analytic vs iterative recovery, both EOS"},
             "taub_matthews_fallbacks_per_pass": nfall, "alg_bytes_per_state": 80,
             "roofline_hbm_frac_ideal": ideal * 80 / 1e9 / peak, "roofline_hbm_frac_tm": tm * 80 / 1e9 / peak,
             "peak_gbs": peak, "peak_source": peak_src}

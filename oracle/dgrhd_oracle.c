@@ -697,6 +697,84 @@ void orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Shock limiter of Moe, Rossmanith & Seal ("the Moe limiter from Moe et al.
+ * [23]"; arXiv:1507.03024).  NOT PRINTED IN PAPER.md -- PARITY UNPINNED: this is ref [23]'s algorithm
+ * as restated in DESIGN.md reading R18, applied to the five conserved variables w = U:
+ *   1. per cell i: average wbar_i (tensor GLL weights) and the extrema w_Mi, w_mi over the cell's
+ *      nodes (GLL nodes include the corners and the face points);
+ *   2. bounds from the face neighbours N_i (periodic wrap; no neighbour beyond any other boundary):
+ *        M_i = max(wbar_i + alpha, max_{j in N_i} w_Mj),  m_i = min(wbar_i - alpha, min_{j in N_i} w_mj);
+ *   3. theta_Mi = phi((M_i - wbar_i)/(w_Mi - wbar_i)), theta_mi = phi((m_i - wbar_i)/(w_mi - wbar_i)),
+ *      phi(y) = min(y/1.1, 1)  (ratio taken as +inf when the cell's own extremum equals its mean);
+ *   4. theta_i = min(1, theta_M, theta_m over all variables);
+ *   5. U <- Ubar_i + theta_i (U - Ubar_i)   (cell averages unchanged; a convex blend of admissible
+ *      states, so the physicality operator's result stays admissible).
+ * ------------------------------------------------------------------------------------------ */
+int64_t orc_shock_limiter(const orc_config *c, double *U, double *theta_out) {
+  const int nd = c->ndim, N = c->order_p + 1, nn = ipow(N, nd);
+  const int64_t nx = c->nelem[0], ny = nd > 1 ? c->nelem[1] : 1, nz = nd > 2 ? c->nelem[2] : 1;
+  const int64_t ne = nx * ny * nz, ndof = ne * nn;
+  const int64_t nel[3] = {nx, ny, nz};
+  double x[5], w[5], D[25];
+  orc_gll(N, x, w, D);
+  double *st = (double *)malloc(sizeof(double) * 15 * (size_t)ne);      /* mean, max, min per cell */
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    double wsum = 0.0, mean[5] = {0, 0, 0, 0, 0}, mx[5], mn[5];
+    for (int n = 0; n < nn; ++n) {
+      double wn = w[n % N];
+      if (nd > 1) wn *= w[(n / N) % N];
+      if (nd > 2) wn *= w[n / (N * N)];
+      wsum += wn;
+      for (int v = 0; v < 5; ++v) {
+        double u = U[v * ndof + e * nn + n];
+        mean[v] += wn * u;
+        if (n == 0 || u > mx[v]) mx[v] = u;
+        if (n == 0 || u < mn[v]) mn[v] = u;
+      }
+    }
+    for (int v = 0; v < 5; ++v) { st[e * 15 + v] = mean[v] / wsum; st[e * 15 + 5 + v] = mx[v]; st[e * 15 + 10 + v] = mn[v]; }
+  }
+  int64_t nlim = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nlim)
+  for (int64_t e = 0; e < ne; ++e) {
+    int64_t ie[3] = {e % nx, (e / nx) % ny, e / (nx * ny)};
+    double theta = 1.0;
+    for (int v = 0; v < 5; ++v) {
+      double wb = st[e * 15 + v], wM = st[e * 15 + 5 + v], wm = st[e * 15 + 10 + v];
+      double M = wb + c->moe_alpha, m = wb - c->moe_alpha;
+      for (int d = 0; d < nd; ++d)
+        for (int side = 0; side < 2; ++side) {
+          int64_t je[3] = {ie[0], ie[1], ie[2]};
+          je[d] += side ? 1 : -1;
+          if (je[d] < 0 || je[d] >= nel[d]) {
+            if ((c->bc[d] & 255) != ORC_BC_PERIODIC) continue;
+            je[d] = (je[d] + nel[d]) % nel[d];
+          }
+          int64_t en = je[0] + nx * (je[1] + ny * je[2]);
+          if (st[en * 15 + 5 + v] > M) M = st[en * 15 + 5 + v];
+          if (st[en * 15 + 10 + v] < m) m = st[en * 15 + 10 + v];
+        }
+      double tM = (wM - wb > 0.0) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
+      double tm = (wb - wm > 0.0) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
+      if (tM < theta) theta = tM;
+      if (tm < theta) theta = tm;
+    }
+    if (theta_out) theta_out[e] = theta;
+    if (theta < 1.0) {
+      nlim++;
+      for (int n = 0; n < nn; ++n)
+        for (int v = 0; v < 5; ++v) {
+          double ub = st[e * 15 + v];
+          U[v * ndof + e * nn + n] = ub + theta * (U[v * ndof + e * nn + n] - ub);
+        }
+    }
+  }
+  free(st);
+  return nlim;
+}
+
+/* ------------------------------------------------------------------------------------------
  * R11  CFL time step ("adaptive time stepping ... to maintain a certain CFL"):
  *   dt = CFL / max_nodes sum_d (2p+1) max(|lambda-_d|,|lambda+_d|)/h_d
  * ------------------------------------------------------------------------------------------ */
@@ -746,6 +824,7 @@ void orc_step(const orc_config *c, double *U, double dt_in, int nsteps, double *
 #pragma omp parallel for schedule(static)
       for (int64_t i = 0; i < 5 * ndof; ++i) U[i] = A[st] * U0[i] + B[st] * (U[i] + dt * R[i]);
       orc_enforce_physicality(c, U, 0, 0, lim);
+      if (c->shock_limiter) orc_shock_limiter(c, U, 0);                /* reading R18 */
       if (counters) { counters[0] += lim[0]; counters[1] += lim[1]; counters[2] += nf; }
     }
     if (t_inout) *t_inout += dt;

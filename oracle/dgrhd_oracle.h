@@ -37,6 +37,10 @@ typedef struct {
   int     rk_stages;     /* 1,2,3 */
   double  eps_q, delta_s;
   int     riemann;       /* ORC_RIEMANN_*: interface flux */
+  int     shock_limiter; /* 0 none; 1 the limiter of Moe, Rossmanith & Seal (PAPER.md:126, :551 ref [23]),
+                            applied after the physicality operator of every stage.  PARITY UNPINNED: the
+                            paper cites the limiter without printing it (reading R18) */
+  double  moe_alpha;     /* its tolerance alpha(h) >= 0 (ref [23] suggests ~ 500 h^1.5), absolute */
   double  bc_state[3][2][5];   /* Dirichlet ghost primitives [axis][side] = rho, ux, uy, uz, P */
 } orc_config;
 
@@ -80,6 +84,9 @@ int64_t orc_ndof(const orc_config *c);
 void   orc_rhs(const orc_config *c, const double *U, double *R, int64_t *n_c2p_fail);
 void   orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag, double *s,
                                int64_t counters[2]);
+/* The shock limiter of Moe et al. (reading R18), in place; theta[n_e] (may be NULL) receives the
+ * rescaling factor of every cell; returns the number of cells with theta < 1. */
+int64_t orc_shock_limiter(const orc_config *c, double *U, double *theta);
 double orc_cfl_dt(const orc_config *c, const double *U, double cfl);
 /* dt > 0 fixed; dt <= 0: CFL number -dt, recomputed every step.  counters[3] accumulates
  * n_flagged, n_bad_mean, n_c2p_fail over all stages. */

@@ -543,3 +543,57 @@ def test_paper_riemann_problems_stay_admissible_and_conserve_up_to_the_boundary_
     inflow = U[0, 0] * (W[1, 0] / np.sqrt(1 + W[1, 0] ** 2 + W[2, 0] ** 2)) * t     # D v_x at x = 0
     outflow = 0.0 if k == 5 else U[0, -1] * float(W[1, -1] / np.sqrt(1 + W[1, -1] ** 2 + W[2, -1] ** 2)) * t
     assert abs((mass1 - mass0) - (float(inflow) - outflow)) <= 1e-10 * mass0
+
+
+# ------------------------------------------------------------------------------------------------
+# Shock limiter of Moe et al. (PAPER.md:126, :551 ref [23]; reading R18).  The paper does not print it:
+# PARITY UNPINNED.  What can be pinned are the properties any such limiter must have.
+# ------------------------------------------------------------------------------------------------
+def test_moe_limiter_keeps_cell_means_leaves_resolved_data_alone_and_bounds_the_extrema():
+    nd, nel, p = 2, [12, 9], 2
+    N, nn = p + 1, 9
+    d = I._cfg(nd, nel, [0.0, 0.0], [1.0, 1.0], [I.BC_PERIODIC, I.BC_OUTFLOW], p, 0, 5.0 / 3.0)
+    cfg = O.make_config(*[d[k] for k in ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad",
+                                          "rk_stages", "eps_q", "delta_s")], shock_limiter=1, moe_alpha=0.0)
+    W, _, _ = _smooth_field(nd, nel, N, [0.0, 0.0], [1.0, 1.0], seed=12)
+    U = O.prim2con_batch(0, 5.0 / 3.0, W)
+    wn = _node_weights(nd, N)
+    # (a) well-resolved monotone data away from extrema: untouched (theta = 1) in most cells, and with a
+    #     generous tolerance alpha in every cell
+    U1, th, nlim = O.shock_limiter(cfg, U)
+    assert (th == 1.0).mean() > 0.5
+    cfg_a = O.make_config(*[d[k] for k in ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad",
+                                            "rk_stages", "eps_q", "delta_s")], shock_limiter=1, moe_alpha=10.0)
+    Ua, tha, na = O.shock_limiter(cfg_a, U)
+    assert na == 0 and (tha == 1.0).all() and np.array_equal(Ua, U)
+    # (b) a jump inside cells: limited there, cell means preserved to rounding, extrema pulled inside
+    #     the neighbours' range
+    Uj = U.copy()
+    Uj[0] *= np.where(np.arange(U.shape[1]) % (7 * nn) < 3 * nn + 4, 1.0, 5.0)
+    U2, th2, n2 = O.shock_limiter(cfg, Uj)
+    assert n2 > 0 and th2.min() < 0.9 and (th2 <= 1.0).all() and (th2 >= 0.0).all()
+    m0 = (Uj.reshape(5, -1, nn) * wn).sum(-1)
+    m1 = (U2.reshape(5, -1, nn) * wn).sum(-1)
+    np.testing.assert_allclose(m1, m0, rtol=1e-13, atol=1e-13)
+    ne = nel[0] * nel[1]
+    mxo, mno = Uj.reshape(5, ne, nn).max(-1), Uj.reshape(5, ne, nn).min(-1)
+    mx2, mn2 = U2.reshape(5, ne, nn).max(-1), U2.reshape(5, ne, nn).min(-1)
+    mean = m0 / wn.sum()
+    for e in range(ne):
+        ix, iy = e % nel[0], e // nel[0]
+        nb = [((ix + 1) % nel[0]) + nel[0] * iy, ((ix - 1) % nel[0]) + nel[0] * iy]
+        nb += [ix + nel[0] * (iy + 1)] if iy + 1 < nel[1] else []
+        nb += [ix + nel[0] * (iy - 1)] if iy > 0 else []
+        M = np.maximum(mean[:, e], mxo[:, nb].max(-1))
+        m = np.minimum(mean[:, e], mno[:, nb].min(-1))
+        assert (mx2[:, e] <= M + 1e-12 * np.abs(M) + 1e-14).all() and (mn2[:, e] >= m - 1e-12 * np.abs(m) - 1e-14).all()
+    # (c) theta depends on ratios only: invariant under a rescaling of the state (alpha = 0)
+    _, th3, _ = O.shock_limiter(cfg, 7.5 * Uj)
+    np.testing.assert_allclose(th3, th2, rtol=1e-12)
+    # (d) inside a step it runs after the physicality operator and keeps every node admissible
+    cfg_s = O.make_config(*[d[k] for k in ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad",
+                                            "rk_stages", "eps_q", "delta_s")], shock_limiter=1, moe_alpha=1e-3)
+    Wj = W.copy()
+    Wj[0] *= np.where(np.arange(U.shape[1]) % (7 * nn) < 3 * nn + 4, 1.0, 5.0)     # a physical density jump
+    Us, _, cnt = O.step(cfg_s, O.prim2con_batch(0, 5.0 / 3.0, Wj), -0.2, 5)
+    assert np.isfinite(Us).all() and all(O.admissible(Us[:, i]) for i in range(0, Us.shape[1], 5))

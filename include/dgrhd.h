@@ -48,6 +48,12 @@ enum { DGRHD_BC_PERIODIC = 0,                /* wrap                            
 /* Interface (Riemann) flux: the two-wave HLL flux (reading R9) or the
  * three-wave HLLC flux of Mignone & Bodo (ref [34]); both with lambda_L, lambda_R of Eq. 23-24. */
 enum { DGRHD_RIEMANN_HLL = 0, DGRHD_RIEMANN_HLLC = 1 };
+/* Shock limiter: none, or the limiter of Moe, Rossmanith & Seal (ref [23]):
+ * every cell is rescaled toward its average by theta = min(1, phi((M - wbar)/(w_M - wbar)), phi((m - wbar)/
+ * (w_m - wbar))) over the five conserved variables, phi(y) = min(y/1.1, 1), with M, m the extrema of the face
+ * neighbours' nodal values widened to wbar +- alpha.  The paper cites it without printing it (DESIGN.md
+ * reading R18). */
+enum { DGRHD_SHOCK_LIMITER_NONE = 0, DGRHD_SHOCK_LIMITER_MOE = 1 };
 enum { DGRHD_OK = 0, DGRHD_EINVAL = 1, DGRHD_ENOMEM = 2, DGRHD_ECUDA = 3, DGRHD_ESTATE = 4 };
 
 /* Problem statement: mesh, order, EOS. */
@@ -63,6 +69,9 @@ typedef struct {
   double  eps_q, delta_s;  /* safety knobs of the physicality operator (reading R13c);
                               0,0 = the paper verbatim; defaults used by the tests: 1e-12, 1e-10   */
   int     riemann;         /* DGRHD_RIEMANN_*                                                       */
+  int     shock_limiter;   /* DGRHD_SHOCK_LIMITER_*: applied after the physicality operator of every
+                              stage of dgrhd_step (two extra small launches per stage)              */
+  double  moe_alpha;       /* tolerance alpha(h) >= 0 of the Moe limiter (ref [23] suggests ~500 h^1.5) */
   double  bc_state[3][2][5]; /* Dirichlet ghost primitives [axis][end] = rho, ux, uy, uz, P          */
 } dgrhd_config;
 
@@ -108,6 +117,11 @@ int dgrhd_rhs(dgrhd_ctx* ctx, const double* U_dev, double* R_dev);
 int dgrhd_enforce_physicality(dgrhd_ctx* ctx, double* U_dev, unsigned char* flag_dev,
                               double* s_dev, int64_t counters_host[2]);
 
+/* The shock limiter the context was created with (DGRHD_SHOCK_LIMITER_MOE), in place on U_dev[5][ndof];
+ * theta_dev[n_elem] (or NULL) receives every cell's rescaling factor (1 = untouched).  ESTATE if the
+ * context has no shock limiter.  Inside dgrhd_step it runs after the physicality operator of every stage. */
+int dgrhd_shock_limiter(dgrhd_ctx* ctx, double* U_dev, double* theta_dev);
+
 /* CFL time step (formula: DESIGN.md reading R11):
  *   dt = cfl / max_nodes sum_d (2p+1) max(|lambda-_d|, |lambda+_d|) / h_d,  lambda+- of Eq. 21-22.
  * U_dev = NULL uses the internal state.  Synchronises; *dt_host receives dt.  ESTATE if the state has no
@@ -131,8 +145,9 @@ int dgrhd_step(dgrhd_ctx* ctx, double dt, int nsteps, double* t_inout_host);
  *                              because the fast route's Newton polish had not converged
  *   out_host[5] n_bad_dt       CFL-mode steps whose wave-speed maximum was not a positive finite
  *                              number: they ran with dt = 0 (state unchanged) instead of dt = inf
+ *   out_host[6] n_shock_limited  cell-rescalings (theta < 1) by the shock limiter; out_host[7] reserved (0)
  * reset != 0 zeroes them afterwards. */
-int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[6], int reset);
+int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[8], int reset);
 
 /* Conserved -> primitive recovery of a flat SoA batch U_dev[5][n] -> W_dev[5][n]:
  * ideal EOS by Newton iteration on the quartic of Eq. 59 (beta = 2w/(1+w^2), Eq. 58; small-xi

@@ -705,7 +705,8 @@ void orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag
  *   2. bounds from the face neighbours N_i (periodic wrap; no neighbour beyond any other boundary):
  *        M_i = max(wbar_i + alpha, max_{j in N_i} w_Mj),  m_i = min(wbar_i - alpha, min_{j in N_i} w_mj);
  *   3. theta_Mi = phi((M_i - wbar_i)/(w_Mi - wbar_i)), theta_mi = phi((m_i - wbar_i)/(w_mi - wbar_i)),
- *      phi(y) = min(y/1.1, 1)  (ratio taken as +inf when the cell's own extremum equals its mean);
+ *      phi(y) = min(y/1.1, 1)  (ratio taken as +inf when the cell's own extremum equals its mean to
+ *      rounding, |w_M - wbar| <= 1e-12 max(|w_M|, |w_m|): a uniform cell is never rescaled);
  *   4. theta_i = min(1, theta_M, theta_m over all variables);
  *   5. U <- Ubar_i + theta_i (U - Ubar_i)   (cell averages unchanged; a convex blend of admissible
  *      states, so the physicality operator's result stays admissible).
@@ -755,8 +756,9 @@ int64_t orc_shock_limiter(const orc_config *c, double *U, double *theta_out) {
           if (st[en * 15 + 5 + v] > M) M = st[en * 15 + 5 + v];
           if (st[en * 15 + 10 + v] < m) m = st[en * 15 + 10 + v];
         }
-      double tM = (wM - wb > 0.0) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
-      double tm = (wb - wm > 0.0) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
+      double tiny = 1e-12 * fmax(fabs(wM), fabs(wm));           /* extremum = mean to rounding: no limit */
+      double tM = (wM - wb > tiny) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
+      double tm = (wb - wm > tiny) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
       if (tM < theta) theta = tM;
       if (tm < theta) theta = tm;
     }

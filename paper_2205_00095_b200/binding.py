@@ -32,6 +32,7 @@ class Config(C.Structure):
                 ("xmax", C.c_double * 3), ("bc", C.c_int * 3), ("order_p", C.c_int),
                 ("eos", C.c_int), ("gamma_ad", C.c_double), ("rk_stages", C.c_int),
                 ("eps_q", C.c_double), ("delta_s", C.c_double), ("riemann", C.c_int),
+                ("shock_limiter", C.c_int), ("moe_alpha", C.c_double),
                 ("bc_state", C.c_double * 5 * 2 * 3)]
 
 
@@ -44,7 +45,7 @@ def _bc_code(b):
 
 
 def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3, eps_q=1e-12,
-                delta_s=1e-10, riemann=0, bc_state=None):
+                delta_s=1e-10, riemann=0, bc_state=None, shock_limiter=0, moe_alpha=0.0):
     c = Config()
     c.ndim = ndim
     for d in range(3):
@@ -55,6 +56,7 @@ def make_config(ndim, nelem, xmin, xmax, bc, order_p, eos, gamma_ad, rk_stages=3
     c.order_p, c.eos, c.gamma_ad, c.rk_stages = order_p, eos, gamma_ad, rk_stages
     c.eps_q, c.delta_s = eps_q, delta_s
     c.riemann = int(riemann)
+    c.shock_limiter, c.moe_alpha = int(shock_limiter), float(moe_alpha)
     for (d, side), W in (bc_state or {}).items():      # {(axis, end): [rho, ux, uy, uz, P]}
         for v in range(5):
             c.bc_state[d][side][v] = float(W[v])
@@ -67,7 +69,7 @@ _vp, _dp, _i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
 EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_state",
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
-           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64", "dgrhd_con2prim_batch_variant",
+           "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64", "dgrhd_con2prim_batch_variant", "dgrhd_shock_limiter",
            "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
 
 
@@ -90,6 +92,7 @@ def lib():
         L.dgrhd_rhs.argtypes = [_vp, _vp, _vp]
         L.dgrhd_enforce_physicality.argtypes = [_vp, _vp, _vp, _vp, _i64p]
         L.dgrhd_cfl_dt.argtypes = [_vp, _vp, C.c_double, _dp]
+        L.dgrhd_shock_limiter.argtypes = [_vp, _vp, _vp]
         L.dgrhd_step.argtypes = [_vp, C.c_double, C.c_int, _dp]
         L.dgrhd_get_counters.argtypes = [_vp, _i64p, C.c_int]
         L.dgrhd_con2prim_batch.argtypes = [C.c_int, C.c_double, C.c_int64, _vp, _vp, _vp, _vp]
@@ -204,6 +207,12 @@ class Context:
                                                _ptr(flag), _ptr(s), cnt if sync else None), self._h)
         return flag, s, (int(cnt[0]), int(cnt[1]))
 
+    def dgrhd_shock_limiter(self, U):
+        """In place on U.  Returns theta[n_e]."""
+        theta = torch.empty(self.n_elem, dtype=torch.float64, device=self.device)
+        _check(lib().dgrhd_shock_limiter(self._h, _ptr(U, 5), _ptr(theta)), self._h)
+        return theta
+
     def dgrhd_cfl_dt(self, cfl, U=None):
         dt = C.c_double()
         _check(lib().dgrhd_cfl_dt(self._h, _ptr(U, 5) if U is not None else None, cfl, C.byref(dt)),
@@ -228,10 +237,10 @@ class Context:
         return tt.value
 
     def dgrhd_get_counters(self, reset=False):
-        out = (C.c_int64 * 6)()
+        out = (C.c_int64 * 8)()
         _check(lib().dgrhd_get_counters(self._h, out, int(reset)), self._h)
         return dict(n_flagged=out[0], n_bad_mean=out[1], n_c2p_fail=out[2], n_stages=out[3],
-                    n_tm_fallback=out[4], n_bad_dt=out[5])
+                    n_tm_fallback=out[4], n_bad_dt=out[5], n_shock_limited=out[6])
 
 
 def dgrhd_con2prim_batch(eos, gamma_ad, U, W=None, status=None):

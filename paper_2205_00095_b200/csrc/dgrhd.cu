@@ -42,7 +42,7 @@ struct DevScalars {
   dg_ull pad_[10];
   dg_ull amax[DG_NSLOT * DG_SLOT_STRIDE];      // ordered-int images of the CFL maximum of the state
   dg_ull amax_tmp[DG_NSLOT * DG_SLOT_STRIDE];  // same, for dgrhd_cfl_dt on a caller state
-  dg_ull counters[DG_NSLOT * DG_SLOT_STRIDE];  // per slot: n_flagged, n_bad_mean, n_c2p_fail, n_tm_fallback
+  dg_ull counters[DG_NSLOT * DG_SLOT_STRIDE];  // per slot: n_flagged, n_bad_mean, n_c2p_fail, n_tm_fallback, n_shock_limited
 };
 
 bool valid_cfg(const dgrhd_config* c) {
@@ -63,6 +63,8 @@ bool valid_cfg(const dgrhd_config* c) {
     }
   }
   if (c->riemann != DGRHD_RIEMANN_HLL && c->riemann != DGRHD_RIEMANN_HLLC) return false;
+  if (c->shock_limiter != DGRHD_SHOCK_LIMITER_NONE && c->shock_limiter != DGRHD_SHOCK_LIMITER_MOE) return false;
+  if (!(c->moe_alpha >= 0.0)) return false;
   if (c->order_p < 0 || c->order_p > 4) return false;
   if (c->eos != DGRHD_EOS_IDEAL && c->eos != DGRHD_EOS_TAUB_MATTHEWS) return false;
   if (c->eos == DGRHD_EOS_IDEAL && !(c->gamma_ad > 1.0)) return false;
@@ -99,6 +101,7 @@ struct dgrhd_ctx {
   // P[0..1]: pressure of the stage input / output, ping-pong; P[par] belongs to the state.
   double* B[3];
   double* P[2];
+  double* moe_stats;        // [n_e][15] cell average / maximum / minimum (shock limiter), else NULL
   int par;
   bool has_state;
   BasisTables basis;
@@ -223,6 +226,48 @@ static cudaError_t launch_limiter(dgrhd_ctx* c, double* U, unsigned char* flag, 
   return launch_limiter_nd<3>(c, U, flag, s, counters);
 }
 
+// The shock limiter on a stage's output (U, P): cell statistics, then bounds / theta / rescale, the
+// pressure of the rescaled cells and, on the step's last stage, the CFL maximum of the limited state.
+template <int ND>
+static cudaError_t launch_moe_nd(dgrhd_ctx* c, double* U, double* P, int do_cfl, dg_ull* amax, dg_ull* counters,
+                                 double* theta) {
+  const LimPar lp = make_limpar(c);
+  MoePar mp;
+  for (int d = 0; d < 3; ++d) {
+    mp.ne[d] = c->cfg.nelem[d];
+    mp.periodic[d] = (d < c->cfg.ndim && (c->cfg.bc[d] & 255) == DGRHD_BC_PERIODIC) ? 1 : 0;
+    mp.cw[d] = (d < c->cfg.ndim) ? (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]) : 0.0;
+  }
+  mp.alpha = c->cfg.moe_alpha;
+  mp.do_cfl = do_cfl;
+#define DG_GO(NV)                                                                                       \
+  {                                                                                                     \
+    constexpr int EPB = 4 * TileShape<ND, NV>::EPW;                                                     \
+    const unsigned nb = (unsigned)((c->nelem + EPB - 1) / EPB);                                         \
+    dg_moe_stats_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, c->moe_stats, lp);     \
+    if (c->cfg.eos == DGRHD_EOS_IDEAL)                                                                  \
+      dg_moe_apply_kernel<ND, NV, 0><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+    else                                                                                                \
+      dg_moe_apply_kernel<ND, NV, 1><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+  }
+  switch (c->N) {
+    case 1: DG_GO(1) break;
+    case 2: DG_GO(2) break;
+    case 3: DG_GO(3) break;
+    case 4: DG_GO(4) break;
+    case 5: DG_GO(5) break;
+  }
+#undef DG_GO
+  return cudaGetLastError();
+}
+
+static cudaError_t launch_moe(dgrhd_ctx* c, double* U, double* P, int do_cfl, dg_ull* amax, dg_ull* counters,
+                              double* theta) {
+  if (c->cfg.ndim == 1) return launch_moe_nd<1>(c, U, P, do_cfl, amax, counters, theta);
+  if (c->cfg.ndim == 2) return launch_moe_nd<2>(c, U, P, do_cfl, amax, counters, theta);
+  return launch_moe_nd<3>(c, U, P, do_cfl, amax, counters, theta);
+}
+
 static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
   memset(&a, 0, sizeof a);
   a.ndof = c->ndof;
@@ -283,6 +328,9 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
 // create / destroy
 // ------------------------------------------------------------------------------------------------
 static size_t pbuf_bytes(long long ndof) { return align_up((size_t)ndof * sizeof(double)); }
+static size_t moe_bytes(const dgrhd_config* cfg, long long ne) {
+  return cfg->shock_limiter ? align_up((size_t)ne * 15 * sizeof(double)) : 0;
+}
 
 extern "C" size_t dgrhd_workspace_bytes(const dgrhd_config* cfg) {
   if (!valid_cfg(cfg)) return 0;
@@ -290,7 +338,7 @@ extern "C" size_t dgrhd_workspace_bytes(const dgrhd_config* cfg) {
   for (int d = 0; d < cfg->ndim; ++d) ne *= cfg->nelem[d];
   const long long ndof = ne * ipow(cfg->order_p + 1, cfg->ndim);
   const size_t sb = align_up((size_t)ndof * 5 * sizeof(double));
-  return align_up(sizeof(DevScalars)) + 3 * sb + 2 * pbuf_bytes(ndof);
+  return align_up(sizeof(DevScalars)) + 3 * sb + 2 * pbuf_bytes(ndof) + moe_bytes(cfg, ne);
 }
 
 extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t workspace_bytes,
@@ -323,6 +371,7 @@ extern "C" int dgrhd_create(const dgrhd_config* cfg, void* workspace_dev, size_t
   const size_t sb = align_up(c->state_bytes);
   for (int i = 0; i < 3; ++i) { c->B[i] = (double*)p;  p += sb; }
   for (int i = 0; i < 2; ++i) { c->P[i] = (double*)p;  p += pbuf_bytes(c->ndof); }
+  c->moe_stats = cfg->shock_limiter ? (double*)p : nullptr;
   // sum of the tensor weights (summed in node order)
   c->wsum = 0.0;
   for (int n = 0; n < c->NN; ++n) {
@@ -442,6 +491,16 @@ extern "C" int dgrhd_enforce_physicality(dgrhd_ctx* c, double* U_dev, unsigned c
   return DGRHD_OK;
 }
 
+extern "C" int dgrhd_shock_limiter(dgrhd_ctx* c, double* U_dev, double* theta_dev) {
+  if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_shock_limiter: NULL argument");
+  if (c->cfg.shock_limiter != DGRHD_SHOCK_LIMITER_MOE)
+    return fail(c, DGRHD_ESTATE, "dgrhd_shock_limiter: the context was created without a shock limiter");
+  if (!aligned16(U_dev)) return fail(c, DGRHD_EINVAL, "dgrhd_shock_limiter: state pointer must be 16-byte aligned");
+  // (the pressure of the rescaled cells lands in the spare pressure buffer; no counters, no CFL)
+  DG_CUDA(c, launch_moe(c, U_dev, c->P[c->par ^ 1], 0, c->sc->amax_tmp, c->sc->amax_tmp, theta_dev));
+  return DGRHD_OK;
+}
+
 extern "C" int dgrhd_cfl_dt(dgrhd_ctx* c, const double* U_dev, double cfl, double* dt_host) {
   if (!c || !dt_host) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: NULL argument");
   if (!(cfl > 0.0)) return fail(c, DGRHD_EINVAL, "dgrhd_cfl_dt: cfl must be > 0");
@@ -499,8 +558,10 @@ static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
     }
     a.Pin = c->P[c->par];
     a.Pout = c->P[c->par ^ 1];
-    a.do_cfl = last ? 1 : 0;
+    const bool moe = (c->cfg.shock_limiter == DGRHD_SHOCK_LIMITER_MOE);
+    a.do_cfl = (last && !moe) ? 1 : 0;                     // with the shock limiter: taken from the limited state
     DG_CUDA(c, launch_stage(c, a));
+    if (moe) DG_CUDA(c, launch_moe(c, a.Uout, a.Pout, last ? 1 : 0, c->sc->amax, c->sc->counters, nullptr));
     c->par ^= 1;
   }
   return DGRHD_OK;
@@ -580,7 +641,7 @@ extern "C" int dgrhd_run_host(dgrhd_ctx* c, const double* U_host_in, double* U_h
   return DGRHD_OK;
 }
 
-extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[6], int reset) {
+extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[8], int reset) {
   if (!c || !out_host) return fail(c, DGRHD_EINVAL, "dgrhd_get_counters: NULL argument");
   DevScalars h;
   DG_CUDA(c, cudaMemcpyAsync(&h, c->sc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
@@ -589,15 +650,17 @@ extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[6], int reset) 
     DG_CUDA(c, cudaMemsetAsync(&c->sc->n_stages, 0, 2 * sizeof(dg_ull), c->stream));
   }
   DG_CUDA(c, cudaStreamSynchronize(c->stream));
-  dg_ull sum[4] = {0, 0, 0, 0};
+  dg_ull sum[5] = {0, 0, 0, 0, 0};
   for (int s = 0; s < DG_NSLOT; ++s)
-    for (int k = 0; k < 4; ++k) sum[k] += h.counters[s * DG_SLOT_STRIDE + k];
+    for (int k = 0; k < 5; ++k) sum[k] += h.counters[s * DG_SLOT_STRIDE + k];
   out_host[0] = (int64_t)sum[0];
   out_host[1] = (int64_t)sum[1];
   out_host[2] = (int64_t)sum[2];
   out_host[3] = (int64_t)h.n_stages;
   out_host[4] = (int64_t)sum[3];
   out_host[5] = (int64_t)h.n_bad_dt;
+  out_host[6] = (int64_t)sum[4];
+  out_host[7] = 0;
   return DGRHD_OK;
 }
 

@@ -195,6 +195,182 @@ dg_limiter_kernel(long long nelem, long long ndof, double* U, unsigned char* fla
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Shock limiter of Moe, Rossmanith & Seal (PAPER.md:126, :551, :621 ref [23]; reading R18:
+// cited, not printed, by the paper).  Two cell-wise kernels in the thread mapping of the stage kernel
+// (a cell = NL consecutive lanes of one warp, reductions by shuffle), run after a stage when the
+// context's shock_limiter is on:
+//   dg_moe_stats_kernel   per cell and conserved variable: average (tensor GLL weights), maximum and
+//                         minimum over the cell's nodes            -> stats[n_e][15]
+//   dg_moe_apply_kernel   bounds from the face neighbours' extrema (periodic wrap; none beyond any
+//                         other boundary) and the tolerance alpha; theta = min(1, phi(.)) over all
+//                         variables, phi(y) = min(y/1.1, 1); U <- Ubar + theta (U - Ubar) in the limited
+//                         cells, whose pressure is recovered again; on the step's last stage the CFL
+//                         maximum is taken here, from the limited state.
+// ---------------------------------------------------------------------------------------------
+template <int NL>
+DG_INL double dg_cell_max(double x, int base) {
+  if ((NL & (NL - 1)) == 0) {
+#pragma unroll
+    for (int o = NL / 2; o > 0; o >>= 1) x = fmax(x, __shfl_xor_sync(0xffffffffu, x, o));
+    return x;
+  }
+  double acc = x;
+#pragma unroll
+  for (int o = 0; o < NL; ++o) acc = fmax(acc, __shfl_sync(0xffffffffu, x, min(base + o, 31)));
+  return acc;
+}
+
+template <int ND, int N>
+__global__ void __launch_bounds__(128)
+dg_moe_stats_kernel(long long nelem, long long ndof, const double* __restrict__ U, double* __restrict__ stats,
+                    LimPar lp) {
+  using TS = TileShape<ND, N>;
+  constexpr int NN = TS::NN, NL = TS::NL, EPW = TS::EPW, SEG = TS::SEG, NSEG = TS::NSEG;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const int ew = lane / NL, lt = lane - ew * NL;
+  const int h = lt % NSEG, ln = lt / NSEG;
+  const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
+  const bool active = (ew < EPW) && (e < nelem);
+  const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
+  const long long g0 = (active ? e : 0) * NN + N * ln + h * SEG;
+  const int base = ew * NL;
+  double wl = 1.0;
+  if (ND >= 2) wl *= lp.w[j];
+  if (ND >= 3) wl *= lp.w[k];
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    double x[SEG];
+    dg_ld_line<SEG>(U + v * ndof + g0, x);
+    double part = 0.0, mx = x[0], mn = x[0];
+#pragma unroll
+    for (int m = 0; m < SEG; ++m) {
+      const double wq = wl * ((NSEG > 1 && h > 0) ? lp.w[(SEG + m) % 5] : lp.w[m]);
+      part = fma(wq, x[m], part);
+      mx = fmax(mx, x[m]);
+      mn = fmin(mn, x[m]);
+    }
+    const double mean = dg_cell_sum<NL>(part, base) / lp.wsum;
+    mx = dg_cell_max<NL>(mx, base);
+    mn = dg_cell_min<NL>(mn, base);
+    if (active && lt == 0) {
+      stats[e * 15 + v] = mean;
+      stats[e * 15 + 5 + v] = mx;
+      stats[e * 15 + 10 + v] = mn;
+    }
+  }
+}
+
+struct MoePar {
+  long long ne[3];
+  int periodic[3];
+  double alpha;
+  double cw[3];
+  int do_cfl;
+};
+
+template <int ND, int N, int EOS>
+__global__ void __launch_bounds__(128)
+dg_moe_apply_kernel(long long nelem, long long ndof, double* U, double* P, const double* __restrict__ stats,
+                    MoePar mp, EosPar eos, dg_ull* amax, dg_ull* counters, double* theta_out) {
+  using TS = TileShape<ND, N>;
+  constexpr int NN = TS::NN, NL = TS::NL, EPW = TS::EPW, SEG = TS::SEG, NSEG = TS::NSEG;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const int ew = lane / NL, lt = lane - ew * NL;
+  const int h = lt % NSEG, ln = lt / NSEG;
+  const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
+  const bool active = (ew < EPW) && (e < nelem);
+  const long long g0 = (active ? e : 0) * NN + N * ln + h * SEG;
+  double theta = 1.0, mean[5] = {0, 0, 0, 0, 0};
+  if (active) {
+    const long long ie[3] = {e % mp.ne[0], (e / mp.ne[0]) % mp.ne[1], e / (mp.ne[0] * mp.ne[1])};
+    const long long es[3] = {1, mp.ne[0], mp.ne[0] * mp.ne[1]};
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      const double wb = stats[e * 15 + v], wM = stats[e * 15 + 5 + v], wm = stats[e * 15 + 10 + v];
+      mean[v] = wb;
+      double M = wb + mp.alpha, m = wb - mp.alpha;
+#pragma unroll
+      for (int d = 0; d < ND; ++d)
+#pragma unroll
+        for (int side = 0; side < 2; ++side) {
+          long long jd = ie[d] + (side ? 1 : -1);
+          if (jd < 0 || jd >= mp.ne[d]) {
+            if (!mp.periodic[d]) continue;
+            jd = (jd + mp.ne[d]) % mp.ne[d];
+          }
+          const long long en = e + (jd - ie[d]) * es[d];
+          M = fmax(M, stats[en * 15 + 5 + v]);
+          m = fmin(m, stats[en * 15 + 10 + v]);
+        }
+      const double tiny = 1e-12 * fmax(fabs(wM), fabs(wm));     // extremum = mean to rounding: no limit
+      const double tM = (wM - wb > tiny) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
+      const double tm = (wb - wm > tiny) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
+      theta = fmin(theta, fmin(tM, tm));
+    }
+  }
+  if (theta_out && active && lt == 0) theta_out[e] = theta;
+  const bool lim = active && (theta < 1.0);
+  const bool need = lim || (active && mp.do_cfl);
+  double speed = 0.0;
+  int nfail = 0, nfall = 0;
+  if (need) {
+    double Uo[SEG][5], Po[SEG];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+      double x[SEG];
+      dg_ld_line<SEG>(U + v * ndof + g0, x);
+#pragma unroll
+      for (int m = 0; m < SEG; ++m) Uo[m][v] = lim ? fma(theta, x[m] - mean[v], mean[v]) : x[m];
+    }
+    if (lim) {
+      int st[SEG];
+      dg_con2prim_n<EOS, SEG, false>(eos, Uo, nullptr, Po, st, &nfall);
+#pragma unroll
+      for (int m = 0; m < SEG; ++m) nfail += (st[m] != 0) ? 1 : 0;
+#pragma unroll
+      for (int v = 0; v < 5; ++v) {
+        double x[SEG];
+#pragma unroll
+        for (int m = 0; m < SEG; ++m) x[m] = Uo[m][v];
+        dg_st_line<SEG>(U + v * ndof + g0, x);
+      }
+      dg_st_line<SEG>(P + g0, Po);
+    } else {
+      dg_ld_line<SEG>(P + g0, Po);
+    }
+    if (mp.do_cfl) {
+#pragma unroll
+      for (int m = 0; m < SEG; ++m) {
+        const double sp = dg_cfl_speed<EOS, ND>(eos, Uo[m], Po[m], mp.cw);
+        if (sp > 0.0) speed = fmax(speed, sp);
+      }
+    }
+  }
+  const int slot = (int)((blockIdx.x * 4 + wrp) % DG_NSLOT) * DG_SLOT_STRIDE;
+  if (mp.do_cfl) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
+    if (lane == 0 && speed > 0.0) atomicMax(amax + slot, dg_ord(speed));
+  }
+  const int nlim = (lim && lt == 0) ? 1 : 0;
+  const unsigned any = __ballot_sync(0xffffffffu, (nlim | nfail | nfall) != 0);
+  if (any) {
+    int c0 = nlim, c1 = nfail, c2 = nfall;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      c0 += __shfl_xor_sync(0xffffffffu, c0, o);
+      c1 += __shfl_xor_sync(0xffffffffu, c1, o);
+      c2 += __shfl_xor_sync(0xffffffffu, c2, o);
+    }
+    if (lane == 0) {
+      if (c0) atomicAdd(&counters[slot + 4], (dg_ull)c0);
+      if (c1) atomicAdd(&counters[slot + 2], (dg_ull)c1);
+      if (c2) atomicAdd(&counters[slot + 3], (dg_ull)c2);
+    }
+  }
+}
+
 // FP64 FMA throughput probe (the roofline denominator of the ALU-bound kernels, measured on the box
 // instead of derived from unit counts): 8 independent DFMA chains per thread, no memory traffic.
 __global__ void __launch_bounds__(256)

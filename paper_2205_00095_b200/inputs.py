@@ -69,7 +69,7 @@ def _u_from_v(v):
 def _cfg(ndim, nelem, xmin, xmax, bc, p, eos, gamma_ad, **kw):
     d = dict(ndim=ndim, nelem=list(nelem), xmin=list(xmin), xmax=list(xmax), bc=list(bc),
              order_p=p, eos=eos, gamma_ad=gamma_ad, rk_stages=3, eps_q=1e-12, delta_s=1e-10,
-             riemann=RIEMANN_HLL, bc_state=None)
+             riemann=RIEMANN_HLL, bc_state=None, shock_limiter=0, moe_alpha=0.0)
     d.update(kw)
     return d
 

@@ -8,7 +8,7 @@ from paper_2205_00095_b200 import inputs as I
 
 DEV = "cuda"
 KEYS = ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad", "rk_stages", "eps_q",
-        "delta_s", "riemann", "bc_state")
+        "delta_s", "riemann", "bc_state", "shock_limiter", "moe_alpha")
 
 
 def B():
@@ -17,12 +17,12 @@ def B():
 
 
 def ocfg(d, **kw):
-    d = {"riemann": 0, "bc_state": None, **d, **kw}
+    d = {"riemann": 0, "bc_state": None, "shock_limiter": 0, "moe_alpha": 0.0, **d, **kw}
     return O.make_config(*[d[k] for k in KEYS])
 
 
 def gcfg(d, **kw):
-    d = {"riemann": 0, "bc_state": None, **d, **kw}
+    d = {"riemann": 0, "bc_state": None, "shock_limiter": 0, "moe_alpha": 0.0, **d, **kw}
     return B().make_config(*[d[k] for k in KEYS])
 
 

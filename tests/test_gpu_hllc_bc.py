@@ -196,3 +196,50 @@ def test_paper_2d_riemann_problems_match_oracle(k, p):
     bound = 1e-9 + 100 * 2.2e-16 * 15 / pe_min
     print(f"    min P/E {pe_min:.2e}: R16 bound {bound:.2e}")
     assert err.max() <= bound and abs(c["n_flagged"] - cnt_o[0]) <= max(2, cnt_o[0] // 50)
+
+
+# ------------------------------------------------------------------------------------------------
+# f2: the shock limiter of Moe et al. (reading R18; cited, not printed, by the paper)
+# ------------------------------------------------------------------------------------------------
+MOE_CASES = [(1, [70], 2, 0, 5 / 3, [1]), (1, [33], 1, 1, 0.0, [0]), (2, [21, 10], 2, 1, 0.0, [0, 1]),
+             (2, [9, 7], 3, 0, 5 / 3, [1, 0]), (3, [5, 3, 3], 3, 0, 5 / 3, [0, 0, 0]),
+             (3, [6, 5, 3], 2, 0, 4 / 3, [0, 1, 0]), (3, [3, 2, 2], 4, 1, 0.0, [1, 1, 0]), (2, [12, 5], 0, 0, 5 / 3, [0, 0])]
+
+
+@pytest.mark.parametrize("nd,nelem,p,eos,G,bc", MOE_CASES)
+def test_shock_limiter_matches_oracle_cell_by_cell(nd, nelem, p, eos, G, bc):
+    import torch
+    d = mesh(nd, nelem, p, eos, G, bc, shock_limiter=1, moe_alpha=1e-3)
+    nn = (p + 1) ** nd
+    W = smooth_prims(d, seed=40 + nd + p)
+    W[0] *= np.where((np.arange(W.shape[1]) // nn) % 5 < 2, 1.0, 6.0)              # density jumps between and
+    W[4] *= np.where(np.arange(W.shape[1]) % (3 * nn) < nn + nn // 2, 1.0, 3.0)    # pressure jumps inside cells
+    U = O.prim2con_batch(eos, G, W)
+    Uo, th_o, n_o = O.shock_limiter(ocfg(d), U)
+    ctx = B().Context(gcfg(d))
+    Ug = to_dev(U)
+    th_g = ctx.dgrhd_shock_limiter(Ug).cpu().numpy()
+    assert (n_o > 0) or p == 0
+    assert np.array_equal(th_g < 1.0, th_o < 1.0)                                  # the same cells are limited
+    np.testing.assert_allclose(th_g, th_o, rtol=1e-11, atol=1e-13)
+    scale = np.abs(Uo).max(axis=0) + 1e-300
+    assert np.max(np.abs(Ug.cpu().numpy() - Uo) / scale) <= 1e-11
+
+
+@pytest.mark.parametrize("k", [1, 4])
+def test_paper_riemann_problems_with_the_shock_limiter_match_oracle(k):
+    """The paper's shock set-up: HLLC + Moe limiter + physicality operator, p = 2."""
+    d, W, _ = I.paper_riemann1d(k, ne=128, p=2, riemann=I.RIEMANN_HLLC)
+    d = dict(d, shock_limiter=1, moe_alpha=500.0 * (1.0 / 128) ** 1.5)
+    U = O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy())
+    Uo, to, cnt_o = O.step(ocfg(d), U, -0.2, 30)
+    ctx = B().Context(gcfg(d))
+    ctx.dgrhd_set_state(to_dev(U))
+    tg = ctx.dgrhd_step(-0.2, 30, t=0.0)
+    Ug = ctx.dgrhd_get_state().cpu().numpy()
+    c = ctx.dgrhd_get_counters()
+    err = relmax(Ug, Uo)[[0, 1, 4]]
+    print(f"paper Riemann problem {k} + Moe limiter: max-norm rel. diff {err.max():.2e}, physicality activations "
+          f"{cnt_o[0]} / {c['n_flagged']}, cells rescaled by the shock limiter {c['n_shock_limited']}")
+    assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to and c["n_shock_limited"] > 0
+    assert err.max() <= 1e-8

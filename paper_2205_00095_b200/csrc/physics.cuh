@@ -320,6 +320,28 @@ static __device__ __noinline__ double dg_tm_closed_form_fp64(double c1, double c
   return Wv;
 }
 
+// Single-precision pieces of the closed form's starting point (their error only moves the seed):
+// acos by the seven-term fit sqrt(1 - x) * poly(x) of Abramowitz & Stegun 4.4.46 (|err| <= 2e-8 on
+// [0, 1], acos(-x) = pi - acos(x)); the real cube root by exp2(log2|x| / 3) on the SFU.
+DG_INL float dg_acos_seed(float x) {
+  const float ax = fabsf(x);
+  float p = -0.0012624911f;
+  p = fmaf(p, ax, 0.0066700901f);
+  p = fmaf(p, ax, -0.0170881256f);
+  p = fmaf(p, ax, 0.0308918810f);
+  p = fmaf(p, ax, -0.0501743046f);
+  p = fmaf(p, ax, 0.0889789874f);
+  p = fmaf(p, ax, -0.2145988016f);
+  p = fmaf(p, ax, 1.5707963050f);
+  float sq;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(sq) : "f"(1.0f - ax));
+  const float r = sq * p;
+  return (x < 0.0f) ? 3.14159265f - r : r;
+}
+DG_INL float dg_cbrt_seed(float x) {
+  return copysignf(exp2f(__log2f(fabsf(x)) * (1.0f / 3.0f)), x);
+}
+
 template <int NS>
 DG_INL void dg_tm_solve_W(const double* D, const double* E, const double* Mabs, double* Wv, int* nfall) {
 #pragma unroll
@@ -342,18 +364,19 @@ DG_INL void dg_tm_solve_W(const double* D, const double* E, const double* Mabs, 
     double W0;
     if (d < 0.0) {
       const double rq = dg_rsqrt(-Q);                                        // 1/sqrt(-Q): serves both roots
-      double arg = R * (rq * rq * rq);
-      arg = fmin(1.0, fmax(-1.0, arg));
-      const float th = acosf((float)arg) * (1.0f / 3.0f);
-      W0 = 2.0 * (-Q * rq) * (double)cosf(th) - c1 * (1.0 / 3.0);            // Eq. 69-70
+      const float arg = fminf(1.0f, fmaxf(-1.0f, __double2float_rn(R * (rq * rq * rq))));
+      const float th = dg_acos_seed(arg) * (1.0f / 3.0f);
+      W0 = 2.0 * (-Q * rq) * (double)__cosf(th) - c1 * (1.0 / 3.0);          // Eq. 69-70 (th in [0, pi/3])
     } else {
       const double sd = dg_sqrt(d);
       const double p = R + sd, q = R - sd;
-      const double cp = (fabs(p) < 1e37) ? (double)cbrtf((float)p) : cbrt(p);
-      const double cq = (fabs(q) < 1e37) ? (double)cbrtf((float)q) : cbrt(q);
-      W0 = cp + cq - c1 * (1.0 / 3.0);                                       // Eq. 71-73
+      const float pf = __double2float_rn(p), qf = __double2float_rn(q);
+      double cs;
+      if (fmaxf(fabsf(pf), fabsf(qf)) < 1e37f) cs = (double)(dg_cbrt_seed(pf) + dg_cbrt_seed(qf));
+      else cs = cbrt(p) + cbrt(q);                                           // beyond the single-precision range
+      W0 = cs - c1 * (1.0 / 3.0);                                            // Eq. 71-73
     }
-    W0 = fmax(W0, 0.0);
+    W0 = (W0 > 0.0) ? W0 : 0.0;                                              // (NaN -> 0 as well)
     // R7b polish: two steps square the ~1e-7 seed error twice; the step is a tight estimate of the error
     // before it, so |dW| <= 1e-9 W certifies the fp64 floor.  States that are not there yet (gamma -> 1,
     // where W is tiny against the seed's absolute error) take two more steps in full precision.

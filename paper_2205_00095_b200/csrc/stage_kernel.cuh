@@ -82,13 +82,13 @@ struct TileShape {
   __host__ __device__ static constexpr int SE(int d) { return d == 0 ? 1 : (d == 1 ? TX : TX * TY); }
   __host__ __device__ static constexpr int SS(int d) { return d == 0 ? 1 : (d == 1 ? N : PK); }
   // Slot of the segment h of line (j,k) of tile element le, and of node (i,j,k).  For the 64-node
-  // hexahedron (two 16-byte segments per line) the eight segments of a k-plane are rotated by k
-  // positions: the line loads of the volume terms stay conflict-free, and the face points -- which
-  // read nodes of one parity of i only, at stride-4 addresses in the natural order (4-way bank
-  // conflicts) -- spread over all banks that parity can reach (2-way for x and y faces, none for z).
+  // hexahedron (two 16-byte segments per line) the four lines of a k-plane are rotated by k lines and
+  // the two segments of a line swapped for odd k: the line loads of the volume terms stay conflict-free,
+  // the y- and z-face loads become conflict-free, and the x-face points -- which read nodes of one
+  // parity of i only (4-way bank conflicts in the natural order) -- reach the 2-way floor.
   static constexpr bool SWZ = (ND == 3 && N == 4);
   __host__ __device__ static constexpr int seg_slot(int le, int h, int j, int k) {
-    return SWZ ? le * ES + 16 * k + 2 * ((2 * j + h + k) & 7) : le * ES + h * SEG + N * j + PK * k;
+    return SWZ ? le * ES + 16 * k + 4 * ((j + k) & 3) + 2 * (h ^ (k & 1)) : le * ES + h * SEG + N * j + PK * k;
   }
   __host__ __device__ static constexpr int node_slot(int le, int i, int j, int k) {
     return SWZ ? seg_slot(le, i >> 1, j, k) + (i & 1) : le * ES + i + N * j + PK * k;
@@ -101,6 +101,13 @@ struct TileShape {
   // interior face planes only (the flux of a boundary plane is kept in its halo slot, see below)
   __host__ __device__ static constexpr int FOFFI(int d) {
     return d <= 0 ? 0 : FOFFI(d - 1) + (T(d - 1) - 1) * FP(d - 1);
+  }
+  // interface fluxes: direction D holds T(D)+1 face planes of PS(D) doubles, a plane = 5 components of
+  // FP(D) points (+ padding: consecutive y-planes of the 64-node hexahedron are shifted by 32 bytes so
+  // that the lift's 16-byte loads of the minus and the plus face fall into different banks)
+  __host__ __device__ static constexpr int PS(int d) { return 5 * FP(d) + ((SWZ && d == 1) ? 4 : 0); }
+  __host__ __device__ static constexpr int FHOFF(int d) {
+    return d <= 0 ? 0 : FHOFF(d - 1) + (T(d - 1) + 1) * PS(d - 1);
   }
   static constexpr int NHALO = HOFF(ND);             // halo points of the tile
   static constexpr int NHP = (NHALO + 1) / 2 * 2;    // halo slots per row (even)
@@ -115,7 +122,7 @@ struct TileShape {
   static constexpr int RS = NS + NHP;                // row stride
   static constexpr int O_X = 0;
   static constexpr int O_FH = O_X + NREC * RS;       // Fhat  [dir][plane][5][FP]
-  static constexpr int O_D = O_FH + (5 * NFACE + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = x, y, z
+  static constexpr int O_D = O_FH + (FHOFF(ND) + 1) / 2 * 2;   // (2/h_d) Dhat[i][q] for d = x, y, z
   static constexpr int SMEM_BYTES = (O_D + 3 * 26) * 8;
   static constexpr int BLK_SMEM = (227 * 1024) / (SMEM_BYTES + 1024);
   static constexpr int REG_FLOOR = (SEG <= 1) ? 64 : ((SEG >= 6) ? 240 : 40 * SEG);   // registers per thread to leave
@@ -447,9 +454,9 @@ DG_INL bool dg_face_sides(int fl, const int teff[3], FaceSides& fs) {
   fs.sr = fs.hr ? hr_slot : TS::node_slot(telem + p * TS::SE(D), cr[0], (ND >= 2) ? cr[1] : 0, (ND >= 3) ? cr[2] : 0);
   DG_ASSERT(fs.sl >= 0 && fs.sl < TS::RS && fs.sr >= 0 && fs.sr < TS::RS);
   DG_ASSERT(TS::HOFF(D) + FPD + fp < TS::NHALO);
-  fs.of = TS::O_FH + 5 * TS::FOFF(D) + p * 5 * FPD + fp;
+  fs.of = TS::O_FH + TS::FHOFF(D) + p * TS::PS(D) + fp;
   fs.fstride = FPD;
-  DG_ASSERT(5 * TS::FOFF(D) + p * 5 * FPD + 4 * FPD + fp < 5 * TS::NFACE);
+  DG_ASSERT(TS::FHOFF(D) + p * TS::PS(D) + 4 * FPD + fp < TS::FHOFF(ND));
   return true;
 }
 
@@ -517,33 +524,34 @@ DG_INL void dg_volume_seg(const double* X, const double* dh, int le, int h, int 
   }
 }
 
-// Volume term of direction x for a thread that owns only a segment of its line: the whole line's
-// records (N adjacent slots) are read once; dh: rows (2/h_x) Dhat[i0+m][.] of the thread's nodes.
+// Volume term of direction x for a thread that owns only a segment of its line: the line's segments
+// (SEG adjacent slots each) are read one after the other; dh: rows (2/h_x) Dhat[i0+m][.] of the
+// thread's nodes.
 template <int ND, int N>
 DG_INL void dg_volume_x_seg(const double* X, const double* dh, int le, int j, int k, double (*R)[5]) {
   using TS = TileShape<ND, N>;
   constexpr int S = TS::RS, SEG = TS::SEG, NSEG = TS::NSEG;
-  double u[4][N], Pq[N], rq[N], c[SEG][N];
 #pragma unroll
   for (int g = 0; g < NSEG; ++g) {
     const double* x = X + TS::seg_slot(le, g, j, k);
+    double u[4][SEG], Pq[SEG], rq[SEG], c[SEG][SEG];
 #pragma unroll
-    for (int v = 0; v < 4; ++v) dg_ld_line<SEG>(x + v * S, u[v] + g * SEG);
-    dg_ld_line<SEG>(x + 5 * S, Pq + g * SEG);
-    dg_ld_line<SEG>(x + 6 * S, rq + g * SEG);
-  }
+    for (int v = 0; v < 4; ++v) dg_ld_line<SEG>(x + v * S, u[v]);
+    dg_ld_line<SEG>(x + 5 * S, Pq);
+    dg_ld_line<SEG>(x + 6 * S, rq);
 #pragma unroll
-  for (int m = 0; m < SEG; ++m) dg_ld_line<N>(dh + m * N, c[m]);
+    for (int m = 0; m < SEG; ++m) dg_ld_line<SEG>(dh + m * N + g * SEG, c[m]);
 #pragma unroll
-  for (int q = 0; q < N; ++q) {
-    const double vx = u[1][q] * rq[q];
+    for (int q = 0; q < SEG; ++q) {
+      const double vx = u[1][q] * rq[q];
 #pragma unroll
-    for (int m = 0; m < SEG; ++m) {
-      const double t = c[m][q] * vx;
+      for (int m = 0; m < SEG; ++m) {
+        const double t = c[m][q] * vx;
 #pragma unroll
-      for (int v = 0; v < 4; ++v) R[m][v] = fma(t, u[v][q], R[m][v]);
-      R[m][1] = fma(c[m][q], Pq[q], R[m][1]);
-      R[m][4] = fma(c[m][q], u[1][q], R[m][4]);
+        for (int v = 0; v < 4; ++v) R[m][v] = fma(t, u[v][q], R[m][v]);
+        R[m][1] = fma(c[m][q], Pq[q], R[m][1]);
+        R[m][4] = fma(c[m][q], u[1][q], R[m][4]);
+      }
     }
   }
 }
@@ -554,7 +562,7 @@ template <int ND, int N, int D>
 DG_INL int dg_flux_off(int p, int teffD, int fp, int& stride) {
   using TS = TileShape<ND, N>;
   stride = TS::FP(D);
-  return TS::O_FH + 5 * TS::FOFF(D) + p * 5 * TS::FP(D) + fp;
+  return TS::O_FH + TS::FHOFF(D) + p * TS::PS(D) + fp;
 }
 
 // Lift of the interface flux of direction D = 1 or 2 onto the thread's nodes (Eq. 18): the segment
@@ -583,6 +591,37 @@ DG_INL void dg_lift_seg(const double* sm, int id, int lcD, int teffD, int fp0, d
     }
   }
 }
+
+// Halo: the facing nodal layer of the neighbouring elements (GLL nodes: the face interpolation of
+// :132-134 is a gather, reading R1) -> halo rows U | P, asynchronously.  One UNIT = UW consecutive face
+// points of direction D on the tile's minus (side 0) or plus (side 1) boundary, first point fp; used for
+// even N, where the units are dealt to the block's threads in flat order (a warp then writes consecutive
+// shared-memory addresses).
+// Source: the own boundary node's global index + a.hoff (one element over) + a.hfix where the tile
+// touches the mesh boundary (periodic wrap or, for the other conditions, the node itself: reading R12).
+template <int ND, int N, int D, int UW>
+DG_INL void dg_halo_unit(const StageArgs& a, double* XH, const int org[3], const int teff[3], int side, int fp) {
+  using TS = TileShape<ND, N>;
+  constexpr int A = (D == 0) ? 1 : 0, B = (D == 2) ? 1 : 2;         // transverse axes (ascending)
+  const int te = fp / TS::NF1, tn = fp - te * TS::NF1;
+  const int la = te % TS::T(A), lb = te / TS::T(A);
+  if (la >= teff[A] || lb >= teff[B]) return;                       // ragged tile
+  int lc[3], nc[3];
+  lc[A] = la; lc[B] = lb; lc[D] = side ? teff[D] - 1 : 0;
+  nc[A] = tn % N; nc[B] = tn / N; nc[D] = side ? N - 1 : 0;
+  const int e = (org[0] + lc[0]) + a.ne[0] * ((org[1] + lc[1]) + a.ne[1] * (org[2] + lc[2]));
+  const bool edge = side ? (org[D] + teff[D] == a.ne[D]) : (org[D] == 0);
+  const int g = e * TS::NN + nc[0] + N * (nc[1] + N * nc[2]) + a.hoff[D][side] + (edge ? a.hfix[D][side] : 0);
+  DG_ASSERT(g >= 0 && g + UW <= a.ndof && TS::HOFF(D) + side * TS::FP(D) + fp + UW <= TS::NHALO);
+  double* dst = XH + (TS::HOFF(D) + side * TS::FP(D) + fp);
+#pragma unroll
+  for (int v = 0; v < 6; ++v) {
+    const double* src = (v < 5) ? a.Us + v * a.ndof + g : a.Pin + g;
+    if (UW == 2) dg_async_line<2>(dst + v * TS::RS, src);
+    else dg_async_copy8(dst + v * TS::RS, src);
+  }
+}
+
 
 template <int ND, int N, int EOS, int RSOL>
 __global__ void __launch_bounds__(TileShape<ND, N>::NT, TileShape<ND, N>::MINB)
@@ -630,68 +669,98 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
       for (int v = 0; v < 5; ++v) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.U0 + v * a.ndof + g0));
     }
   }
-  // 1b. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
-  //     periodic wrap or, at an outflow boundary, the node itself) -> halo rows U | P, asynchronously
-  if (active) {
-    {                                                                // x: one point per line and side
-      const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
-      if (xlo && lc[0] == 0) {
-        const int g = g0 + a.hoff[0][0] + ((org[0] == 0) ? a.hfix[0][0] : 0);
-        DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + fp < TS::NHALO);
-        double* dst = XH + (TS::HOFF(0) + fp);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_copy8(dst + 5 * RS, a.Pin + g);
-      }
-      if (xhi && lc[0] == teff[0] - 1) {
-        const int g = g0 + (SEG - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
-        DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + TS::FP(0) + fp < TS::NHALO);
-        double* dst = XH + (TS::HOFF(0) + TS::FP(0) + fp);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_copy8(dst + 5 * RS, a.Pin + g);
-      }
-    }
-    if constexpr (ND >= 2) {                                         // y: the thread's segment of the line
-      const int fp0 = i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]);
-      if (j == 0 && lc[1] == 0) {
-        const int g = g0 + a.hoff[1][0] + ((org[1] == 0) ? a.hfix[1][0] : 0);
-        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + fp0 + SEG <= TS::NHALO);
-        double* dst = XH + (TS::HOFF(1) + fp0);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
-      }
-      if (j == N - 1 && lc[1] == teff[1] - 1) {
-        const int g = g0 + a.hoff[1][1] + ((org[1] + teff[1] == a.ne[1]) ? a.hfix[1][1] : 0);
-        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + SEG <= TS::NHALO);
-        double* dst = XH + (TS::HOFF(1) + TS::FP(1) + fp0);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+  // 1b. halo -> halo rows U | P, asynchronously.  Even N (16-byte units): the units are dealt to the
+  //     block's threads in flat order (dg_halo_unit), so a warp writes consecutive shared-memory addresses
+  //     and every thread issues the same number of copies (3D p=3: 0.84 fewer wavefronts per node).  Odd N
+  //     (8-byte copies): each boundary thread fetches the layer facing its own nodes, which measured
+  //     3 % faster on the 2D p=2 shear layer.
+  if constexpr (N % 2 == 0) {
+    {
+      constexpr int UW = 2;                                             // 16-byte units along x-lines
+      constexpr int NU0 = 2 * TS::FP(0);
+      constexpr int NU1 = (ND >= 2) ? 2 * TS::FP(1) / UW : 0, NU2 = (ND >= 3) ? 2 * TS::FP(2) / UW : 0;
+      for (int u = t; u < NU0 + NU1 + NU2; u += NT) {
+        if (u < NU0) {
+          const int sd = u / TS::FP(0);
+          dg_halo_unit<ND, N, 0, 1>(a, XH, org, teff, sd, u - sd * TS::FP(0));
+        } else if (ND == 2 || u < NU0 + NU1) {
+          if constexpr (ND >= 2) {
+            constexpr int H = TS::FP(1) / UW;
+            const int w = u - NU0, sd = w / H;
+            dg_halo_unit<ND, N, 1, UW>(a, XH, org, teff, sd, (w - sd * H) * UW);
+          }
+        } else {
+          if constexpr (ND >= 3) {
+            constexpr int H = TS::FP(2) / UW;
+            const int w = u - NU0 - NU1, sd = w / H;
+            dg_halo_unit<ND, N, 2, UW>(a, XH, org, teff, sd, (w - sd * H) * UW);
+          }
+        }
       }
     }
-    if constexpr (ND >= 3) {                                         // z: the thread's segment of the line
-      const int fp0 = i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]);
-      if (k == 0 && lc[2] == 0) {
-        const int g = g0 + a.hoff[2][0] + ((org[2] == 0) ? a.hfix[2][0] : 0);
-        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + fp0 + SEG <= TS::NHALO);
-        double* dst = XH + (TS::HOFF(2) + fp0);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+  } else {
+    // 1b. halo: the facing nodal layer of the neighbouring elements (a.hoff: one element over; a.hfix:
+    //     periodic wrap or, at an outflow boundary, the node itself) -> halo rows U | P, asynchronously
+    if (active) {
+      {                                                                // x: one point per line and side
+        const int fp = ln + TS::NF1 * (lc[1] + TS::TY * lc[2]);
+        if (xlo && lc[0] == 0) {
+          const int g = g0 + a.hoff[0][0] + ((org[0] == 0) ? a.hfix[0][0] : 0);
+          DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + fp < TS::NHALO);
+          double* dst = XH + (TS::HOFF(0) + fp);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_copy8(dst + 5 * RS, a.Pin + g);
+        }
+        if (xhi && lc[0] == teff[0] - 1) {
+          const int g = g0 + (SEG - 1) + a.hoff[0][1] + ((org[0] + teff[0] == a.ne[0]) ? a.hfix[0][1] : 0);
+          DG_ASSERT(g >= 0 && g < a.ndof && TS::HOFF(0) + TS::FP(0) + fp < TS::NHALO);
+          double* dst = XH + (TS::HOFF(0) + TS::FP(0) + fp);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_copy8(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_copy8(dst + 5 * RS, a.Pin + g);
+        }
       }
-      if (k == N - 1 && lc[2] == teff[2] - 1) {
-        const int g = g0 + a.hoff[2][1] + ((org[2] + teff[2] == a.ne[2]) ? a.hfix[2][1] : 0);
-        DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + SEG <= TS::NHALO);
-        double* dst = XH + (TS::HOFF(2) + TS::FP(2) + fp0);
-#pragma unroll
-        for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
-        dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+      if constexpr (ND >= 2) {                                         // y: the thread's segment of the line
+        const int fp0 = i0 + N * k + TS::NF1 * (lc[0] + TS::TX * lc[2]);
+        if (j == 0 && lc[1] == 0) {
+          const int g = g0 + a.hoff[1][0] + ((org[1] == 0) ? a.hfix[1][0] : 0);
+          DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + fp0 + SEG <= TS::NHALO);
+          double* dst = XH + (TS::HOFF(1) + fp0);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+        }
+        if (j == N - 1 && lc[1] == teff[1] - 1) {
+          const int g = g0 + a.hoff[1][1] + ((org[1] + teff[1] == a.ne[1]) ? a.hfix[1][1] : 0);
+          DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(1) + TS::FP(1) + fp0 + SEG <= TS::NHALO);
+          double* dst = XH + (TS::HOFF(1) + TS::FP(1) + fp0);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+        }
+      }
+      if constexpr (ND >= 3) {                                         // z: the thread's segment of the line
+        const int fp0 = i0 + N * j + TS::NF1 * (lc[0] + TS::TX * lc[1]);
+        if (k == 0 && lc[2] == 0) {
+          const int g = g0 + a.hoff[2][0] + ((org[2] == 0) ? a.hfix[2][0] : 0);
+          DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + fp0 + SEG <= TS::NHALO);
+          double* dst = XH + (TS::HOFF(2) + fp0);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+        }
+        if (k == N - 1 && lc[2] == teff[2] - 1) {
+          const int g = g0 + a.hoff[2][1] + ((org[2] + teff[2] == a.ne[2]) ? a.hfix[2][1] : 0);
+          DG_ASSERT(g >= 0 && g + SEG <= a.ndof && TS::HOFF(2) + TS::FP(2) + fp0 + SEG <= TS::NHALO);
+          double* dst = XH + (TS::HOFF(2) + TS::FP(2) + fp0);
+  #pragma unroll
+          for (int v = 0; v < 5; ++v) dg_async_line<SEG>(dst + v * RS, a.Us + v * a.ndof + g);
+          dg_async_line<SEG>(dst + 5 * RS, a.Pin + g);
+        }
       }
     }
   }
-
   // 1c. own nodes -> records
   double R[SEG][5];
 #pragma unroll

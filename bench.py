@@ -41,10 +41,10 @@ DESIGN_BYTES_PER_DOF_STAGE = ALG_BYTES_PER_DOF_STAGE + 16.0
 # per DOF (dram__bytes_read + dram__bytes_write).  Each entry names the capture it comes from; the
 # summaries are under profiles/.  Stale after any kernel change: re-capture (profiles/r2_README.md).
 KERNEL_CONSTANTS = {
-    "box3d": {"flop_per_dof_stage": 487.2, "dram_bytes_per_dof_stage": 135.3,
-              "source": "profiles/r2_ncu_stage_box3d_128.md (capture at 128^3, commit 5f0c1d2+)"},
-    "kh2d": {"flop_per_dof_stage": 445.6, "dram_bytes_per_dof_stage": 114.1,
-             "source": "profiles/r2_ncu_stage_kh2d.md (cold-cache replays: in a timed run the 189 MB state stays in L2)"},
+    "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 135.4,
+              "source": "profiles/r2_ncu_stage_box3d_128.md (capture at 128^3, commit 27b63d4)"},
+    "kh2d": {"flop_per_dof_stage": 449.5, "dram_bytes_per_dof_stage": 114.1,
+             "source": "profiles/r2_ncu_stage_kh2d.md (commit 27b63d4; cold-cache replays: in a timed run most of the 189 MB state stays in L2)"},
 }
 # fp64 peak derived from unit counts: 148 SMs x 64 DFMA/clk/SM x 2 flop x max SM clock; the measured
 # figure (dgrhd_probe_fp64, a register-only DFMA kernel timed in this run) is reported beside it.

@@ -5,8 +5,10 @@
  * (no fast-math, no FMA contraction) [-fopenmp: outer loops over elements / states only, which
  * does not change any arithmetic or summation order].
  *
- * Pins (tests/test_oracle_*.py, -m "not gpu"): every function below is pinned; see DESIGN.md
- * "Oracle pins".  No function here is "parity unpinned".
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): every function the paper prints is pinned; see DESIGN.md
+ * "Oracle pins".  PARITY UNPINNED: orc_shock_limiter (the Moe limiter and the minmod limiter), which the
+ * paper cites (refs [23], [24]) without printing; they are restated in DESIGN.md readings R18 / R19 and
+ * pinned by their properties and special cases only.
  */
 #include "dgrhd_oracle.h"
 #include <math.h>
@@ -711,7 +713,108 @@ void orc_enforce_physicality(const orc_config *c, double *U, unsigned char *flag
  *   5. U <- Ubar_i + theta_i (U - Ubar_i)   (cell averages unchanged; a convex blend of admissible
  *      states, so the physicality operator's result stays admissible).
  * ------------------------------------------------------------------------------------------ */
+/* ------------------------------------------------------------------------------------------
+ * Minmod limiter (PAPER.md:126 "the minmod limiter [24]", :597; ref [24] = van Leer 1979).  NOT
+ * PRINTED IN PAPER.md -- PARITY UNPINNED: restated in DESIGN.md reading R19 as van Leer's minmod
+ * slope ratio in the scaling form of the Moe limiter (a convex blend toward the cell average, so
+ * the physicality operator's result stays admissible), on the five conserved variables w = U:
+ *   1. per cell i: average wbar_i and, per direction d, the cell's linear coefficient
+ *        a_d = sum_n w_n xi_d(n) w(n) / sum_n w_n xi_d(n)^2      (tensor GLL weights, xi in [-1,1]:
+ *      the linear part of w changes by +-a_d from the cell centre to its faces);
+ *   2. neighbour differences D+ = wbar_{i+e_d} - wbar_i, D- = wbar_i - wbar_{i-e_d} (periodic wrap; a
+ *      missing neighbour beyond any other boundary drops out of the minmod);
+ *   3. limited coefficient  a~_d = minmod(a_d, beta D+/2, beta D-/2)  (beta = 1: van Leer's minmod,
+ *      the face value stays within the half difference; beta = 2: the generalised slope limiter of
+ *      the RKDG literature [19-22]);  ratio r_d = a~_d / a_d in [0,1]  (1 where |a_d| is zero to
+ *      rounding, <= 1e-12 max|w| of the cell);
+ *   4. theta_i = min over the variables and directions of r_d, taken as 1 if >= 1 - 1e-12;
+ *   5. U <- Ubar_i + theta_i (U - Ubar_i).
+ * ------------------------------------------------------------------------------------------ */
+static double orc_minmod3(double a, double b, int has_b, double c, int has_c) {
+  double s = (a > 0.0) - (a < 0.0), m = fabs(a);
+  if (s == 0.0) return 0.0;
+  if (has_b) { if (b * s <= 0.0) return 0.0; if (fabs(b) < m) m = fabs(b); }
+  if (has_c) { if (c * s <= 0.0) return 0.0; if (fabs(c) < m) m = fabs(c); }
+  return s * m;
+}
+
+static int64_t orc_minmod_limiter(const orc_config *c, double *U, double *theta_out) {
+  const int nd = c->ndim, N = c->order_p + 1, nn = ipow(N, nd);
+  const int64_t nx = c->nelem[0], ny = nd > 1 ? c->nelem[1] : 1, nz = nd > 2 ? c->nelem[2] : 1;
+  const int64_t ne = nx * ny * nz, ndof = ne * nn;
+  const int64_t nel[3] = {nx, ny, nz};
+  const double beta = (c->moe_alpha > 0.0) ? c->moe_alpha : 1.0;
+  double x[5], w[5], D[25];
+  orc_gll(N, x, w, D);
+  double *st = (double *)malloc(sizeof(double) * 25 * (size_t)ne);   /* mean[5], a[3][5], max|w|[5] */
+#pragma omp parallel for schedule(static)
+  for (int64_t e = 0; e < ne; ++e) {
+    double wsum = 0.0, xx[3] = {0, 0, 0}, mean[5] = {0, 0, 0, 0, 0}, a[3][5] = {{0}}, big[5] = {0, 0, 0, 0, 0};
+    for (int n = 0; n < nn; ++n) {
+      const int idx[3] = {n % N, (n / N) % N, n / (N * N)};
+      double wn = w[idx[0]];
+      if (nd > 1) wn *= w[idx[1]];
+      if (nd > 2) wn *= w[idx[2]];
+      wsum += wn;
+      for (int d = 0; d < nd; ++d) xx[d] += wn * x[idx[d]] * x[idx[d]];
+      for (int v = 0; v < 5; ++v) {
+        double u = U[v * ndof + e * nn + n];
+        mean[v] += wn * u;
+        for (int d = 0; d < nd; ++d) a[d][v] += wn * x[idx[d]] * u;
+        if (fabs(u) > big[v]) big[v] = fabs(u);
+      }
+    }
+    for (int v = 0; v < 5; ++v) {
+      st[e * 25 + v] = mean[v] / wsum;
+      for (int d = 0; d < 3; ++d) st[e * 25 + 5 + 5 * d + v] = (d < nd && N > 1) ? a[d][v] / xx[d] : 0.0;
+      st[e * 25 + 20 + v] = big[v];
+    }
+  }
+  int64_t nlim = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nlim)
+  for (int64_t e = 0; e < ne; ++e) {
+    int64_t ie[3] = {e % nx, (e / nx) % ny, e / (nx * ny)};
+    double theta = 1.0;
+    for (int v = 0; v < 5; ++v) {
+      const double wb = st[e * 25 + v], tiny = 1e-12 * st[e * 25 + 20 + v];
+      for (int d = 0; d < nd; ++d) {
+        const double a = st[e * 25 + 5 + 5 * d + v];
+        if (!(fabs(a) > tiny)) continue;
+        double dif[2] = {0, 0};
+        int has[2] = {0, 0};
+        for (int side = 0; side < 2; ++side) {
+          int64_t je[3] = {ie[0], ie[1], ie[2]};
+          je[d] += side ? 1 : -1;
+          if (je[d] < 0 || je[d] >= nel[d]) {
+            if ((c->bc[d] & 255) != ORC_BC_PERIODIC) continue;
+            je[d] = (je[d] + nel[d]) % nel[d];
+          }
+          int64_t en = je[0] + nx * (je[1] + ny * je[2]);
+          dif[side] = side ? st[en * 25 + v] - wb : wb - st[en * 25 + v];
+          has[side] = 1;
+        }
+        const double al = orc_minmod3(a, 0.5 * beta * dif[1], has[1], 0.5 * beta * dif[0], has[0]);
+        const double r = al / a;
+        if (r < theta) theta = r;
+      }
+    }
+    if (theta >= 1.0 - 1e-12) theta = 1.0;
+    if (theta_out) theta_out[e] = theta;
+    if (theta < 1.0) {
+      nlim++;
+      for (int n = 0; n < nn; ++n)
+        for (int v = 0; v < 5; ++v) {
+          double ub = st[e * 25 + v];
+          U[v * ndof + e * nn + n] = ub + theta * (U[v * ndof + e * nn + n] - ub);
+        }
+    }
+  }
+  free(st);
+  return nlim;
+}
+
 int64_t orc_shock_limiter(const orc_config *c, double *U, double *theta_out) {
+  if (c->shock_limiter == 2) return orc_minmod_limiter(c, U, theta_out);
   const int nd = c->ndim, N = c->order_p + 1, nn = ipow(N, nd);
   const int64_t nx = c->nelem[0], ny = nd > 1 ? c->nelem[1] : 1, nz = nd > 2 ? c->nelem[2] : 1;
   const int64_t ne = nx * ny * nz, ndof = ne * nn;

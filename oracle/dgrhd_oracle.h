@@ -37,10 +37,12 @@ typedef struct {
   int     rk_stages;     /* 1,2,3 */
   double  eps_q, delta_s;
   int     riemann;       /* ORC_RIEMANN_*: interface flux */
-  int     shock_limiter; /* 0 none; 1 the limiter of Moe, Rossmanith & Seal (PAPER.md:126, :551 ref [23]),
-                            applied after the physicality operator of every stage.  PARITY UNPINNED: the
-                            paper cites the limiter without printing it (reading R18) */
-  double  moe_alpha;     /* its tolerance alpha(h) >= 0 (ref [23] suggests ~ 500 h^1.5), absolute */
+  int     shock_limiter; /* 0 none; 1 the limiter of Moe, Rossmanith & Seal (PAPER.md:126, :551 ref [23]);
+                            2 the minmod limiter (PAPER.md:126, :597 ref [24]); applied after the
+                            physicality operator of every stage.  PARITY UNPINNED: the paper cites both
+                            without printing them (readings R18, R19) */
+  double  moe_alpha;     /* Moe: tolerance alpha(h) >= 0 (ref [23] suggests ~ 500 h^1.5), absolute;
+                            minmod: beta in [1,2] (0 = 1) */
   double  bc_state[3][2][5];   /* Dirichlet ghost primitives [axis][side] = rho, ux, uy, uz, P */
 } orc_config;
 

@@ -597,3 +597,78 @@ def test_moe_limiter_keeps_cell_means_leaves_resolved_data_alone_and_bounds_the_
     Wj[0] *= np.where(np.arange(U.shape[1]) % (7 * nn) < 3 * nn + 4, 1.0, 5.0)     # a physical density jump
     Us, _, cnt = O.step(cfg_s, O.prim2con_batch(0, 5.0 / 3.0, Wj), -0.2, 5)
     assert np.isfinite(Us).all() and all(O.admissible(Us[:, i]) for i in range(0, Us.shape[1], 5))
+
+
+# ------------------------------------------------------------------------------------------------
+# Minmod limiter (PAPER.md:126, :597 ref [24] van Leer; reading R19).  The paper does not print it:
+# PARITY UNPINNED.  Pinned here: the special case that reduces to the textbook routine (1D, p = 1, one
+# varying variable: the limited slope is van Leer's minmod of the cell's slope and the two half
+# differences of the neighbouring means, computed independently in numpy), and the properties.
+# ------------------------------------------------------------------------------------------------
+def _mm_cfg(d, beta=0.0):
+    return O.make_config(*[d[k] for k in ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad",
+                                          "rk_stages", "eps_q", "delta_s")], shock_limiter=2, moe_alpha=beta)
+
+
+@pytest.mark.parametrize("beta", [1.0, 2.0])
+def test_minmod_limiter_reduces_to_van_leers_minmod_for_piecewise_linear_data(beta):
+    ne = 40
+    d = I._cfg(1, [ne], [0.0], [1.0], [I.BC_OUTFLOW], 1, 0, 5.0 / 3.0)
+    rng = np.random.default_rng(5)
+    mean = np.cumsum(rng.normal(size=ne)) + 20.0
+    half = rng.normal(size=ne) * 0.7                 # node values mean -+ half (p = 1: nodes at the faces)
+    U = np.ones((5, 2 * ne))
+    U[1:4] = 0.0
+    U[4] = 100.0
+    U[0, 0::2], U[0, 1::2] = mean - half, mean + half
+    U1, th, nlim = O.shock_limiter(_mm_cfg(d, beta), U)
+    dp = np.append(np.diff(mean), np.nan)            # D+ ; no neighbour at the ends
+    dm = np.insert(np.diff(mean), 0, np.nan)
+    exp = np.empty(ne)
+    for i in range(ne):
+        args = [half[i]] + [0.5 * beta * x for x in (dp[i], dm[i]) if not np.isnan(x)]
+        sg = np.sign(args)
+        exp[i] = sg[0] * min(abs(a) for a in args) if (sg == sg[0]).all() else 0.0
+    got = 0.5 * (U1[0, 1::2] - U1[0, 0::2])
+    np.testing.assert_allclose(got, exp, rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(0.5 * (U1[0, 1::2] + U1[0, 0::2]), mean, rtol=1e-14)
+    assert nlim == int((np.abs(exp - half) > 1e-12 * np.abs(half)).sum())
+    np.testing.assert_array_equal(U1[1:], U[1:])
+
+
+def test_minmod_limiter_properties():
+    nd, nel, p = 2, [10, 8], 2
+    N, nn = p + 1, 9
+    d = I._cfg(nd, nel, [0.0, 0.0], [1.0, 1.0], [I.BC_PERIODIC, I.BC_OUTFLOW], p, 0, 5.0 / 3.0)
+    cfg = _mm_cfg(d, 1.0)
+    W, X, _ = _smooth_field(nd, nel, N, [0.0, 0.0], [1.0, 1.0], seed=4)
+    U = O.prim2con_batch(0, 5.0 / 3.0, W)
+    wn = _node_weights(nd, N)
+    U1, th, nlim = O.shock_limiter(cfg, U)
+    # theta in [0,1]; cell means kept; the blend is toward the mean (every node moves toward it)
+    assert (th >= 0.0).all() and (th <= 1.0).all() and nlim == int((th < 1.0).sum())
+    m0 = (U.reshape(5, -1, nn) * wn).sum(-1)
+    m1 = (U1.reshape(5, -1, nn) * wn).sum(-1)
+    np.testing.assert_allclose(m1, m0, rtol=1e-13, atol=1e-13)
+    mean = (m0 / wn.sum())[:, :, None]
+    np.testing.assert_allclose(U1.reshape(5, -1, nn) - mean, th[None, :, None] * (U.reshape(5, -1, nn) - mean),
+                               rtol=1e-12, atol=1e-13)
+    # a cell whose mean is a strict local extremum of some variable in some direction is flattened
+    mD = (m0 / wn.sum())[0].reshape(nel[1], nel[0])
+    ext = (mD > np.roll(mD, 1, 1)) & (mD > np.roll(mD, -1, 1)) | (mD < np.roll(mD, 1, 1)) & (mD < np.roll(mD, -1, 1))
+    assert ext.any() and (th.reshape(nel[1], nel[0])[ext] == 0.0).all()
+    # data that are linear in x and y with every variable (non-periodic box): untouched in every cell;
+    # beta = 2 never limits more than beta = 1; ratios only: invariant under rescaling
+    d2 = I._cfg(nd, nel, [0.0, 0.0], [1.0, 1.0], [I.BC_OUTFLOW, I.BC_OUTFLOW], p, 0, 5.0 / 3.0)
+    Ul = np.stack([3.0 + 1.5 * X[0] - 0.7 * X[1], 0.2 * X[0], -0.1 * X[1], 0.05 * (X[0] + X[1]), 9.0 + X[0] + 2.0 * X[1]])
+    _, thl, nl = O.shock_limiter(_mm_cfg(d2, 1.0), Ul)
+    assert nl == 0 and (thl == 1.0).all()
+    _, th2, _ = O.shock_limiter(_mm_cfg(d, 2.0), U)
+    assert (th2 >= th - 1e-15).all()
+    _, th3, _ = O.shock_limiter(cfg, 3.25 * U)
+    np.testing.assert_allclose(th3, th, rtol=1e-12, atol=1e-15)
+    # idempotent on a limited cell's own slope ratio is not claimed; inside a step it keeps admissibility
+    Wj = W.copy()
+    Wj[0] *= np.where(np.arange(U.shape[1]) % (7 * nn) < 3 * nn + 4, 1.0, 5.0)
+    Us, _, _ = O.step(cfg, O.prim2con_batch(0, 5.0 / 3.0, Wj), -0.2, 5)
+    assert np.isfinite(Us).all() and all(O.admissible(Us[:, i]) for i in range(0, Us.shape[1], 5))

@@ -51,9 +51,11 @@ enum { DGRHD_RIEMANN_HLL = 0, DGRHD_RIEMANN_HLLC = 1 };
 /* Shock limiter: none, or the limiter of Moe, Rossmanith & Seal (ref [23]):
  * every cell is rescaled toward its average by theta = min(1, phi((M - wbar)/(w_M - wbar)), phi((m - wbar)/
  * (w_m - wbar))) over the five conserved variables, phi(y) = min(y/1.1, 1), with M, m the extrema of the face
- * neighbours' nodal values widened to wbar +- alpha.  The paper cites it without printing it (DESIGN.md
- * reading R18). */
-enum { DGRHD_SHOCK_LIMITER_NONE = 0, DGRHD_SHOCK_LIMITER_MOE = 1 };
+ * neighbours' nodal values widened to wbar +- alpha; or the minmod limiter (ref [24], van Leer) in the same scaling
+ * form: theta = min over variables and directions of minmod(a_d, beta D+/2, beta D-/2) / a_d, a_d the cell's linear
+ * coefficient along d, D+- the differences of the neighbouring cell averages.  The paper cites both without printing
+ * them (readings R18, R19). */
+enum { DGRHD_SHOCK_LIMITER_NONE = 0, DGRHD_SHOCK_LIMITER_MOE = 1, DGRHD_SHOCK_LIMITER_MINMOD = 2 };
 enum { DGRHD_OK = 0, DGRHD_EINVAL = 1, DGRHD_ENOMEM = 2, DGRHD_ECUDA = 3, DGRHD_ESTATE = 4 };
 
 /* Problem statement: mesh, order, EOS. */
@@ -71,7 +73,8 @@ typedef struct {
   int     riemann;         /* DGRHD_RIEMANN_*                                                       */
   int     shock_limiter;   /* DGRHD_SHOCK_LIMITER_*: applied after the physicality operator of every
                               stage of dgrhd_step (two extra small launches per stage)              */
-  double  moe_alpha;       /* tolerance alpha(h) >= 0 of the Moe limiter (ref [23] suggests ~500 h^1.5) */
+  double  moe_alpha;       /* Moe: tolerance alpha(h) >= 0 (ref [23] suggests ~500 h^1.5); minmod: beta in
+                              [1,2] (1 = van Leer's minmod, 2 = generalised slope limiter; 0 means 1)   */
   double  bc_state[3][2][5]; /* Dirichlet ghost primitives [axis][end] = rho, ux, uy, uz, P          */
 } dgrhd_config;
 
@@ -117,7 +120,7 @@ int dgrhd_rhs(dgrhd_ctx* ctx, const double* U_dev, double* R_dev);
 int dgrhd_enforce_physicality(dgrhd_ctx* ctx, double* U_dev, unsigned char* flag_dev,
                               double* s_dev, int64_t counters_host[2]);
 
-/* The shock limiter the context was created with (DGRHD_SHOCK_LIMITER_MOE), in place on U_dev[5][ndof];
+/* The shock limiter the context was created with (DGRHD_SHOCK_LIMITER_MOE or _MINMOD), in place on U_dev[5][ndof];
  * theta_dev[n_elem] (or NULL) receives every cell's rescaling factor (1 = untouched).  ESTATE if the
  * context has no shock limiter.  Inside dgrhd_step it runs after the physicality operator of every stage. */
 int dgrhd_shock_limiter(dgrhd_ctx* ctx, double* U_dev, double* theta_dev);

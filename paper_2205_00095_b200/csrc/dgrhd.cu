@@ -63,7 +63,8 @@ bool valid_cfg(const dgrhd_config* c) {
     }
   }
   if (c->riemann != DGRHD_RIEMANN_HLL && c->riemann != DGRHD_RIEMANN_HLLC) return false;
-  if (c->shock_limiter != DGRHD_SHOCK_LIMITER_NONE && c->shock_limiter != DGRHD_SHOCK_LIMITER_MOE) return false;
+  if (c->shock_limiter != DGRHD_SHOCK_LIMITER_NONE && c->shock_limiter != DGRHD_SHOCK_LIMITER_MOE &&
+      c->shock_limiter != DGRHD_SHOCK_LIMITER_MINMOD) return false;
   if (!(c->moe_alpha >= 0.0)) return false;
   if (c->order_p < 0 || c->order_p > 4) return false;
   if (c->eos != DGRHD_EOS_IDEAL && c->eos != DGRHD_EOS_TAUB_MATTHEWS) return false;
@@ -238,17 +239,32 @@ static cudaError_t launch_moe_nd(dgrhd_ctx* c, double* U, double* P, int do_cfl,
     mp.periodic[d] = (d < c->cfg.ndim && (c->cfg.bc[d] & 255) == DGRHD_BC_PERIODIC) ? 1 : 0;
     mp.cw[d] = (d < c->cfg.ndim) ? (2.0 * c->cfg.order_p + 1.0) * (double)c->cfg.nelem[d] / (c->cfg.xmax[d] - c->cfg.xmin[d]) : 0.0;
   }
-  mp.alpha = c->cfg.moe_alpha;
+  const bool minmod = (c->cfg.shock_limiter == DGRHD_SHOCK_LIMITER_MINMOD);
+  mp.alpha = minmod ? (c->cfg.moe_alpha > 0.0 ? c->cfg.moe_alpha : 1.0) : c->cfg.moe_alpha;
+  MmPar mm;
+  {
+    double sxx = 0.0, sw = 0.0;
+    for (int i = 0; i < 5; ++i) mm.x[i] = (i < c->N) ? c->basis.x[i] : 0.0;
+    for (int i = 0; i < c->N; ++i) { sxx += c->basis.w[i] * c->basis.x[i] * c->basis.x[i]; sw += c->basis.w[i]; }
+    for (int d = 1; d < c->cfg.ndim; ++d) sxx *= sw;
+    mm.rxx = (sxx > 0.0) ? 1.0 / sxx : 0.0;
+  }
   mp.do_cfl = do_cfl;
 #define DG_GO(NV)                                                                                       \
   {                                                                                                     \
     constexpr int EPB = 4 * TileShape<ND, NV>::EPW;                                                     \
     const unsigned nb = (unsigned)((c->nelem + EPB - 1) / EPB);                                         \
-    dg_moe_stats_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, c->moe_stats, lp);     \
-    if (c->cfg.eos == DGRHD_EOS_IDEAL)                                                                  \
-      dg_moe_apply_kernel<ND, NV, 0><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+    if (minmod)                                                                                         \
+      dg_mm_stats_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, c->moe_stats, lp, mm); \
     else                                                                                                \
-      dg_moe_apply_kernel<ND, NV, 1><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+      dg_moe_stats_kernel<ND, NV><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, c->moe_stats, lp);   \
+    if (c->cfg.eos == DGRHD_EOS_IDEAL) {                                                                \
+      if (minmod) dg_moe_apply_kernel<ND, NV, 0, 1><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+      else dg_moe_apply_kernel<ND, NV, 0, 0><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+    } else {                                                                                            \
+      if (minmod) dg_moe_apply_kernel<ND, NV, 1, 1><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+      else dg_moe_apply_kernel<ND, NV, 1, 0><<<nb, 128, 0, c->stream>>>(c->nelem, c->ndof, U, P, c->moe_stats, mp, c->eos, amax, counters, theta); \
+    }                                                                                                   \
   }
   switch (c->N) {
     case 1: DG_GO(1) break;
@@ -329,7 +345,7 @@ static void fill_stage_args(dgrhd_ctx* c, StageArgs& a) {
 // ------------------------------------------------------------------------------------------------
 static size_t pbuf_bytes(long long ndof) { return align_up((size_t)ndof * sizeof(double)); }
 static size_t moe_bytes(const dgrhd_config* cfg, long long ne) {
-  return cfg->shock_limiter ? align_up((size_t)ne * 15 * sizeof(double)) : 0;
+  return cfg->shock_limiter ? align_up((size_t)ne * 25 * sizeof(double)) : 0;   // Moe uses 15, minmod 25 per cell
 }
 
 extern "C" size_t dgrhd_workspace_bytes(const dgrhd_config* cfg) {
@@ -493,7 +509,7 @@ extern "C" int dgrhd_enforce_physicality(dgrhd_ctx* c, double* U_dev, unsigned c
 
 extern "C" int dgrhd_shock_limiter(dgrhd_ctx* c, double* U_dev, double* theta_dev) {
   if (!c || !U_dev) return fail(c, DGRHD_EINVAL, "dgrhd_shock_limiter: NULL argument");
-  if (c->cfg.shock_limiter != DGRHD_SHOCK_LIMITER_MOE)
+  if (c->cfg.shock_limiter == DGRHD_SHOCK_LIMITER_NONE)
     return fail(c, DGRHD_ESTATE, "dgrhd_shock_limiter: the context was created without a shock limiter");
   if (!aligned16(U_dev)) return fail(c, DGRHD_EINVAL, "dgrhd_shock_limiter: state pointer must be 16-byte aligned");
   // (the pressure of the rescaled cells lands in the spare pressure buffer; no counters, no CFL)
@@ -558,7 +574,7 @@ static int enqueue_step(dgrhd_ctx* c, double dt, StageArgs& a) {
     }
     a.Pin = c->P[c->par];
     a.Pout = c->P[c->par ^ 1];
-    const bool moe = (c->cfg.shock_limiter == DGRHD_SHOCK_LIMITER_MOE);
+    const bool moe = (c->cfg.shock_limiter != DGRHD_SHOCK_LIMITER_NONE);
     a.do_cfl = (last && !moe) ? 1 : 0;                     // with the shock limiter: taken from the limited state
     DG_CUDA(c, launch_stage(c, a));
     if (moe) DG_CUDA(c, launch_moe(c, a.Uout, a.Pout, last ? 1 : 0, c->sc->amax, c->sc->counters, nullptr));

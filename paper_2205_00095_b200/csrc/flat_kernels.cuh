@@ -206,7 +206,8 @@ dg_limiter_kernel(long long nelem, long long ndof, double* U, unsigned char* fla
 //                         other boundary) and the tolerance alpha; theta = min(1, phi(.)) over all
 //                         variables, phi(y) = min(y/1.1, 1); U <- Ubar + theta (U - Ubar) in the limited
 //                         cells, whose pressure is recovered again; on the step's last stage the CFL
-//                         maximum is taken here, from the limited state.
+//                         maximum is taken here, from the limited state.  LIMK = 1: theta of the
+//                         minmod limiter (dg_mm_theta, statistics of dg_mm_stats_kernel) instead.
 // ---------------------------------------------------------------------------------------------
 template <int NL>
 DG_INL double dg_cell_max(double x, int base) {
@@ -261,15 +262,108 @@ dg_moe_stats_kernel(long long nelem, long long ndof, const double* __restrict__ 
   }
 }
 
+// Minmod limiter (PAPER.md:126, :597 ref [24]; reading R19: cited, not printed): statistics per
+// cell and conserved variable -> stats[n_e][25] = average[5] | linear coefficients a_d[3][5] | max|w|[5],
+//   a_d = sum_n w_n xi_d(n) w(n) / sum_n w_n xi_d(n)^2   (tensor GLL weights; rxx = 1 / that denominator).
+struct MmPar {
+  double x[5];      // GLL nodes on [-1,1]
+  double rxx;
+};
+
+template <int ND, int N>
+__global__ void __launch_bounds__(128)
+dg_mm_stats_kernel(long long nelem, long long ndof, const double* __restrict__ U, double* __restrict__ stats,
+                   LimPar lp, MmPar mm) {
+  using TS = TileShape<ND, N>;
+  constexpr int NN = TS::NN, NL = TS::NL, EPW = TS::EPW, SEG = TS::SEG, NSEG = TS::NSEG;
+  const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+  const int ew = lane / NL, lt = lane - ew * NL;
+  const int h = lt % NSEG, ln = lt / NSEG;
+  const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
+  const bool active = (ew < EPW) && (e < nelem);
+  const int j = (ND >= 2) ? ln % N : 0, k = (ND >= 3) ? ln / N : 0;
+  const long long g0 = (active ? e : 0) * NN + N * ln + h * SEG;
+  const int base = ew * NL;
+  double wl = 1.0;
+  if (ND >= 2) wl *= lp.w[j];
+  if (ND >= 3) wl *= lp.w[k];
+  const double xy = (ND >= 2) ? mm.x[j] : 0.0, xz = (ND >= 3) ? mm.x[k] : 0.0;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    double x[SEG];
+    dg_ld_line<SEG>(U + v * ndof + g0, x);
+    double pm = 0.0, px = 0.0, big = 0.0;
+#pragma unroll
+    for (int m = 0; m < SEG; ++m) {
+      const int i = (NSEG > 1 && h > 0) ? (SEG + m) % 5 : m;
+      const double wq = wl * lp.w[i];
+      pm = fma(wq, x[m], pm);
+      px = fma(wq * mm.x[i], x[m], px);
+      big = fmax(big, fabs(x[m]));
+    }
+    const double mean = dg_cell_sum<NL>(pm, base) / lp.wsum;
+    const double ax = dg_cell_sum<NL>(px, base) * mm.rxx;
+    const double ay = (ND >= 2) ? dg_cell_sum<NL>(pm * xy, base) * mm.rxx : 0.0;
+    const double az = (ND >= 3) ? dg_cell_sum<NL>(pm * xz, base) * mm.rxx : 0.0;
+    big = dg_cell_max<NL>(big, base);
+    if (active && lt == 0) {
+      stats[e * 25 + v] = mean;
+      stats[e * 25 + 5 + v] = (N > 1) ? ax : 0.0;
+      stats[e * 25 + 10 + v] = (N > 1) ? ay : 0.0;
+      stats[e * 25 + 15 + v] = (N > 1) ? az : 0.0;
+      stats[e * 25 + 20 + v] = big;
+    }
+  }
+}
+
+// theta of the minmod limiter for cell e (reading R19): min over variables and directions of
+// minmod(a_d, beta D+/2, beta D-/2) / a_d, D+- the differences of the neighbouring cell averages
+// (periodic wrap; a missing neighbour drops out); 1 if >= 1 - 1e-12.
+template <int ND>
+DG_INL double dg_mm_theta(const double* __restrict__ stats, long long e, const long long ne[3], const int periodic[3],
+                          double beta, double mean[5]) {
+  const long long ie[3] = {e % ne[0], (e / ne[0]) % ne[1], e / (ne[0] * ne[1])};
+  const long long es[3] = {1, ne[0], ne[0] * ne[1]};
+  double theta = 1.0;
+#pragma unroll
+  for (int v = 0; v < 5; ++v) {
+    const double wb = stats[e * 25 + v], tiny = 1e-12 * stats[e * 25 + 20 + v];
+    mean[v] = wb;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+      const double a = stats[e * 25 + 5 + 5 * d + v];
+      if (!(fabs(a) > tiny)) continue;
+      const double sg = (a > 0.0) ? 1.0 : -1.0;
+      double m = fabs(a);
+      bool zero = false;
+#pragma unroll
+      for (int side = 0; side < 2; ++side) {
+        long long jd = ie[d] + (side ? 1 : -1);
+        if (jd < 0 || jd >= ne[d]) {
+          if (!periodic[d]) continue;
+          jd = (jd + ne[d]) % ne[d];
+        }
+        const double wn = stats[(e + (jd - ie[d]) * es[d]) * 25 + v];
+        const double b = 0.5 * beta * (side ? wn - wb : wb - wn);
+        if (b * sg <= 0.0) zero = true;
+        m = fmin(m, fabs(b));
+      }
+      const double r = zero ? 0.0 : (sg * m) / a;
+      theta = fmin(theta, r);
+    }
+  }
+  return (theta >= 1.0 - 1e-12) ? 1.0 : theta;
+}
+
 struct MoePar {
   long long ne[3];
   int periodic[3];
-  double alpha;
+  double alpha;          // Moe: tolerance alpha; minmod: beta
   double cw[3];
   int do_cfl;
 };
 
-template <int ND, int N, int EOS>
+template <int ND, int N, int EOS, int LIMK>
 __global__ void __launch_bounds__(128)
 dg_moe_apply_kernel(long long nelem, long long ndof, double* U, double* P, const double* __restrict__ stats,
                     MoePar mp, EosPar eos, dg_ull* amax, dg_ull* counters, double* theta_out) {
@@ -282,7 +376,8 @@ dg_moe_apply_kernel(long long nelem, long long ndof, double* U, double* P, const
   const bool active = (ew < EPW) && (e < nelem);
   const long long g0 = (active ? e : 0) * NN + N * ln + h * SEG;
   double theta = 1.0, mean[5] = {0, 0, 0, 0, 0};
-  if (active) {
+  if (active && LIMK == 1) theta = dg_mm_theta<ND>(stats, e, mp.ne, mp.periodic, mp.alpha, mean);
+  if (active && LIMK == 0) {
     const long long ie[3] = {e % mp.ne[0], (e / mp.ne[0]) % mp.ne[1], e / (mp.ne[0] * mp.ne[1])};
     const long long es[3] = {1, mp.ne[0], mp.ne[0] * mp.ne[1]};
 #pragma unroll

@@ -243,3 +243,45 @@ def test_paper_riemann_problems_with_the_shock_limiter_match_oracle(k):
           f"{cnt_o[0]} / {c['n_flagged']}, cells rescaled by the shock limiter {c['n_shock_limited']}")
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to and c["n_shock_limited"] > 0
     assert err.max() <= 1e-8
+
+
+# ------------------------------------------------------------------------------------------------
+# f2: the minmod limiter (reading R19; cited, not printed, by the paper) -- same harness as the Moe limiter
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("beta", [0.0, 2.0])
+@pytest.mark.parametrize("nd,nelem,p,eos,G,bc", MOE_CASES)
+def test_minmod_limiter_matches_oracle_cell_by_cell(nd, nelem, p, eos, G, bc, beta):
+    d = mesh(nd, nelem, p, eos, G, bc, shock_limiter=2, moe_alpha=beta)
+    nn = (p + 1) ** nd
+    W = smooth_prims(d, seed=60 + nd + p)
+    W[0] *= np.where((np.arange(W.shape[1]) // nn) % 5 < 2, 1.0, 6.0)
+    W[4] *= np.where(np.arange(W.shape[1]) % (3 * nn) < nn + nn // 2, 1.0, 3.0)
+    U = O.prim2con_batch(eos, G, W)
+    Uo, th_o, n_o = O.shock_limiter(ocfg(d), U)
+    ctx = B().Context(gcfg(d))
+    Ug = to_dev(U)
+    th_g = ctx.dgrhd_shock_limiter(Ug).cpu().numpy()
+    assert (n_o > 0) or p == 0
+    # theta is a ratio of rounded sums: a cell sitting exactly on the 1 - 1e-12 switch may fall either way
+    marginal = np.abs(th_o - 1.0) < 1e-10
+    assert np.array_equal((th_g < 1.0)[~marginal], (th_o < 1.0)[~marginal])
+    np.testing.assert_allclose(th_g, th_o, rtol=1e-10, atol=1e-12)
+    scale = np.abs(Uo).max(axis=0) + 1e-300
+    assert np.max(np.abs(Ug.cpu().numpy() - Uo) / scale) <= 1e-10
+
+
+def test_paper_riemann_problem_with_the_minmod_limiter_matches_oracle():
+    """the minmod limiter as the alternative to the Moe limiter on the shock tests (Sod, p = 1)."""
+    d, W, _ = I.paper_riemann1d(4, ne=128, p=1, riemann=I.RIEMANN_HLLC)
+    d = dict(d, shock_limiter=2, moe_alpha=1.0)
+    U = O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy())
+    Uo, to, cnt_o = O.step(ocfg(d), U, -0.2, 30)
+    ctx = B().Context(gcfg(d))
+    ctx.dgrhd_set_state(to_dev(U))
+    tg = ctx.dgrhd_step(-0.2, 30, t=0.0)
+    Ug = ctx.dgrhd_get_state().cpu().numpy()
+    c = ctx.dgrhd_get_counters()
+    err = relmax(Ug, Uo)[[0, 1, 4]]
+    print(f"paper Riemann problem 4 + minmod limiter: max-norm rel. diff {err.max():.2e}, cells rescaled {c['n_shock_limited']}")
+    assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to and c["n_shock_limited"] > 0
+    assert err.max() <= 1e-8

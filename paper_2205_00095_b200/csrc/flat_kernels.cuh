@@ -35,8 +35,10 @@ __device__ __forceinline__ void dg_block_atomic_max(double x, double* sRed, dg_u
 }
 
 // NS = 2: n even and U, W 16-byte aligned (checked by the host); NS = 1: any n / alignment.
+// Resident blocks per SM (measured at 2^26 states): the ideal-EOS solve wants 80 registers (no spills, 3 blocks:
+// 0.86 of HBM against 0.82 with 4 blocks and 64 registers), the Taub-Matthews solve fits 64 (4 blocks: 0.86).
 template <int EOS, int NS>
-__global__ void __launch_bounds__(DG_FLAT_NT, 4)
+__global__ void __launch_bounds__(DG_FLAT_NT, (EOS == DG_EOS_IDEAL) ? 3 : 4)
 dg_c2p_batch_kernel(long long n, const double* __restrict__ U, double* __restrict__ W,
                     int* __restrict__ status, EosPar eos) {
   const long long i = ((long long)blockIdx.x * DG_FLAT_NT + threadIdx.x) * NS;

@@ -43,8 +43,8 @@ DESIGN_BYTES_PER_DOF_STAGE = ALG_BYTES_PER_DOF_STAGE + 16.0
 KERNEL_CONSTANTS = {
     "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 135.4,
               "source": "profiles/r2_ncu_stage_box3d_128.md (capture at 128^3, commit 27b63d4)"},
-    "kh2d": {"flop_per_dof_stage": 449.5, "dram_bytes_per_dof_stage": 114.1,
-             "source": "profiles/r2_ncu_stage_kh2d.md (commit 27b63d4; cold-cache replays: in a timed run most of the 189 MB state stays in L2)"},
+    "kh2d": {"flop_per_dof_stage": 449.7, "dram_bytes_per_dof_stage": 114.3,
+             "source": "profiles/r2_ncu_stage_kh2d.md (96 registers / 5 blocks per SM; cold-cache replays: in a timed run most of the 189 MB state stays in L2)"},
 }
 # fp64 peak derived from unit counts: 148 SMs x 64 DFMA/clk/SM x 2 flop x max SM clock; the measured
 # figure (dgrhd_probe_fp64, a register-only DFMA kernel timed in this run) is reported beside it.

@@ -1,0 +1,71 @@
+"""Randomised parity: seeded random configurations -- dimension, ragged mesh sizes against the tile
+shapes, order p = 0..4, both EOS, HLL / HLLC, a different boundary condition at every axis end
+(periodic, outflow, wall, Dirichlet), no / Moe / minmod shock limiter, RK1 / SSPRK2 / SSPRK3 -- on smooth
+or jumpy seeded fields, half of them with a log-normal density contrast that drives the physicality
+operator: the residual L(U) and three limited steps against the oracle."""
+import numpy as np
+import pytest
+
+import oracle as O
+from _util import B, gcfg, mesh, ocfg, relmax, smooth_prims, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def random_case(rng, it):
+    nd = int(rng.integers(1, 4))
+    p = int(rng.integers(0, 5))
+    eos = int(rng.integers(0, 2))
+    G = [5 / 3, 4 / 3][int(rng.integers(0, 2))] if eos == 0 else 0.0
+    nelem = [int(rng.integers(1, {1: 90, 2: 23, 3: 9}[nd] + 1)) for _ in range(nd)]
+    bc, bcs = [], {}
+    for d in range(nd):
+        if int(rng.integers(0, 4)) == 0:
+            bc.append(0)
+            continue
+        lo, hi = int(rng.integers(1, 4)), int(rng.integers(1, 4))
+        bc.append((lo, hi))
+        for side, kk in ((0, lo), (1, hi)):
+            if kk == 3:
+                u = rng.uniform(-0.5, 0.5, 3) * np.array([1, nd > 1, nd > 2])
+                bcs[(d, side)] = [float(rng.uniform(0.5, 2)), *[float(x) for x in u], float(rng.uniform(0.3, 1.5))]
+    lim = int(rng.integers(0, 3))
+    d = mesh(nd, nelem, p, eos, G, bc, riemann=int(rng.integers(0, 2)), bc_state=bcs or None, shock_limiter=lim,
+             moe_alpha=[0.0, 1e-3, float(rng.uniform(1, 2))][lim], rk_stages=int(rng.integers(1, 4)))
+    W = smooth_prims(d, seed=1000 + it, amp=float(rng.uniform(0.1, 0.45)))
+    nn = (p + 1) ** nd
+    if rng.random() < 0.5:                            # jumps between and inside cells
+        W[0] *= np.where((np.arange(W.shape[1]) // nn) % 5 < 2, 1.0, float(rng.uniform(2, 8)))
+        W[4] *= np.where(np.arange(W.shape[1]) % (3 * nn) < nn + nn // 2, 1.0, float(rng.uniform(1.5, 4)))
+    if rng.random() < 0.5:                            # near-vacuum nodes: the physicality operator fires
+        W[0] *= np.exp(2.0 * rng.normal(size=W.shape[1]) * (rng.random(W.shape[1]) < 0.2))
+        W[4] = 0.02 * W[0]
+    return d, W
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14])
+def test_random_configurations_match_oracle(seed):
+    rng = np.random.default_rng(seed)
+    n_lim = n_shock = 0
+    for it in range(40):
+        d, W = random_case(rng, it)
+        U = O.prim2con_batch(d["eos"], d["gamma_ad"], W)
+        tag = {k: d[k] for k in ("ndim", "nelem", "order_p", "eos", "bc", "riemann", "shock_limiter", "rk_stages")}
+        Ro, _ = O.rhs(ocfg(d), U)
+        ctx = B().Context(gcfg(d))
+        Rg = ctx.dgrhd_rhs(to_dev(U)).cpu().numpy()
+        act = np.max(np.abs(Ro), axis=1) > 1e-9
+        assert (relmax(Rg, Ro)[act] <= 1e-11).all(), (it, tag)
+        Uo, to, cnt = O.step(ocfg(d), U, -0.25, 3)
+        ctx.dgrhd_set_state(to_dev(U))
+        tg = ctx.dgrhd_step(-0.25, 3, t=0.0)
+        Ug = ctx.dgrhd_get_state().cpu().numpy()
+        c = ctx.dgrhd_get_counters()
+        assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-11 * to, (it, tag)
+        assert c["n_flagged"] == cnt[0] and c["n_bad_mean"] == cnt[1], (it, tag, c, cnt)
+        assert relmax(Ug, Uo).max() <= 1e-9, (it, tag, relmax(Ug, Uo))
+        n_lim += cnt[0] > 0
+        n_shock += c["n_shock_limited"] > 0
+        ctx.close()
+    print(f"seed {seed}: 40 configurations, physicality operator active in {n_lim}, shock limiter active in {n_shock}")
+    assert n_lim >= 5 and n_shock >= 5

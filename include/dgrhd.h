@@ -110,6 +110,47 @@ int dgrhd_get_prims(dgrhd_ctx* ctx, double* W_dev);
  * state.  U_dev and R_dev must not overlap. */
 int dgrhd_rhs(dgrhd_ctx* ctx, const double* U_dev, double* R_dev);
 
+/* R = L(U) for callers that cannot allocate device memory: the same operator, kernels and results as
+ * dgrhd_rhs (Eq. 15-18), but with no context and no caller workspace.
+ *
+ * Who this is for.  dgrhd_rhs needs a context, and a context needs a workspace the caller got from
+ * cudaMalloc (or from a pool that did).  Some callers have no way to get one at the point where they
+ * need the residual: a plug-in inside a host application that has already handed (almost) all of the
+ * GPU's memory to its own arena, so that a fresh cudaMalloc fails; a process whose device-memory budget
+ * was fixed by its operator up front (an MPS client with a memory limit, a multi-tenant job) and is
+ * spent; a latency-critical loop that must not take the device-wide synchronisation and the driver
+ * locks that cudaMalloc / cudaFree bring with them.  For them the scratch
+ * this operator needs (the pressure of every node, Eq. 16, between its two kernels, plus a few KiB of
+ * failure counters) lives in ONE array compiled into the library, a file-scope __device__ array of
+ * 12544 + 8 * DGRHD_STATIC_MAX_NDOF bytes (about 8 MiB).  Every GPU on which the library's code is
+ * loaded holds that array from load until the process exits, whether or not this call is ever made.
+ *
+ * The caller still passes the input U_dev[5][ndof] and the output R_dev[5][ndof] (canonical layout, device
+ * pointers, 16-byte aligned, not overlapping; the caller's own memory).  cfg describes the mesh as for
+ * dgrhd_create (rk_stages, shock_limiter and the physicality knobs are checked but play no part in L).
+ * n_c2p_fail_host (or NULL) receives the number of nodes of THIS call whose recovery failed; non-NULL
+ * makes the call synchronise cuda_stream, NULL leaves it asynchronous.
+ *
+ * Limit: ndof = nelem_total * (p+1)^ndim <= DGRHD_STATIC_MAX_NDOF.  A larger mesh is refused with
+ * DGRHD_ENOMEM and a message that names both numbers; nothing is launched.  Other errors as dgrhd_rhs
+ * (EINVAL for a bad configuration, NULL, misaligned or overlapping pointers; ECUDA).
+ *
+ * The call itself allocates nothing: no cudaMalloc, cudaFree, stream, event or graph, and no host heap
+ * memory.  The first call on each device does a one-time set-up with that device current: it asks the
+ * runtime for the device address of the array (the array's name in host code is only a handle, never a
+ * pointer a kernel may be given) and opts the stage kernel into its shared-memory size.  Make that first
+ * call per device before any stream capture begins; later calls on that device only enqueue a 12 KiB
+ * memset of the counters and two kernels.
+ *
+ * All calls on a device share the one array and it keeps what the previous call left in it.  The call
+ * clears the counters itself and overwrites every pressure value before reading it, so calls that run
+ * one after another (same stream, or ordered by events) are independent of each other.  Two calls
+ * whose kernels can overlap on the GPU (different streams without ordering, or different host threads
+ * on different streams) race on the array and both results are undefined: serialise them. */
+#define DGRHD_STATIC_MAX_NDOF 1048576
+int dgrhd_rhs_static(const dgrhd_config* cfg, const double* U_dev, double* R_dev,
+                     int64_t* n_c2p_fail_host, void* cuda_stream);
+
 /* The physicality-enforcing operator of PAPER.md:175-254 (Eq. 25-37), in place on U_dev[5][ndof]
  * (NULL = the internal state, whose primitives are then refreshed): per cell, blend toward the
  * volume average with the largest s in [0,1] that makes every node admissible (D > 0,

@@ -70,7 +70,7 @@ EXPORTS = ("dgrhd_workspace_bytes", "dgrhd_create", "dgrhd_destroy", "dgrhd_set_
            "dgrhd_get_state", "dgrhd_get_prims", "dgrhd_rhs", "dgrhd_enforce_physicality",
            "dgrhd_cfl_dt", "dgrhd_step", "dgrhd_get_counters", "dgrhd_con2prim_batch",
            "dgrhd_prim2con_batch", "dgrhd_con2prim_batch_host", "dgrhd_run_host", "dgrhd_tm_fallback_count", "dgrhd_probe_fp64", "dgrhd_con2prim_batch_variant", "dgrhd_shock_limiter",
-           "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version")
+           "dgrhd_set_option", "dgrhd_last_error", "dgrhd_version", "dgrhd_rhs_static")
 
 
 def lib():
@@ -90,6 +90,7 @@ def lib():
         L.dgrhd_get_state.argtypes = [_vp, _vp]
         L.dgrhd_get_prims.argtypes = [_vp, _vp]
         L.dgrhd_rhs.argtypes = [_vp, _vp, _vp]
+        L.dgrhd_rhs_static.argtypes = [C.POINTER(Config), _vp, _vp, _i64p, _vp]
         L.dgrhd_enforce_physicality.argtypes = [_vp, _vp, _vp, _vp, _i64p]
         L.dgrhd_cfl_dt.argtypes = [_vp, _vp, C.c_double, _dp]
         L.dgrhd_shock_limiter.argtypes = [_vp, _vp, _vp]
@@ -241,6 +242,25 @@ class Context:
         _check(lib().dgrhd_get_counters(self._h, out, int(reset)), self._h)
         return dict(n_flagged=out[0], n_bad_mean=out[1], n_c2p_fail=out[2], n_stages=out[3],
                     n_tm_fallback=out[4], n_bad_dt=out[5], n_shock_limited=out[6])
+
+
+STATIC_MAX_NDOF = 1 << 20          # DGRHD_STATIC_MAX_NDOF of include/dgrhd.h
+
+
+def dgrhd_rhs_static(cfg, U, out=None, count_failures=True):
+    """R = L(U) through the entry point that needs no context and no workspace: its scratch is an array
+    built into libdgrhd.so (at most STATIC_MAX_NDOF nodes; a larger mesh raises DgrhdError ENOMEM).  It is
+    meant for callers that cannot allocate device memory at that point (a plug-in whose host application
+    owns all of the GPU's memory, a process with a spent memory budget, a loop that must not stall on
+    cudaMalloc); the C call allocates nothing.  This wrapper only marshals: when `out` is None it asks
+    torch for the output tensor, so pass your own `out` if torch must not allocate either.  Calls share the
+    one array: do not let two of them overlap on the GPU.  Returns (R, n_c2p_fail of this call), or
+    (R, None) without synchronising when count_failures is False."""
+    out = torch.empty_like(U) if out is None else out
+    nfail = C.c_int64(-1)
+    _check(lib().dgrhd_rhs_static(C.byref(cfg), _ptr(U, 5), _ptr(out, 5),
+                                  C.byref(nfail) if count_failures else None, _stream()))
+    return out, (int(nfail.value) if count_failures else None)
 
 
 def dgrhd_con2prim_batch(eos, gamma_ad, U, W=None, status=None):

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "basis.h"
@@ -480,6 +481,120 @@ extern "C" int dgrhd_rhs(dgrhd_ctx* c, const double* U_dev, double* R_dev) {
   a.Pin = Ptmp;
   a.Rout = R_dev;
   DG_CUDA(c, launch_stage(c, a));
+  return DGRHD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// R = L(U) without a context or a workspace (dgrhd_rhs_static, include/dgrhd.h): for callers that
+// cannot obtain device memory.  Same two kernels as dgrhd_rhs; their scratch -- the device scalars
+// (of which MODE_RHS touches only the counter slots) followed by the nodal pressure -- is the array
+// below, which every GPU that loads this translation unit's code holds until the process exits.
+//
+// In host code the name g_rhs_static_scratch is a handle for the runtime's symbol calls, NOT a device
+// address: handing it to a kernel would fault or, where the GPU can reach host memory, quietly use the
+// wrong memory.  The device address comes from cudaGetSymbolAddress, asked once per device with that
+// device current (each device has its own copy of the array), under a mutex, and cached.
+// ------------------------------------------------------------------------------------------------
+namespace {
+constexpr size_t STATIC_HEAD_BYTES = (sizeof(DevScalars) + ALIGN - 1) / ALIGN * ALIGN;
+static_assert(STATIC_HEAD_BYTES == 12544, "include/dgrhd.h states this size");
+static_assert(STATIC_HEAD_BYTES % sizeof(double) == 0, "the pressure rows follow the head");
+constexpr size_t STATIC_WORDS = STATIC_HEAD_BYTES / sizeof(double) + (size_t)DGRHD_STATIC_MAX_NDOF;
+constexpr int STATIC_MAX_DEVICES = 64;
+}  // namespace
+
+static __device__ __align__(256) double g_rhs_static_scratch[STATIC_WORDS];
+
+namespace {
+std::mutex g_static_mu;
+double* g_static_addr[STATIC_MAX_DEVICES];                 // device address of the array, per device
+unsigned g_static_prepared[STATIC_MAX_DEVICES][6];         // [device][N]: bit (ndim*4 + eos*2 + riemann)
+}  // namespace
+
+// One-time set-up per device (and per kernel instantiation): the array's device address and the stage
+// kernel's shared-memory opt-in.  Runs with the caller's device current; allocates nothing.
+static int static_setup(dgrhd_ctx* c, double** scratch) {
+  int dev = -1;
+  DG_CUDA(nullptr, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES)
+    return fail(nullptr, DGRHD_ECUDA, "dgrhd_rhs_static: device ordinal %d outside 0..%d", dev, STATIC_MAX_DEVICES - 1);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_addr[dev]) {
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_rhs_static_scratch);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "dgrhd_rhs_static: cudaGetSymbolAddress");
+    if (!p || ((uintptr_t)p % ALIGN) != 0)
+      return fail(nullptr, DGRHD_ECUDA, "dgrhd_rhs_static: the built-in scratch array has no usable device address");
+    g_static_addr[dev] = p;
+  }
+  const unsigned bit = 1u << (c->cfg.ndim * 4 + c->cfg.eos * 2 + c->cfg.riemann);
+  if (!(g_static_prepared[dev][c->N] & bit)) {
+    const cudaError_t e = prepare_stage(c);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "dgrhd_rhs_static: kernel attributes");
+    g_static_prepared[dev][c->N] |= bit;
+  }
+  *scratch = g_static_addr[dev];
+  return DGRHD_OK;
+}
+
+extern "C" int dgrhd_rhs_static(const dgrhd_config* cfg, const double* U_dev, double* R_dev,
+                                int64_t* n_c2p_fail_host, void* cuda_stream) {
+  if (!valid_cfg(cfg)) return fail(nullptr, DGRHD_EINVAL, "dgrhd_rhs_static: invalid configuration");
+  if (!U_dev || !R_dev) return fail(nullptr, DGRHD_EINVAL, "dgrhd_rhs_static: NULL argument");
+  if (U_dev == R_dev) return fail(nullptr, DGRHD_EINVAL, "dgrhd_rhs_static: U_dev and R_dev overlap");
+  if (!aligned16(U_dev) || !aligned16(R_dev))
+    return fail(nullptr, DGRHD_EINVAL, "dgrhd_rhs_static: state pointers must be 16-byte aligned");
+  // a context on the host stack: the host-side fields the launch helpers read, nothing on the device
+  dgrhd_ctx c;
+  memset(&c, 0, sizeof c);
+  c.cfg = *cfg;
+  c.N = cfg->order_p + 1;
+  c.NN = ipow(c.N, cfg->ndim);
+  c.nelem = 1;
+  for (int d = 0; d < cfg->ndim; ++d) c.nelem *= cfg->nelem[d];
+  c.ndof = c.nelem * c.NN;
+  if (c.ndof > (long long)DGRHD_STATIC_MAX_NDOF)
+    return fail(nullptr, DGRHD_ENOMEM,
+                "dgrhd_rhs_static: the mesh has %lld nodes, the built-in scratch array holds at most %d "
+                "(DGRHD_STATIC_MAX_NDOF); use dgrhd_rhs with a workspace of your own for larger meshes",
+                c.ndof, (int)DGRHD_STATIC_MAX_NDOF);
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(nullptr, DGRHD_ECUDA, "dgrhd_rhs_static: no CUDA device (there is no CPU fallback)");
+  c.state_bytes = (size_t)c.ndof * 5 * sizeof(double);
+  c.stream = (cudaStream_t)cuda_stream;
+  c.eos = make_eos(cfg->eos, cfg->gamma_ad);
+  dgbasis::build(c.N, c.basis);
+  for (int n = 0; n < c.NN; ++n) {                         // tensor-weight sum, as dgrhd_create forms it
+    double w = c.basis.w[n % c.N];
+    if (cfg->ndim > 1) w *= c.basis.w[(n / c.N) % c.N];
+    if (cfg->ndim > 2) w *= c.basis.w[n / (c.N * c.N)];
+    c.wsum += w;
+  }
+  double* scratch = nullptr;
+  const int r = static_setup(&c, &scratch);
+  if (r != DGRHD_OK) return r;
+  c.sc = (DevScalars*)scratch;
+  double* P = scratch + STATIC_HEAD_BYTES / sizeof(double);
+  // the array keeps the previous call's contents: the counters must start at zero (the pressure needs
+  // no clearing, the first kernel writes all ndof values before the second reads any)
+  DG_CUDA(nullptr, cudaMemsetAsync(c.sc, 0, sizeof(DevScalars), c.stream));
+  DG_CUDA(nullptr, launch_c2p_state(&c, U_dev, P, nullptr, nullptr, c.sc->counters));
+  StageArgs a;
+  fill_stage_args(&c, a);
+  a.mode = DG_MODE_RHS;
+  a.Us = U_dev;
+  a.Pin = P;
+  a.Rout = R_dev;
+  DG_CUDA(nullptr, launch_stage(&c, a));
+  if (n_c2p_fail_host) {
+    dg_ull h[DG_NSLOT * DG_SLOT_STRIDE];
+    DG_CUDA(nullptr, cudaMemcpyAsync(h, c.sc->counters, sizeof h, cudaMemcpyDeviceToHost, c.stream));
+    DG_CUDA(nullptr, cudaStreamSynchronize(c.stream));
+    dg_ull nfail = 0;
+    for (int s = 0; s < DG_NSLOT; ++s) nfail += h[s * DG_SLOT_STRIDE + 2];
+    *n_c2p_fail_host = (int64_t)nfail;
+  }
   return DGRHD_OK;
 }
 

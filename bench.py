@@ -13,8 +13,8 @@ north_star -> N independent replicas ("replicas only"), value = sum o
 DOF-updates / max time.
 
 Besides the timed region the default run (N = 1) adds, outside it: a parity check of the very
-configuration that was timed against the oracle ("parity"), the end-to-end leg through host buffers
-("e2e"), the con2prim batch micro-benchmark ("con2prim"), the measured FP64 peak, and the oracle's
+configuration that was timed against the oracle ("parity"), the same mesh with the HLLC flux and with the shock limiters
+("variants"), the end-to-end leg through host buffers ("e2e"), the con2prim batch micro-benchmark ("con2prim"), the measured FP64 peak, and the oracle's
 own rate on the host cores ("cpu_baseline").  --no-extra skips them.
 """
 import argparse
@@ -303,7 +303,7 @@ def sub_box_cols(nelem, nn, org, m):
 def parity_leg(b, torch, cfgd, U):
     """Outside the timed region: the residual R = L(U) of the timed configuration (same mesh, same launch
     configuration) against the oracle on seeded sub-boxes -- an element's residual depends on its face
-    neighbours only, so the interior of a sub-box is exact -- and one RK1 stage's activation count."""
+    neighbours only, so the interior of a sub-box is exact."""
     import numpy as np
     import oracle as O
     ctx = b.Context(b.make_config(*cfg_args(cfgd)))
@@ -328,6 +328,52 @@ def parity_leg(b, torch, cfgd, U):
             "residual_max_rel_err": worst, "tolerance": 1e-11, "ok": bool(worst <= 1e-11)}
 
 
+def variant_leg(b, torch, cfgd, U, default_stage_s, hbm_peak, steps=5):
+    """Outside the timed region: the timed mesh and state with the paper's other choices of the same path --
+    the HLLC interface flux (its choice for the Kelvin-Helmholtz and shock problems)
+    and the shock limiters (Moe et al., minmod; :126, :551), which add two launches per stage (cell
+    statistics, rescale) and one more read of the state.  Same timing recipe as the headline (CUDA events on
+    the launching stream, 3 warm-up steps), `steps` SSPRK3 steps each; the HBM fraction is on the same
+    algorithmic bytes per DOF and stage as the headline, so the limiter's extra traffic shows as a lower fraction."""
+    nd = cfgd["ndim"]
+    h = (cfgd["xmax"][0] - cfgd["xmin"][0]) / cfgd["nelem"][0]
+    alpha = 500.0 * h ** 1.5                      # the tolerance ref [23] suggests (include/dgrhd.h, moe_alpha)
+    variants = [("hllc", dict(riemann=1)),
+                ("hll_moe_limiter", dict(shock_limiter=1, moe_alpha=alpha)),
+                ("hll_minmod_limiter", dict(shock_limiter=2, moe_alpha=1.0)),
+                ("hllc_moe_limiter", dict(riemann=1, shock_limiter=1, moe_alpha=alpha))]
+    out = {"what": "same mesh, state and timing recipe as the headline; per variant: ms per stage, DOF-updates/s per "
+                   "stage, fraction of the HBM roofline on the headline's algorithmic bytes, cost relative to the "
+                   "headline configuration (HLL flux, no shock limiter)",
+           "steps": steps, "moe_alpha": alpha, "minmod_beta": 1.0}
+    for name, kw in variants:
+        ctx = b.Context(b.make_config(*cfg_args(cfgd), **kw))
+        ndof = ctx.ndof
+        ctx.dgrhd_set_state(U)
+        for _ in range(3):
+            ctx.dgrhd_step(-0.3, 1)
+        ctx.dgrhd_get_counters(reset=True)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ctx.dgrhd_step(-0.3, steps)
+        e1.record()
+        e1.synchronize()
+        st = e0.elapsed_time(e1) * 1e-3 / (STAGES * steps)
+        cnt = ctx.dgrhd_get_counters()
+        out[name] = {"ms_per_stage": 1e3 * st, "value": ndof / st, "unit": UNIT,
+                     "hbm_frac_alg_bytes": ALG_BYTES_PER_DOF_STAGE * ndof / st / 1e9 / hbm_peak,
+                     "cost_vs_headline": st / default_stage_s,
+                     "launches_per_stage": 3 if kw.get("shock_limiter") else 1,
+                     "shock_limited_cells_per_stage": cnt["n_shock_limited"] / max(cnt["n_stages"], 1),
+                     "physicality_activations_per_stage": cnt["n_flagged"] / max(cnt["n_stages"], 1),
+                     "n_c2p_fail": cnt["n_c2p_fail"], "n_bad_dt": cnt["n_bad_dt"]}
+        ctx.close()
+        del ctx
+        torch.cuda.empty_cache()
+    return out
+
+
 def run_cuda(a):
     import torch
     import torch.distributed as dist
@@ -347,11 +393,15 @@ def run_cuda(a):
         torch.cuda.synchronize()
 
     peak, peak_src = peaks()
+    library = b.dgrhd_version()
+    if "+asserts" in library:
+        raise SystemExit(f"bench.py: {library} is the bounds-checked debug build; unset DGRHD_DEBUG_ASSERTS")
     if a.workload == "c2p":            # configs[2]: the con2prim batch micro-benchmark alone
         n = a.size or (1 << 26)
         r = c2p_leg(b, torch, n, peak, peak_src)
         print(json.dumps({"metric": "con2prim states/s", "value": r["ideal_gamma_4_3"], "unit": "states/s",
                           "n_gpus": 1, "dtype": "f64", "data": "synthetic", "higher_is_better": True,
+                          "library": library,
                           "config": {"workload": f"con2prim batch, {n} states, ideal Gamma=4/3 and Taub-Matthews (configs[2])"},
                           "con2prim": r, "gpu_launches": 16,
                           "roofline": {"kernel": "dg_c2p_batch_kernel", "bound": "hbm", "unit": "GB/s", "peak": peak,
@@ -394,7 +444,7 @@ def run_cuda(a):
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps,
         "warmup": warm, "ms_per_step": 1e3 * secs / a.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "library": library,
         "config": {"workload": label, "dof": ndof, "stages_per_step": STAGES,
                    "l2": "state (5 x DOF x 8 B per copy) is larger than L2; no flush needed"
                    if ndof * 40 > 2 * 126e6 else "state fits L2: noted, algorithmic bytes used",
@@ -410,6 +460,7 @@ def run_cuda(a):
     }
     if rank == 0 and world == 1 and not a.no_extra:
         out["parity"] = parity_leg(b, torch, cfgd, U)
+        out["variants"] = variant_leg(b, torch, cfgd, U, stage_s, peak)
         # end to end through the C ABI with HOST buffers (pinned): H2D state, 1 step, D2H state
         Uh = U.cpu().pin_memory()
         Uo = torch.empty_like(Uh).pin_memory()

@@ -44,7 +44,10 @@ enum { DGRHD_BC_PERIODIC = 0,                /* wrap                            
        DGRHD_BC_OUTFLOW = 1,                 /* transmissive: ghost face state = own face state (:621)*/
        DGRHD_BC_REFLECT = 2,                 /* wall: ghost = own state, normal velocity reversed (:541)*/
        DGRHD_BC_DIRICHLET = 3 };             /* ghost = the fixed primitive state bc_state[d][side] (:541)*/
-#define DGRHD_BC_PAIR(lo, hi) ((lo) + 256 * (((hi) == (lo)) ? 0 : (hi)))
+/* (a pair with periodic at exactly one end has no encoding: the macro yields -1, which every call rejects) */
+#define DGRHD_BC_PAIR(lo, hi)                                                                      \
+  (((hi) == (lo)) ? (lo)                                                                           \
+                  : (((lo) == DGRHD_BC_PERIODIC || (hi) == DGRHD_BC_PERIODIC) ? -1 : (lo) + 256 * (hi)))
 /* Interface (Riemann) flux: the two-wave HLL flux (reading R9) or the
  * three-wave HLLC flux of Mignone & Bodo (ref [34]); both with lambda_L, lambda_R of Eq. 23-24. */
 enum { DGRHD_RIEMANN_HLL = 0, DGRHD_RIEMANN_HLLC = 1 };
@@ -75,7 +78,8 @@ typedef struct {
                               stage of dgrhd_step (two extra small launches per stage)              */
   double  moe_alpha;       /* Moe: tolerance alpha(h) >= 0 (ref [23] suggests ~500 h^1.5); minmod: beta in
                               [1,2] (1 = van Leer's minmod, 2 = generalised slope limiter; 0 means 1)   */
-  double  bc_state[3][2][5]; /* Dirichlet ghost primitives [axis][end] = rho, ux, uy, uz, P          */
+  double  bc_state[3][2][5]; /* Dirichlet ghost primitives [axis][end] = rho, ux, uy, uz, P: all five
+                                finite, rho > 0, P > 0 (else the configuration is invalid)            */
 } dgrhd_config;
 
 /* Bytes of device workspace dgrhd_create needs for this configuration (0 if cfg is invalid). */
@@ -163,7 +167,8 @@ int dgrhd_enforce_physicality(dgrhd_ctx* ctx, double* U_dev, unsigned char* flag
 
 /* The shock limiter the context was created with (DGRHD_SHOCK_LIMITER_MOE or _MINMOD), in place on U_dev[5][ndof];
  * theta_dev[n_elem] (or NULL) receives every cell's rescaling factor (1 = untouched).  ESTATE if the
- * context has no shock limiter.  Inside dgrhd_step it runs after the physicality operator of every stage. */
+ * context has no shock limiter.  Inside dgrhd_step it runs after the physicality operator of every stage.
+ * The stand-alone call touches no counter of dgrhd_get_counters (count theta_dev < 1 instead). */
 int dgrhd_shock_limiter(dgrhd_ctx* ctx, double* U_dev, double* theta_dev);
 
 /* CFL time step (formula: DESIGN.md reading R11):
@@ -177,18 +182,26 @@ int dgrhd_cfl_dt(dgrhd_ctx* ctx, const double* U_dev, double cfl, double* dt_hos
  * state; the last stage also reduces the CFL maximum for the next step.
  * dt > 0: fixed step.  dt <= 0: CFL number = -dt, the step is recomputed on the device every step
  * from the state at the start of the step (no host round trip).
- * t_inout_host (or NULL): *t += sum of the steps taken; non-NULL makes the call synchronise. */
+ * t_inout_host (or NULL): *t += sum of the steps taken; non-NULL makes the call synchronise.
+ * A CFL-mode step that finds no positive finite wave speed in its state (every recovery failed) cannot form
+ * dt = CFL / max: it runs with dt = 0 and is counted in n_bad_dt.  Such a state has a non-finite residual, so
+ * it comes out non-finite, and every later step is bad too.  With t_inout_host the call reports this as
+ * DGRHD_ESTATE (after adding the time actually advanced), once per batch of new bad steps, so that a loop
+ * "step until t_end" ends instead of spinning on dt = 0; without it, poll n_bad_dt. */
 int dgrhd_step(dgrhd_ctx* ctx, double dt, int nsteps, double* t_inout_host);
 
 /* Device counters accumulated since create / the last reset (synchronises):
  *   out_host[0] n_flagged      cell-activations of the physicality operator inside dgrhd_step
  *   out_host[1] n_bad_mean     cells whose average was itself inadmissible (flattened)
- *   out_host[2] n_c2p_fail     nodes where con2prim failed (inadmissible input or P <= 0)
+ *   out_host[2] n_c2p_fail     recoveries that failed (inadmissible input or P <= 0), counted in every pass that
+ *                              recovers a node: dgrhd_set_state, dgrhd_rhs, the end of every stage and, with a
+ *                              shock limiter on, once more for the nodes of every cell it rescaled (so the same
+ *                              bad node of the same stage can count twice); 0 means no recovery failed anywhere
  *   out_host[3] n_stages       RK stages executed by dgrhd_step
  *   out_host[4] n_tm_fallback  Taub-Matthews recoveries that took the double-precision closed form
  *                              because the fast route's Newton polish had not converged
  *   out_host[5] n_bad_dt       CFL-mode steps whose wave-speed maximum was not a positive finite
- *                              number: they ran with dt = 0 (state unchanged) instead of dt = inf
+ *                              number: they ran with dt = 0 instead of dt = inf (see dgrhd_step)
  *   out_host[6] n_shock_limited  cell-rescalings (theta < 1) by the shock limiter; out_host[7] reserved (0)
  * reset != 0 zeroes them afterwards. */
 int dgrhd_get_counters(dgrhd_ctx* ctx, int64_t out_host[8], int reset);
@@ -243,7 +256,8 @@ int dgrhd_probe_fp64(void* scratch_dev, double* tflops_host, double* sm_mhz_host
  * thread).  Never NULL; valid until the next call on the same context / thread. */
 const char* dgrhd_last_error(const dgrhd_ctx* ctx);
 
-/* Library version string, e.g. "dgrhd 0.2 (sm_100a)". */
+/* Library version string: "dgrhd 0.3 (sm_100a) src=<16 hex digits>", the hash being that of the sources the
+ * library was compiled from (paper_2205_00095_b200/build.py); the bounds-checked debug build appends "+asserts". */
 const char* dgrhd_version(void);
 
 #ifdef __cplusplus

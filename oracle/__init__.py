@@ -25,9 +25,12 @@ class Config(C.Structure):
 
 
 def _bc_code(b):
-    """int (both ends) or (lo, hi) -> lo + 256*hi (hi = 0: same as lo)."""
+    """int (both ends) or (lo, hi) -> lo + 256*hi (hi = 0: same as lo).  Periodic (0) is a property of the
+    whole axis: a pair with periodic at one end only is refused."""
     if isinstance(b, (tuple, list)):
         lo, hi = int(b[0]), int(b[1])
+        if lo != hi and 0 in (lo, hi):
+            raise ValueError(f"boundary pair {b}: periodic at one end only")
         return lo + 256 * (hi if hi != lo else 0)
     return int(b)
 

@@ -17,7 +17,8 @@ OPT_CUDA_GRAPH = 0
 C2P_DEFAULT, C2P_ALTERNATE = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdgrhd.so")
+# DGRHD_DEBUG_ASSERTS=1 selects the bounds-checked debug build (python -m paper_2205_00095_b200.build --debug-asserts)
+LIB_PATH = os.path.join(_HERE, "libdgrhd_dbg.so" if os.environ.get("DGRHD_DEBUG_ASSERTS") == "1" else "libdgrhd.so")
 
 
 class DgrhdError(RuntimeError):
@@ -37,10 +38,13 @@ class Config(C.Structure):
 
 
 def _bc_code(b):
-    """int (both ends) or (lo, hi) -> DGRHD_BC_PAIR(lo, hi)."""
+    """int (both ends) or (lo, hi) -> DGRHD_BC_PAIR(lo, hi); periodic at exactly one end has no encoding
+    and gives -1, which the library rejects as an invalid configuration."""
     if isinstance(b, (tuple, list)):
         lo, hi = int(b[0]), int(b[1])
-        return lo + 256 * (hi if hi != lo else 0)
+        if lo == hi:
+            return lo
+        return -1 if BC_PERIODIC in (lo, hi) else lo + 256 * hi
     return int(b)
 
 

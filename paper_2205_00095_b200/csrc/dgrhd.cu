@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -59,7 +60,12 @@ bool valid_cfg(const dgrhd_config* c) {
       if (lo == DGRHD_BC_PERIODIC && hi != 0) return false;     // periodic is both ends
       for (int sd = 0; sd < 2; ++sd) {
         const int k = (sd && hi) ? hi : lo;
-        if (k == DGRHD_BC_DIRICHLET && !(c->bc_state[d][sd][0] > 0.0 && c->bc_state[d][sd][4] > 0.0)) return false;
+        if (k == DGRHD_BC_DIRICHLET) {                          // ghost primitives: finite, rho > 0, P > 0
+          const double* w = c->bc_state[d][sd];
+          for (int v = 0; v < 5; ++v)
+            if (!std::isfinite(w[v])) return false;
+          if (!(w[0] > 0.0 && w[4] > 0.0)) return false;
+        }
       }
     }
   }
@@ -114,6 +120,7 @@ struct dgrhd_ctx {
   cudaStream_t cap_stream;
   cudaGraphExec_t gexec[2];
   double gdt[2];
+  dg_ull bad_dt_seen;       // n_bad_dt as last read back by dgrhd_step / dgrhd_get_counters
   char err[512];
 };
 
@@ -627,8 +634,9 @@ extern "C" int dgrhd_shock_limiter(dgrhd_ctx* c, double* U_dev, double* theta_de
   if (c->cfg.shock_limiter == DGRHD_SHOCK_LIMITER_NONE)
     return fail(c, DGRHD_ESTATE, "dgrhd_shock_limiter: the context was created without a shock limiter");
   if (!aligned16(U_dev)) return fail(c, DGRHD_EINVAL, "dgrhd_shock_limiter: state pointer must be 16-byte aligned");
-  // (the pressure of the rescaled cells lands in the spare pressure buffer; no counters, no CFL)
-  DG_CUDA(c, launch_moe(c, U_dev, c->P[c->par ^ 1], 0, c->sc->amax_tmp, c->sc->amax_tmp, theta_dev));
+  // (the pressure of the rescaled cells lands in the spare pressure buffer; no counters, no CFL: the
+  // apply kernel skips both, so neither array is touched)
+  DG_CUDA(c, launch_moe(c, U_dev, c->P[c->par ^ 1], 0, nullptr, nullptr, theta_dev));
   return DGRHD_OK;
 }
 
@@ -746,10 +754,17 @@ extern "C" int dgrhd_step(dgrhd_ctx* c, double dt, int nsteps, double* t_inout_h
     if (r != DGRHD_OK) return r;
   }
   if (t_inout_host) {
-    double h = 0.0;
+    struct { double t_acc; dg_ull n_stages, n_bad_dt; } h = {0.0, 0ull, 0ull};   // consecutive in DevScalars
+    static_assert(offsetof(DevScalars, n_bad_dt) == offsetof(DevScalars, t_acc) + 16, "read back as one block");
     DG_CUDA(c, cudaMemcpyAsync(&h, &c->sc->t_acc, sizeof h, cudaMemcpyDeviceToHost, c->stream));
     DG_CUDA(c, cudaStreamSynchronize(c->stream));
-    *t_inout_host += h;
+    *t_inout_host += h.t_acc;
+    if (h.n_bad_dt > c->bad_dt_seen) {       // a caller looping to a final time must not spin on dt = 0
+      const dg_ull nbad = h.n_bad_dt - c->bad_dt_seen;
+      c->bad_dt_seen = h.n_bad_dt;
+      return fail(c, DGRHD_ESTATE, "dgrhd_step: %llu step(s) found no positive finite wave speed in the state and "
+                  "ran with dt = 0 (con2prim failures? see dgrhd_get_counters)", nbad);
+    }
   }
   return DGRHD_OK;
 }
@@ -781,6 +796,7 @@ extern "C" int dgrhd_get_counters(dgrhd_ctx* c, int64_t out_host[8], int reset) 
     DG_CUDA(c, cudaMemsetAsync(&c->sc->n_stages, 0, 2 * sizeof(dg_ull), c->stream));
   }
   DG_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->bad_dt_seen = reset ? 0ull : h.n_bad_dt;
   dg_ull sum[5] = {0, 0, 0, 0, 0};
   for (int s = 0; s < DG_NSLOT; ++s)
     for (int k = 0; k < 5; ++k) sum[k] += h.counters[s * DG_SLOT_STRIDE + k];
@@ -927,4 +943,15 @@ extern "C" int dgrhd_probe_fp64(void* scratch_dev, double* tflops_host, double* 
 
 extern "C" const char* dgrhd_last_error(const dgrhd_ctx* c) { return c ? c->err : g_err; }
 
-extern "C" const char* dgrhd_version(void) { return "dgrhd 0.2 (sm_100a)"; }
+// The version string carries the hash of the sources this library was compiled from (build.py passes
+// it and reads it back from the file to decide whether a rebuild is due) and says when the kernels are
+// the bounds-checked debug ones.
+#ifndef DG_SRC_HASH
+#define DG_SRC_HASH "unknown"
+#endif
+#ifdef DG_DEBUG_ASSERTS
+#define DG_VERSION_TAIL "+asserts"
+#else
+#define DG_VERSION_TAIL ""
+#endif
+extern "C" const char* dgrhd_version(void) { return "dgrhd 0.3 (sm_100a) src=" DG_SRC_HASH DG_VERSION_TAIL; }

@@ -460,7 +460,7 @@ dg_moe_apply_kernel(long long nelem, long long ndof, double* U, double* P, const
       c1 += __shfl_xor_sync(0xffffffffu, c1, o);
       c2 += __shfl_xor_sync(0xffffffffu, c2, o);
     }
-    if (lane == 0) {
+    if (lane == 0 && counters) {                            // NULL: the stand-alone call keeps no counts
       if (c0) atomicAdd(&counters[slot + 4], (dg_ull)c0);
       if (c1) atomicAdd(&counters[slot + 2], (dg_ull)c1);
       if (c2) atomicAdd(&counters[slot + 3], (dg_ull)c2);

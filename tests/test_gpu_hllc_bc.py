@@ -79,8 +79,15 @@ def test_bad_boundary_configurations_are_rejected():
     b = B()
     d = mesh(1, [8], 2, 0, 5 / 3, [(I.BC_PERIODIC, I.BC_OUTFLOW)])                 # periodic at one end only
     assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
+    d = mesh(1, [8], 2, 0, 5 / 3, [(I.BC_OUTFLOW, I.BC_PERIODIC)])                 # ... at the other end only
+    assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
     d = mesh(1, [8], 2, 0, 5 / 3, [I.BC_DIRICHLET])                               # no ghost state given
     assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
+    for bad in (float("nan"), float("inf")):                                      # ghost velocity not finite
+        gs = {(0, 0): [1.0, bad, 0.0, 0.0, 1.0], (0, 1): [1.0, 0.0, 0.0, 0.0, 1.0]}
+        assert b.dgrhd_workspace_bytes(gcfg(mesh(1, [8], 2, 0, 5 / 3, [I.BC_DIRICHLET], bc_state=gs))) == 0
+    gs = {(0, 0): [1.0, 0.3, 0.0, 0.0, 1.0], (0, 1): [1.0, 0.0, 0.0, 0.0, 1.0]}
+    assert b.dgrhd_workspace_bytes(gcfg(mesh(1, [8], 2, 0, 5 / 3, [I.BC_DIRICHLET], bc_state=gs))) > 0
     d = mesh(1, [8], 2, 0, 5 / 3, [1], riemann=7)
     assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
 

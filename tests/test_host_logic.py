@@ -32,6 +32,20 @@ def test_library_exports_every_declared_symbol():
     assert set(binding.EXPORTS) == names
 
 
+def test_library_proves_what_it_was_built_from():
+    """dgrhd_version() carries the hash of the sources the library was compiled from; build() reuses a library
+    only when that hash matches, and the bounds-checked debug build is a different file behind an env switch."""
+    from paper_2205_00095_b200 import build, binding as b
+    path = build.build()
+    assert build.LAST_MODE in ("compiled", "reused") and path == build.LIB != build.LIB_DBG
+    v = b.dgrhd_version()
+    assert v == build.library_version(path) and v.endswith("src=" + build.source_hash())
+    assert build.library_version(os.path.join(ROOT, "README.md")) == ""
+    r = subprocess.run([sys.executable, "-c", "from paper_2205_00095_b200 import binding; print(binding.LIB_PATH)"],
+                       capture_output=True, text=True, cwd=ROOT, env=dict(os.environ, DGRHD_DEBUG_ASSERTS="1"))
+    assert r.stdout.strip() == build.LIB_DBG
+
+
 def test_argument_errors_are_detected_without_a_device():
     from paper_2205_00095_b200 import binding as b
     L = b.lib()
@@ -51,8 +65,16 @@ def test_argument_errors_are_detected_without_a_device():
     assert b.dgrhd_workspace_bytes(mutated()) > 0
     for bad in (mutated(ndim=4), mutated(ndim=0), mutated(xmax=(0, -1.0)), mutated(order_p=5), mutated(gamma_ad=1.0),
                 mutated(bc=(0, 7)), mutated(eos=3), mutated(rk_stages=4), mutated(nelem=(0, 0)), mutated(nelem=(1, 2)),
-                mutated(eps_q=-1.0), b.make_config(3, [2048] * 3, [0] * 3, [1] * 3, [0] * 3, 3, 0, 5 / 3)):
+                mutated(eps_q=-1.0), b.make_config(3, [2048] * 3, [0] * 3, [1] * 3, [0] * 3, 3, 0, 5 / 3),
+                # periodic at one end of an axis only, either way round; a Dirichlet ghost state that is not finite
+                b.make_config(1, [8], [0], [1], [(1, 0)], 2, 0, 5 / 3), b.make_config(1, [8], [0], [1], [(0, 2)], 2, 0, 5 / 3),
+                b.make_config(1, [8], [0], [1], [3], 2, 0, 5 / 3,
+                              bc_state={(0, 0): [1, float("nan"), 0, 0, 1], (0, 1): [1, 0, 0, 0, 1]}),
+                b.make_config(1, [8], [0], [1], [(3, 1)], 2, 0, 5 / 3, bc_state={(0, 0): [1, 0, float("inf"), 0, 1]})):
         assert b.dgrhd_workspace_bytes(bad) == 0
+    assert b._bc_code((1, 0)) == -1 and b._bc_code((0, 0)) == 0 and b._bc_code((2, 2)) == 2 and b._bc_code((1, 3)) == 1 + 256 * 3
+    assert b.dgrhd_workspace_bytes(b.make_config(1, [8], [0], [1], [(3, 1)], 2, 0, 5 / 3,
+                                                 bc_state={(0, 0): [1, 0.2, 0, 0, 1]})) > 0
     h = ctypes.c_void_p()
     assert L.dgrhd_create(ctypes.byref(good), None, 0, None, ctypes.byref(h)) == b.EINVAL
     assert b"workspace" in L.dgrhd_last_error(None)

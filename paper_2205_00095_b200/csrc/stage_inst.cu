@@ -2,6 +2,9 @@
 // and every order p = 0..4; compiled once per triple (-DDG_INST_ND=1|2|3 -DDG_INST_EOS=0|1
 // -DDG_INST_RS=0|1) so that the translation units build in parallel.  Exports a launcher and a per-device preparation call,
 // declared in dgrhd.cu.
+#include <cstdlib>
+#include <cstring>
+
 #include "stage_kernel.cuh"
 
 #ifndef DG_INST_ND
@@ -24,6 +27,14 @@ static cudaError_t prepare_n() {
   return cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 
+// log2 of the brick edge in tiles along axis d = 1 (y), 2 (z); EXPERIMENT knob DG_BRICK_LOG2="yz", default "33"
+static int dg_brick_target(int d) {
+  const char* e = getenv("DG_BRICK_LOG2");
+  if (!e || strlen(e) != 2) return 3;
+  const int v = e[d - 1] - '0';
+  return (v < 0 || v > 6) ? 3 : v;
+}
+
 template <int N>
 static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
   using TS = TileShape<DG_INST_ND, N>;
@@ -31,8 +42,27 @@ static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
                   ntz = (a.ne[2] + TS::TZ - 1) / TS::TZ;
   if (ntx <= 0 || nty <= 0 || ntz <= 0 || ntx > 2147483647LL || nty > 65535 || ntz > 65535)
     return cudaErrorInvalidConfiguration;
+  long long gy = nty, gz = ntz;
+  if (DG_INST_ND == 3) {
+    // brick order (dg_tile_of_block): the largest power-of-two brick edge <= the target whose padding
+    // adds at most 1/8 to the tile count of that axis; the y extent of the grid holds BZ y-columns
+    StageArgs b = a;
+    int lby = 0, lbz = 0;
+    static const int target_y = dg_brick_target(1), target_z = dg_brick_target(2);
+    for (int l = target_y; l > 0 && !lby; --l) if (((nty + (1 << l) - 1) >> l << l) * 8 <= nty * 9) lby = l;
+    for (int l = target_z; l > 0 && !lbz; --l) if (((ntz + (1 << l) - 1) >> l << l) * 8 <= ntz * 9) lbz = l;
+    const long long py = (nty + (1 << lby) - 1) >> lby << lby;
+    if ((py << lbz) > 65535) lbz = 0;
+    b.lby = lby;
+    b.lbz = lbz;
+    gy = py << lbz;
+    gz = (ntz + (1 << lbz) - 1) >> lbz;
+    dg_stage_kernel<DG_INST_ND, N, DG_INST_EOS, DG_INST_RS>
+        <<<dim3((unsigned)ntx, (unsigned)gy, (unsigned)gz), TS::NT, TS::SMEM_BYTES, st>>>(b);
+    return cudaGetLastError();
+  }
   dg_stage_kernel<DG_INST_ND, N, DG_INST_EOS, DG_INST_RS>
-      <<<dim3((unsigned)ntx, (unsigned)nty, (unsigned)ntz), TS::NT, TS::SMEM_BYTES, st>>>(a);
+      <<<dim3((unsigned)ntx, (unsigned)gy, (unsigned)gz), TS::NT, TS::SMEM_BYTES, st>>>(a);
   return cudaGetLastError();
 }
 

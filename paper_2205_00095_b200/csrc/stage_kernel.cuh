@@ -159,7 +159,21 @@ struct StageArgs {
   int bcm[3][2];          // at a mesh boundary [axis][end]: 0 ghost = halo value as loaded (periodic wrap /
                           // outflow copy), DG_BC_REFLECT normal momentum reversed, DG_BC_DIRICHLET fixed state
   double bcU[3][2][6];    // Dirichlet ghost state: U (Eq. 4 of the given primitives) and P
+  int lby, lbz;           // 3D launch order: tiles are walked in bricks of (all x) x 2^lby x 2^lbz tiles, see
+                          // dg_tile_of_block; 0, 0 = plain x-fastest order (grid = tile grid)
 };
+
+// Tile (y, z) index of a block.  The hardware starts blocks in blockIdx order, x fastest, then y, then z.
+// In that plain order the z-neighbour of a tile runs a whole xy-plane of tiles later (4096 tiles = ~100 MB
+// of traffic at 128^3, p = 3: its halo rows have left L2 by then).  Brick order keeps both neighbours
+// close: blockIdx.y = ty_local + BY (tz_local + BZ * brick_y), blockIdx.z = brick_z, BY = 2^lby,
+// BZ = 2^lbz, so the z-neighbour runs ntx * BY tiles later.  The launch pads the tile grid to whole
+// bricks; blocks of the padding return at once.
+DG_INL void dg_tile_of_block(const StageArgs& a, int& ty, int& tz) {
+  const int by = (int)blockIdx.y;
+  ty = (by & ((1 << a.lby) - 1)) | ((by >> (a.lby + a.lbz)) << a.lby);
+  tz = ((by >> a.lby) & ((1 << a.lbz) - 1)) + ((int)blockIdx.z << a.lbz);
+}
 
 // ---------------------------------------------------------------------------------------------
 // line access helpers: N consecutive doubles, 16-byte vectors when N is even (p 16-byte aligned)
@@ -639,7 +653,12 @@ dg_stage_kernel(const __grid_constant__ StageArgs a) {
   double* sDz = sDy + 26;
 
   // tile of this block; element, line (j,k) and segment h of this thread
-  const int org[3] = {(int)blockIdx.x * TS::TX, (int)blockIdx.y * TS::TY, (int)blockIdx.z * TS::TZ};
+  int ty = (int)blockIdx.y, tz = (int)blockIdx.z;
+  if constexpr (ND == 3) {
+    dg_tile_of_block(a, ty, tz);
+    if (ty * TS::TY >= a.ne[1] || tz * TS::TZ >= a.ne[2]) return;    // padding of the brick grid
+  }
+  const int org[3] = {(int)blockIdx.x * TS::TX, ty * TS::TY, tz * TS::TZ};
   const int teff[3] = {min(TS::TX, a.ne[0] - org[0]), min(TS::TY, a.ne[1] - org[1]),
                        min(TS::TZ, a.ne[2] - org[2])};
   const int t = threadIdx.x, lane = t & 31, wrp = t >> 5;

@@ -38,13 +38,16 @@ ALG_BYTES_PER_DOF_STAGE = (80.0 + 120.0 + 120.0) / 3.0
 DESIGN_BYTES_PER_DOF_STAGE = ALG_BYTES_PER_DOF_STAGE + 16.0
 # Per-workload constants of dg_stage_kernel taken from ncu captures of THIS kernel (mean of the three
 # stages of one step): executed fp64 work per DOF (2*dfma + dmul + dadd, thread level) and DRAM bytes
-# per DOF (dram__bytes_read + dram__bytes_write).  Each entry names the capture it comes from; the
-# summaries are under profiles/.  Stale after any kernel change: re-capture (profiles/r2_README.md).
+# per DOF (dram__bytes_read + dram__bytes_write).  Each entry names the capture it comes from (summaries
+# under profiles/) and the hash of the stage kernel's sources at that capture ("stage_src",
+# paper_2205_00095_b200.build.stage_kernel_hash()): when the sources have changed since, the line prints
+# traffic = null and no ALU fraction instead of stale numbers -- re-capture (profiles/r3_README.md).
 KERNEL_CONSTANTS = {
-    "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 135.4,
-              "source": "profiles/r2_ncu_stage_box3d_128.md (capture at 128^3, commit 27b63d4)"},
-    "kh2d": {"flop_per_dof_stage": 449.7, "dram_bytes_per_dof_stage": 114.3,
-             "source": "profiles/r2_ncu_stage_kh2d.md (96 registers / 5 blocks per SM; cold-cache replays: in a timed run most of the 189 MB state stays in L2)"},
+    "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 128.9, "stage_src": "57ae52f586578bff",
+              "source": "profiles/r3_ncu_stage_box3d_128.md (capture at 128^3, library src=e857100547a6b864)"},
+    "kh2d": {"flop_per_dof_stage": 449.7, "dram_bytes_per_dof_stage": 114.3, "stage_src": None,
+             "source": "profiles/r2_ncu_stage_kh2d.md (round 2, 96 registers / 5 blocks per SM; not re-captured in round 3: the 2D kernel's "
+                       "code path is unchanged but its sources are not byte-identical, so the line marks these as stale)"},
 }
 # fp64 peak derived from unit counts: 148 SMs x 64 DFMA/clk/SM x 2 flop x max SM clock; the measured
 # figure (dgrhd_probe_fp64, a register-only DFMA kernel timed in this run) is reported beside it.
@@ -58,6 +61,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="box3d", choices=["box3d", "kh2d", "c2p"])
+    ap.add_argument("--riemann", default="hll", choices=["hll", "hllc"], help="interface flux of the timed run")
+    ap.add_argument("--shock-limiter", default="none", choices=["none", "moe", "minmod"],
+                    help="shock limiter of the timed run (adds two launches per stage)")
     ap.add_argument("--size", type=int, default=0, help="override elements per axis (debug)")
     ap.add_argument("--no-extra", action="store_true", help="skip parity / con2prim / e2e / cpu legs")
     return ap.parse_args()
@@ -137,6 +143,24 @@ def workload_cfg(name, size, device):
 def cfg_args(cfgd):
     return (cfgd["ndim"], cfgd["nelem"], cfgd["xmin"], cfgd["xmax"], cfgd["bc"], cfgd["order_p"],
             cfgd["eos"], cfgd["gamma_ad"], cfgd["rk_stages"], cfgd["eps_q"], cfgd["delta_s"])
+
+
+def cfg_kw(cfgd):
+    """Flux / shock-limiter choice of the run (keyword arguments of both make_config's)."""
+    return dict(riemann=cfgd.get("riemann", 0), shock_limiter=cfgd.get("shock_limiter", 0),
+                moe_alpha=cfgd.get("moe_alpha", 0.0))
+
+
+def apply_choices(cfgd, a):
+    """--riemann / --shock-limiter on top of the workload's configuration; returns a label suffix."""
+    cfgd["riemann"] = 1 if a.riemann == "hllc" else 0
+    lim = {"none": 0, "moe": 1, "minmod": 2}[a.shock_limiter]
+    cfgd["shock_limiter"] = lim
+    h = (cfgd["xmax"][0] - cfgd["xmin"][0]) / cfgd["nelem"][0]
+    cfgd["moe_alpha"] = [0.0, 500.0 * h ** 1.5, 1.0][lim]
+    extra = (", HLLC flux" if cfgd["riemann"] else "") + ["", f", Moe shock limiter (alpha = 500 h^1.5 = {cfgd['moe_alpha']:.4g})",
+                                                          ", minmod shock limiter (beta = 1)"][lim]
+    return extra
 
 
 # ------------------------------------------------------------------------------------------------
@@ -255,7 +279,9 @@ def roofline_stage(workload, ndof, stage_s, clocks, hbm_peak, peak_src, fp64_mea
     """Roofline of the dominant kernel (the fused stage kernel; > 99.9 % of the step, the dt kernel
     being one thread).  The slower of the two resources bounds it: fp64 ALUs (executed flop / fp64
     peak) or HBM (algorithmic bytes / measured copy bandwidth); both fractions are reported."""
-    kc = KERNEL_CONSTANTS[workload]
+    from paper_2205_00095_b200 import build as _build
+    kc = dict(KERNEL_CONSTANTS[workload])
+    stale = kc.get("stage_src") != _build.stage_kernel_hash()
     ach_hbm = ALG_BYTES_PER_DOF_STAGE * ndof / stage_s / 1e9
     hbm = {"achieved": ach_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": ach_hbm / hbm_peak,
            "peak_source": peak_src, "alg_bytes_per_dof_stage": ALG_BYTES_PER_DOF_STAGE,
@@ -274,7 +300,13 @@ def roofline_stage(workload, ndof, stage_s, clocks, hbm_peak, peak_src, fp64_mea
     traffic = kc["dram_bytes_per_dof_stage"] * ndof if kc["dram_bytes_per_dof_stage"] else None
     out = {"kernel": "dg_stage_kernel", "avg_launch_ms": 1e3 * stage_s,
            "avg_launch_how": "CUDA events around the timed region on the launching stream / (3 x steps)",
-           "traffic": traffic, "constants_source": kc["source"], "hbm": hbm, "alu": alu}
+           "traffic": traffic, "constants_source": kc["source"], "constants_stale": stale, "hbm": hbm, "alu": alu}
+    if stale:       # the capture is of other sources: no traffic, no executed-flop fractions; the HBM roofline on
+        out.update({"traffic": None,           # algorithmic bytes needs no capture and stands
+                    "alu": {"stale": True, "flop_per_dof_stage_at_capture": kc["flop_per_dof_stage"],
+                            "peak_measured": fp64_measured, "peak_derived": alu_derived}})
+        out.update({"bound": "hbm", "achieved": ach_hbm, "peak": hbm_peak, "unit": "GB/s", "frac": ach_hbm / hbm_peak})
+        return out
     if t_alu >= t_hbm:
         peak = fp64_measured or alu_derived
         out.update({"bound": "alu", "achieved": ach_alu, "peak": peak, "unit": "TFLOP/s", "frac": ach_alu / peak})
@@ -306,7 +338,7 @@ def parity_leg(b, torch, cfgd, U):
     neighbours only, so the interior of a sub-box is exact."""
     import numpy as np
     import oracle as O
-    ctx = b.Context(b.make_config(*cfg_args(cfgd)))
+    ctx = b.Context(b.make_config(*cfg_args(cfgd), **cfg_kw(cfgd)))
     R = ctx.dgrhd_rhs(U).cpu().numpy()
     Uh = U.cpu().numpy()
     nd, nelem, nn = cfgd["ndim"], cfgd["nelem"][:cfgd["ndim"]], (cfgd["order_p"] + 1) ** cfgd["ndim"]
@@ -318,11 +350,12 @@ def parity_leg(b, torch, cfgd, U):
     worst = 0.0
     for org in orgs:
         cols, inner = sub_box_cols(nelem, nn, org, m)
-        Ro, _ = O.rhs(O.make_config(*cfg_args(sub)), np.ascontiguousarray(Uh[:, cols]))
+        Ro, _ = O.rhs(O.make_config(*cfg_args(sub), **cfg_kw(sub)), np.ascontiguousarray(Uh[:, cols]))
         scale = np.maximum(np.max(np.abs(Ro[:, inner]), axis=1), 1e-300)
         err = np.max(np.abs(R[:, cols][:, inner] - Ro[:, inner]), axis=1) / scale
-        act = np.max(np.abs(Ro[:, inner]), axis=1) > 1e-9
-        worst = max(worst, float(err[act].max()))
+        act = np.max(np.abs(Ro[:, inner]), axis=1) > 1e-9      # rows that are ~0 (unused axes, uniform flow): absolute
+        worst = max(worst, float(err[act].max(initial=0.0)),
+                    float(np.max(np.abs(R[:, cols][:, inner] - Ro[:, inner])[~act], initial=0.0)))
     ctx.close()
     return {"what": f"dgrhd_rhs of the timed configuration vs the oracle on {len(orgs)} sub-boxes of {m}^{nd} elements (interior)",
             "residual_max_rel_err": worst, "tolerance": 1e-11, "ok": bool(worst <= 1e-11)}
@@ -412,7 +445,9 @@ def run_cuda(a):
                                        "frac_tm": r["roofline_hbm_frac_tm"], "traffic": None}}))
         return
     cfgd, W, label = workload_cfg(a.workload, a.size, "cuda")
-    ctx = b.Context(b.make_config(*cfg_args(cfgd)))
+    label += apply_choices(cfgd, a)
+    lps = 3 if cfgd["shock_limiter"] else 1                 # launches per stage
+    ctx = b.Context(b.make_config(*cfg_args(cfgd), **cfg_kw(cfgd)))
     U = b.dgrhd_prim2con_batch(cfgd["eos"], cfgd["gamma_ad"], W)
     del W
     ndof = ctx.ndof
@@ -454,13 +489,14 @@ def run_cuda(a):
                    "n_tm_fallback": cnt["n_tm_fallback"], "n_bad_dt": cnt["n_bad_dt"]},
         # kernels of this library launched inside the timed region: per step 1 dt kernel + 3 fused stage
         # kernels, replayed as ONE captured CUDA graph per step
-        "gpu_launches": a.steps * (STAGES + 1), "graph_launches": a.steps,
+        "gpu_launches": a.steps * (STAGES * lps + 1), "graph_launches": a.steps,
         "clocks": clocks,
         "roofline": roofline_stage(a.workload, ndof, stage_s, clocks, peak, peak_src, fp64_meas),
     }
     if rank == 0 and world == 1 and not a.no_extra:
         out["parity"] = parity_leg(b, torch, cfgd, U)
-        out["variants"] = variant_leg(b, torch, cfgd, U, stage_s, peak)
+        if not (cfgd["riemann"] or cfgd["shock_limiter"]):
+            out["variants"] = variant_leg(b, torch, cfgd, U, stage_s, peak)
         # end to end through the C ABI with HOST buffers (pinned): H2D state, 1 step, D2H state
         Uh = U.cpu().pin_memory()
         Uo = torch.empty_like(Uh).pin_memory()

@@ -6,9 +6,10 @@
  * does not change any arithmetic or summation order].
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): every function the paper prints is pinned; see DESIGN.md
- * "Oracle pins".  PARITY UNPINNED: orc_shock_limiter (the Moe limiter and the minmod limiter), which the
- * paper cites (refs [23], [24]) without printing; they are restated in DESIGN.md readings R18 / R19 and
- * pinned by their properties and special cases only.
+ * "Oracle pins".  PARITY UNPINNED BY THE PAPER: orc_shock_limiter (the Moe limiter and the minmod limiter),
+ * which the paper cites (refs [23], [24]) without printing; they are restated in DESIGN.md readings R18 / R19.
+ * What is pinned is the reading: the Moe branch by hand-worked cases (tests/golden/moe_limiter_cases.txt) and
+ * its properties, the minmod branch by its reduction to van Leer's minmod and its properties.
  */
 #include "dgrhd_oracle.h"
 #include <math.h>

@@ -55,6 +55,16 @@ def source_hash() -> str:
     return h.hexdigest()[:16]
 
 
+def stage_kernel_hash() -> str:
+    """Hash of the sources the fused stage kernel is compiled from.  bench.py's per-DOF constants (executed flop,
+    DRAM bytes) come from an ncu capture of that kernel and are valid only for the sources they were taken on."""
+    h = hashlib.sha256()
+    for name in ("stage_kernel.cuh", "physics.cuh", "stage_inst.cu"):
+        with open(os.path.join(CSRC, name), "rb") as fh:
+            h.update(name.encode() + b"\0" + fh.read() + b"\0")
+    return h.hexdigest()[:16]
+
+
 def library_version(path: str) -> str:
     """The dgrhd_version() string of a built library, read from the file's bytes (no dlopen: a library that
     is about to be rebuilt must not already be mapped into this process).  '' if there is none."""

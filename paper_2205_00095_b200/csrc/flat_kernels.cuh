@@ -318,43 +318,68 @@ dg_mm_stats_kernel(long long nelem, long long ndof, const double* __restrict__ U
   }
 }
 
-// theta of the minmod limiter for cell e (reading R19): min over variables and directions of
-// minmod(a_d, beta D+/2, beta D-/2) / a_d, D+- the differences of the neighbouring cell averages
-// (periodic wrap; a missing neighbour drops out); 1 if >= 1 - 1e-12.
+// Neighbour of cell e along axis d on side `side` (0 minus, 1 plus): its index, or -1 when there is none
+// (periodic wrap; no neighbour beyond any other boundary).  Cell indices fit 32 bits (ndof < 2^31).
+DG_INL int dg_cell_neighbour(int e, const int ie[3], const int ne[3], const int periodic[3], int d, int side) {
+  const int es = (d == 0) ? 1 : (d == 1 ? ne[0] : ne[0] * ne[1]);
+  int jd = ie[d] + (side ? 1 : -1);
+  if (jd < 0 || jd >= ne[d]) {
+    if (!periodic[d]) return -1;
+    jd = (jd < 0) ? ne[d] - 1 : 0;
+  }
+  return e + (jd - ie[d]) * es;
+}
+
+// theta of the minmod limiter (reading R19) from ONE variable v of cell e: min over the directions of
+// minmod(a_d, beta D+/2, beta D-/2) / a_d, D+- the differences of the neighbouring cell averages (a missing
+// neighbour drops out).  The cell's theta is the minimum over v, set to 1 if >= 1 - 1e-12 (by the caller).
 template <int ND>
-DG_INL double dg_mm_theta(const double* __restrict__ stats, long long e, const long long ne[3], const int periodic[3],
-                          double beta, double mean[5]) {
-  const long long ie[3] = {e % ne[0], (e / ne[0]) % ne[1], e / (ne[0] * ne[1])};
-  const long long es[3] = {1, ne[0], ne[0] * ne[1]};
+DG_INL double dg_mm_theta_var(const double* __restrict__ stats, int e, int v, const int ie[3], const int ne[3],
+                              const int periodic[3], double beta) {
+  const double wb = stats[(long long)e * 25 + v], tiny = 1e-12 * stats[(long long)e * 25 + 20 + v];
   double theta = 1.0;
 #pragma unroll
-  for (int v = 0; v < 5; ++v) {
-    const double wb = stats[e * 25 + v], tiny = 1e-12 * stats[e * 25 + 20 + v];
-    mean[v] = wb;
+  for (int d = 0; d < ND; ++d) {
+    const double a = stats[(long long)e * 25 + 5 + 5 * d + v];
+    if (!(fabs(a) > tiny)) continue;
+    const double sg = (a > 0.0) ? 1.0 : -1.0;
+    double m = fabs(a);
+    bool zero = false;
 #pragma unroll
-    for (int d = 0; d < ND; ++d) {
-      const double a = stats[e * 25 + 5 + 5 * d + v];
-      if (!(fabs(a) > tiny)) continue;
-      const double sg = (a > 0.0) ? 1.0 : -1.0;
-      double m = fabs(a);
-      bool zero = false;
-#pragma unroll
-      for (int side = 0; side < 2; ++side) {
-        long long jd = ie[d] + (side ? 1 : -1);
-        if (jd < 0 || jd >= ne[d]) {
-          if (!periodic[d]) continue;
-          jd = (jd + ne[d]) % ne[d];
-        }
-        const double wn = stats[(e + (jd - ie[d]) * es[d]) * 25 + v];
-        const double b = 0.5 * beta * (side ? wn - wb : wb - wn);
-        if (b * sg <= 0.0) zero = true;
-        m = fmin(m, fabs(b));
-      }
-      const double r = zero ? 0.0 : (sg * m) / a;
-      theta = fmin(theta, r);
+    for (int side = 0; side < 2; ++side) {
+      const int en = dg_cell_neighbour(e, ie, ne, periodic, d, side);
+      if (en < 0) continue;
+      const double wn = stats[(long long)en * 25 + v];
+      const double b = 0.5 * beta * (side ? wn - wb : wb - wn);
+      if (b * sg <= 0.0) zero = true;
+      m = fmin(m, fabs(b));
     }
+    const double r = zero ? 0.0 : (sg * m) / a;
+    theta = fmin(theta, r);
   }
-  return (theta >= 1.0 - 1e-12) ? 1.0 : theta;
+  return theta;
+}
+
+// theta of the Moe limiter (reading R18) from ONE variable v of cell e: bounds from the face neighbours'
+// extrema and the tolerance alpha, phi(y) = min(y/1.1, 1) on both sides.
+template <int ND>
+DG_INL double dg_moe_theta_var(const double* __restrict__ stats, int e, int v, const int ie[3], const int ne[3],
+                               const int periodic[3], double alpha) {
+  const double wb = stats[(long long)e * 15 + v], wM = stats[(long long)e * 15 + 5 + v], wm = stats[(long long)e * 15 + 10 + v];
+  double M = wb + alpha, m = wb - alpha;
+#pragma unroll
+  for (int d = 0; d < ND; ++d)
+#pragma unroll
+    for (int side = 0; side < 2; ++side) {
+      const int en = dg_cell_neighbour(e, ie, ne, periodic, d, side);
+      if (en < 0) continue;
+      M = fmax(M, stats[(long long)en * 15 + 5 + v]);
+      m = fmin(m, stats[(long long)en * 15 + 10 + v]);
+    }
+  const double tiny = 1e-12 * fmax(fabs(wM), fabs(wm));     // extremum = mean to rounding: no limit
+  const double tM = (wM - wb > tiny) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
+  const double tm = (wb - wm > tiny) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
+  return fmin(tM, tm);
 }
 
 struct MoePar {
@@ -377,34 +402,23 @@ dg_moe_apply_kernel(long long nelem, long long ndof, double* U, double* P, const
   const long long e = ((long long)blockIdx.x * 4 + wrp) * EPW + ew;
   const bool active = (ew < EPW) && (e < nelem);
   const long long g0 = (active ? e : 0) * NN + N * ln + h * SEG;
-  double theta = 1.0, mean[5] = {0, 0, 0, 0, 0};
-  if (active && LIMK == 1) theta = dg_mm_theta<ND>(stats, e, mp.ne, mp.periodic, mp.alpha, mean);
-  if (active && LIMK == 0) {
-    const long long ie[3] = {e % mp.ne[0], (e / mp.ne[0]) % mp.ne[1], e / (mp.ne[0] * mp.ne[1])};
-    const long long es[3] = {1, mp.ne[0], mp.ne[0] * mp.ne[1]};
+  // theta: lane v of the cell takes variable v (its own and its face neighbours' statistics), the cell's
+  // lanes then share the minimum.  (Every lane working through all five variables, with 64-bit index
+  // arithmetic, made this kernel cost as much as a stage: 6.7 ms at 128^3, p = 3.)
+  double th = 1.0;
+  if (active && lt < 5) {
+    const int ei = (int)e, ne[3] = {(int)mp.ne[0], (int)mp.ne[1], (int)mp.ne[2]};
+    const int ie[3] = {ei % ne[0], (ei / ne[0]) % ne[1], ei / (ne[0] * ne[1])};
+    for (int v = lt; v < 5; v += NL)
+      th = fmin(th, LIMK == 1 ? dg_mm_theta_var<ND>(stats, ei, v, ie, ne, mp.periodic, mp.alpha)
+                              : dg_moe_theta_var<ND>(stats, ei, v, ie, ne, mp.periodic, mp.alpha));
+  }
+  double theta = dg_cell_min<NL>(th, ew * NL);
+  if (LIMK == 1) theta = (theta >= 1.0 - 1e-12) ? 1.0 : theta;
+  double mean[5] = {0, 0, 0, 0, 0};
+  if (active && theta < 1.0) {
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-      const double wb = stats[e * 15 + v], wM = stats[e * 15 + 5 + v], wm = stats[e * 15 + 10 + v];
-      mean[v] = wb;
-      double M = wb + mp.alpha, m = wb - mp.alpha;
-#pragma unroll
-      for (int d = 0; d < ND; ++d)
-#pragma unroll
-        for (int side = 0; side < 2; ++side) {
-          long long jd = ie[d] + (side ? 1 : -1);
-          if (jd < 0 || jd >= mp.ne[d]) {
-            if (!mp.periodic[d]) continue;
-            jd = (jd + mp.ne[d]) % mp.ne[d];
-          }
-          const long long en = e + (jd - ie[d]) * es[d];
-          M = fmax(M, stats[en * 15 + 5 + v]);
-          m = fmin(m, stats[en * 15 + 10 + v]);
-        }
-      const double tiny = 1e-12 * fmax(fabs(wM), fabs(wm));     // extremum = mean to rounding: no limit
-      const double tM = (wM - wb > tiny) ? fmin((M - wb) / (wM - wb) / 1.1, 1.0) : 1.0;
-      const double tm = (wb - wm > tiny) ? fmin((wb - m) / (wb - wm) / 1.1, 1.0) : 1.0;
-      theta = fmin(theta, fmin(tM, tm));
-    }
+    for (int v = 0; v < 5; ++v) mean[v] = stats[e * (LIMK == 1 ? 25 : 15) + v];
   }
   if (theta_out && active && lt == 0) theta_out[e] = theta;
   const bool lim = active && (theta < 1.0);

@@ -2,9 +2,6 @@
 // and every order p = 0..4; compiled once per triple (-DDG_INST_ND=1|2|3 -DDG_INST_EOS=0|1
 // -DDG_INST_RS=0|1) so that the translation units build in parallel.  Exports a launcher and a per-device preparation call,
 // declared in dgrhd.cu.
-#include <cstdlib>
-#include <cstring>
-
 #include "stage_kernel.cuh"
 
 #ifndef DG_INST_ND
@@ -27,13 +24,11 @@ static cudaError_t prepare_n() {
   return cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 
-// log2 of the brick edge in tiles along axis d = 1 (y), 2 (z); EXPERIMENT knob DG_BRICK_LOG2="yz", default "33"
-static int dg_brick_target(int d) {
-  const char* e = getenv("DG_BRICK_LOG2");
-  if (!e || strlen(e) != 2) return 3;
-  const int v = e[d - 1] - '0';
-  return (v < 0 || v > 6) ? 3 : v;
-}
+// log2 of the brick edge in tiles along y and z.  Measured at 128^3, p = 3 (profiles/r3_brick_order.md): 4 x 4
+// tiles reads least from DRAM (plain order 108.6 / 148.9 / 148.7 B per DOF in the three stages, 4 x 4 bricks
+// 101.0 / 143.9 / 141.8, 8 x 8 and 16 x 16 in between); the launch time does not move (the kernel is bound by
+// instruction issue, not by DRAM).
+constexpr int DG_BRICK_LOG2 = 2;
 
 template <int N>
 static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
@@ -48,9 +43,8 @@ static cudaError_t launch_n(const StageArgs& a, cudaStream_t st) {
     // adds at most 1/8 to the tile count of that axis; the y extent of the grid holds BZ y-columns
     StageArgs b = a;
     int lby = 0, lbz = 0;
-    static const int target_y = dg_brick_target(1), target_z = dg_brick_target(2);
-    for (int l = target_y; l > 0 && !lby; --l) if (((nty + (1 << l) - 1) >> l << l) * 8 <= nty * 9) lby = l;
-    for (int l = target_z; l > 0 && !lbz; --l) if (((ntz + (1 << l) - 1) >> l << l) * 8 <= ntz * 9) lbz = l;
+    for (int l = DG_BRICK_LOG2; l > 0 && !lby; --l) if (((nty + (1 << l) - 1) >> l << l) * 8 <= nty * 9) lby = l;
+    for (int l = DG_BRICK_LOG2; l > 0 && !lbz; --l) if (((ntz + (1 << l) - 1) >> l << l) * 8 <= ntz * 9) lbz = l;
     const long long py = (nty + (1 << lby) - 1) >> lby << lby;
     if ((py << lbz) > 65535) lbz = 0;
     b.lby = lby;

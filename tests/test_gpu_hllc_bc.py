@@ -92,6 +92,22 @@ def test_bad_boundary_configurations_are_rejected():
     assert b.dgrhd_workspace_bytes(gcfg(d)) == 0
 
 
+def test_moe_limiter_hand_worked_cases_on_the_gpu():
+    """The CUDA path against tests/golden/moe_limiter_cases.txt directly: theta and the limited state worked by hand
+    from reading R18, not taken from the oracle."""
+    from _golden import moe_cases
+    for c in moe_cases():
+        ctx = B().Context(gcfg(c["cfg"]))
+        U = to_dev(c["state"])
+        theta = ctx.dgrhd_shock_limiter(U).cpu().numpy()
+        assert np.max(np.abs(theta - c["theta"])) <= 1e-14, (c["name"], theta, c["theta"])
+        Ul = U.cpu().numpy()
+        for v in range(5):
+            want = c["out"].get(v, c["state"][v])
+            assert np.max(np.abs(Ul[v] - want)) <= 1e-14 * max(1.0, np.max(np.abs(want))), (c["name"], v, Ul[v], want)
+        ctx.close()
+
+
 @pytest.mark.parametrize("k", [1, 2, 3, 4, 5])
 def test_paper_riemann_problems_forty_steps_match_oracle(k):
     """PAPER.md Eq. 85-89 with the paper's boundaries (Dirichlet; test 5: a wall at x = 1), HLLC, p = 2,

@@ -546,9 +546,30 @@ def test_paper_riemann_problems_stay_admissible_and_conserve_up_to_the_boundary_
 
 
 # ------------------------------------------------------------------------------------------------
-# Shock limiter of Moe et al. (PAPER.md:126, :551 ref [23]; reading R18).  The paper does not print it:
-# PARITY UNPINNED.  What can be pinned are the properties any such limiter must have.
+# Shock limiter of Moe et al. (PAPER.md:126, :551 ref [23]; reading R18).  The paper does not print it: PARITY
+# UNPINNED BY THE PAPER.  What is pinned: the reading itself, by hand-worked cases (tests/golden/moe_limiter_cases.txt),
+# and the properties any such limiter must have.
 # ------------------------------------------------------------------------------------------------
+def test_moe_limiter_reproduces_the_hand_worked_cases():
+    """tests/golden/moe_limiter_cases.txt: theta and the limited state of small 1D / 2D configurations worked by hand
+    from reading R18 (upper / lower bound from a neighbour, alpha in either bound, alpha alone, a non-periodic
+    boundary against its periodic twin, the weighted p = 2 average, face neighbours only, minimum over variables).
+    A wrong 1/1.1, a corner neighbour, a dropped alpha or an unweighted mean each fail a case."""
+    from _golden import moe_cases
+    cases = moe_cases()
+    assert len(cases) >= 8
+    for c in cases:
+        d = c["cfg"]
+        cfg = O.make_config(*[d[k] for k in ("ndim", "nelem", "xmin", "xmax", "bc", "order_p", "eos", "gamma_ad",
+                                              "rk_stages", "eps_q", "delta_s")], shock_limiter=1, moe_alpha=d["moe_alpha"])
+        Ul, theta, nlim = O.shock_limiter(cfg, c["state"])
+        assert np.max(np.abs(theta - c["theta"])) <= 1e-14, (c["name"], theta, c["theta"])
+        assert nlim == int(np.sum(c["theta"] < 1.0)), c["name"]
+        for v in range(5):
+            want = c["out"].get(v, c["state"][v])              # variables without an "out" line stay as they were
+            assert np.max(np.abs(Ul[v] - want)) <= 1e-14 * max(1.0, np.max(np.abs(want))), (c["name"], v, Ul[v], want)
+
+
 def test_moe_limiter_keeps_cell_means_leaves_resolved_data_alone_and_bounds_the_extrema():
     nd, nel, p = 2, [12, 9], 2
     N, nn = p + 1, 9

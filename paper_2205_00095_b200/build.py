@@ -95,6 +95,9 @@ def build(force: bool = False, verbose: bool = False, debug_asserts: bool = Fals
     nvcc = _nvcc()
     jobs = [([nvcc, *NVCC_FLAGS, f'-DDG_SRC_HASH="{src}"', "-c", os.path.join(CSRC, "dgrhd.cu"), "-o",
               os.path.join(obj_dir, "dgrhd.o")], os.path.join(obj_dir, "dgrhd.o"))]
+    # the con2prim comparison variants: no FMA contraction, so that Brent's path matches the oracle's (c2p_variant.cu)
+    jobs.append(([nvcc, *NVCC_FLAGS, "-fmad=false", "-c", os.path.join(CSRC, "c2p_variant.cu"), "-o",
+                  os.path.join(obj_dir, "c2p_variant.o")], os.path.join(obj_dir, "c2p_variant.o")))
     for nd in (3, 2, 1):                                     # the slowest translation units first
         for eos in (0, 1):
             for rs in (0, 1):                                    # HLL, HLLC

@@ -24,6 +24,10 @@ DG_DECL(1, 0, 0) DG_DECL(1, 1, 0) DG_DECL(2, 0, 0) DG_DECL(2, 1, 0) DG_DECL(3, 0
 DG_DECL(1, 0, 1) DG_DECL(1, 1, 1) DG_DECL(2, 0, 1) DG_DECL(2, 1, 1) DG_DECL(3, 0, 1) DG_DECL(3, 1, 1)
 #undef DG_DECL
 
+// launcher of the con2prim comparison variants: c2p_variant.cu (compiled with -fmad=false)
+cudaError_t dg_launch_c2p_variant(int eos, long long n, const double* U, double* W, int* status, EosPar e,
+                                  int max_iter, cudaStream_t st);
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -851,12 +855,8 @@ extern "C" int dgrhd_con2prim_batch_variant(int eos, int variant, double gamma_a
   int r = check_batch("dgrhd_con2prim_batch_variant", eos, gamma_ad, n, U_dev, W_dev);
   if (r != DGRHD_OK || n == 0) return r;
   if (max_iter < 1) return fail(nullptr, DGRHD_EINVAL, "dgrhd_con2prim_batch_variant: max_iter must be >= 1");
-  const EosPar e = make_eos(eos, gamma_ad);
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  const unsigned nb = (unsigned)((n + DG_FLAT_NT - 1) / DG_FLAT_NT);
-  if (eos == DGRHD_EOS_IDEAL) dg_c2p_variant_kernel<0><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e, max_iter);
-  else dg_c2p_variant_kernel<1><<<nb, DG_FLAT_NT, 0, st>>>((long long)n, U_dev, W_dev, status_dev, e, max_iter);
-  DG_CUDA(nullptr, cudaGetLastError());
+  DG_CUDA(nullptr, dg_launch_c2p_variant(eos, (long long)n, U_dev, W_dev, status_dev, make_eos(eos, gamma_ad), max_iter,
+                                         (cudaStream_t)cuda_stream));
   return DGRHD_OK;
 }
 

@@ -67,27 +67,7 @@ dg_c2p_batch_kernel(long long n, const double* __restrict__ U, double* __restric
   if (EOS == DG_EOS_TM && nfall) atomicAdd(&g_tm_fallbacks, (dg_ull)nfall);
 }
 
-// The comparison variants of con2prim (physics.cuh): one state per thread.
-template <int EOS>
-__global__ void __launch_bounds__(DG_FLAT_NT)
-dg_c2p_variant_kernel(long long n, const double* __restrict__ U, double* __restrict__ W,
-                      int* __restrict__ status, EosPar eos, int max_iter) {
-  const long long i = (long long)blockIdx.x * DG_FLAT_NT + threadIdx.x;
-  if (i >= n) return;
-  double u[5], w[5];
-#pragma unroll
-  for (int v = 0; v < 5; ++v) u[v] = __ldg(U + v * n + i);
-  int st = 1;
-  if (dg_admissible(u, 1.0)) {
-    st = (EOS == DG_EOS_IDEAL) ? dg_c2p_ideal_analytic(eos, u, w) : dg_c2p_tm_brent(u, w, max_iter);
-  } else {
-#pragma unroll
-    for (int v = 0; v < 5; ++v) w[v] = __longlong_as_double(0x7ff8000000000000LL);
-  }
-#pragma unroll
-  for (int v = 0; v < 5; ++v) W[v * n + i] = w[v];
-  if (status) status[i] = st;
-}
+// (the comparison variants of con2prim live in c2p_variant.cu, compiled without FMA contraction)
 
 template <int EOS>
 __global__ void __launch_bounds__(DG_FLAT_NT)

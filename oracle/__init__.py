@@ -245,3 +245,31 @@ def step(cfg, U, dt, nsteps, t=0.0):
     cnt = (C.c_int64 * 3)(0, 0, 0)
     lib().orc_step(C.byref(cfg), _p(U), dt, nsteps, C.cast(C.byref(tt), _dp), cnt)
     return U, tt.value, (cnt[0], cnt[1], cnt[2])
+
+
+# ---------------------------------------------------------------------------------------------
+# Norm used by the parity tests and by smoke() (no method arithmetic)
+# ---------------------------------------------------------------------------------------------
+def cell_local_ratio(a, b, nelem, nn):
+    """Cell-local error norm for multi-scale states: per variable and cell, max over the cell's nodes of |a - b|
+    divided by the max of |b| over the cell AND its face neighbours (no wrap: at a mesh face the neighbourhood is
+    just smaller, which only makes the norm stricter).  The three momentum rows share the scale |M| (a component
+    that vanishes locally has no scale of its own), floored at 1e-6 of the neighbourhood's energy density (same
+    units, c = 1) so that fluid at rest, whose momentum is rounding noise around zero, has a scale at all.  Unlike relmax, which divides by the GLOBAL maximum, this does
+    not let a near-vacuum cell hide a large relative error behind a dense cell elsewhere.  Returns [5, n_elem]."""
+    a, b = np.asarray(a), np.asarray(b)
+    nd = len(nelem)
+    ne = int(np.prod(nelem))
+    err = np.abs(a - b).reshape(5, ne, nn).max(2)
+    sc = np.abs(b).reshape(5, ne, nn).max(2)
+    sc[1:4] = np.maximum(np.sqrt((b[1:4] ** 2).sum(0)).reshape(ne, nn).max(1), 1e-6 * sc[4])[None, :]
+    grid = sc.reshape((5,) + tuple(reversed([int(n) for n in nelem])))          # [5, (nz,) (ny,) nx]
+    nb = grid.copy()
+    for ax in range(1, nd + 1):
+        pad = [(0, 0)] * (nd + 1)
+        pad[ax] = (1, 1)
+        g = np.pad(grid, pad, mode="edge")
+        lo = np.take(g, range(0, grid.shape[ax]), axis=ax)
+        hi = np.take(g, range(2, grid.shape[ax] + 2), axis=ax)
+        nb = np.maximum(nb, np.maximum(lo, hi))
+    return err / np.maximum(nb.reshape(5, ne), 1e-300)

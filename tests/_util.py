@@ -36,6 +36,14 @@ def relmax(a, b):
     return np.max(np.abs(a - b), axis=1) / np.maximum(np.max(np.abs(b), axis=1), 1e-300)
 
 
+cell_local_ratio = O.cell_local_ratio          # the cell-local error norm (oracle/__init__.py, test infrastructure)
+
+
+def cellmax(a, b, nelem, nn):
+    """max over cells of cell_local_ratio, per variable."""
+    return cell_local_ratio(a, b, nelem, nn).max(1)
+
+
 def smooth_prims(cfgd, seed, amp=0.3):
     """Smooth, bounded, seeded primitive field on the mesh of cfgd (pure input data)."""
     nd, N = cfgd["ndim"], cfgd["order_p"] + 1

@@ -17,9 +17,14 @@ import torch
 import oracle as O
 from paper_2205_00095_b200 import inputs as I
 
-from _util import B, DEV, gcfg, interior_mask, ocfg, relmax, sub_box, to_dev
+from _util import B, DEV, cell_local_ratio, cellmax, gcfg, interior_mask, ocfg, relmax, sub_box, to_dev
 
 pytestmark = pytest.mark.gpu
+
+# Tolerances within 100x of what the code achieves (printed by the tests; round 3 on a B200), in the global max norm
+# (relmax) and in the cell-local norm (cell_local_ratio), which a near-vacuum cell cannot hide behind a dense one.
+TOL_128_GLOBAL, TOL_128_LOCAL = 1e-10, 1e-10    # one step at 128^3: achieved 1.1e-12 / 1.3e-12
+TOL_64_GLOBAL, TOL_64_LOCAL = 1e-10, 2e-9       # 20 steps (60 limited stages) at 64^3: achieved 9.3e-13 / 2.0e-11
 
 
 def test_box3d_128_one_ssprk3_step_sampled_subboxes_match_oracle():
@@ -43,8 +48,9 @@ def test_box3d_128_one_ssprk3_step_sampled_subboxes_match_oracle():
     orgs = [(0, 0, 0), (122, 122, 122), (60, 122, 3)] + [tuple(rng.integers(0, 128, 3)) for _ in range(5)]
     sub = dict(d, nelem=[m] * 3, bc=[I.BC_OUTFLOW] * 3, xmin=[0.0] * 3, xmax=[m / 128.0] * 3)
     in1, in3 = interior_mask(m, 3, 1).repeat(nn), interior_mask(m, 3, 3).repeat(nn)
-    worst_r = worst_u = 0.0
+    worst_r = worst_u = worst_loc = 0.0
     nflag = 0
+    cells3 = interior_mask(m, 3, 3)
     for org in orgs:
         Us, e = sub_box(U_h, ne, nn, org, m)
         cols = (e[:, None] * nn + np.arange(nn)[None, :]).reshape(-1)
@@ -54,11 +60,12 @@ def test_box3d_128_one_ssprk3_step_sampled_subboxes_match_oracle():
         er = np.max(np.abs(Rg_h[:, cols][:, in1] - Ro[:, in1]), axis=1) / np.max(np.abs(Ro[:, in1]), axis=1)
         eu = relmax(Ug_h[:, cols][:, in3], Uo[:, in3])
         worst_r, worst_u = max(worst_r, er.max()), max(worst_u, eu.max())
+        worst_loc = max(worst_loc, cell_local_ratio(Ug_h[:, cols], Uo, [m] * 3, nn)[:, cells3].max())
     print(f"box3d 128^3: {len(orgs)} sub-boxes of {m}^3 elements, residual {worst_r:.2e}, state after one "
-          f"SSPRK3 step {worst_u:.2e} (max-norm, relative); oracle activations in the sub-boxes {nflag}; "
-          f"CUDA activations on the full mesh {c['n_flagged']}")
+          f"SSPRK3 step {worst_u:.2e} (max-norm, relative), {worst_loc:.2e} (cell-local norm); oracle activations in "
+          f"the sub-boxes {nflag}; CUDA activations on the full mesh {c['n_flagged']}")
     assert nflag > 0
-    assert worst_r <= 1e-11 and worst_u <= 1e-9
+    assert worst_r <= 1e-11 and worst_u <= TOL_128_GLOBAL and worst_loc <= TOL_128_LOCAL
 
 
 def test_box3d_64_twenty_steps_match_oracle():
@@ -72,15 +79,15 @@ def test_box3d_64_twenty_steps_match_oracle():
     c = ctx.dgrhd_get_counters()
     Uo, to, cnt_o = O.step(ocfg(d), U.cpu().numpy(), -0.3, 20)
     err = relmax(Ug, Uo)
+    loc = cellmax(Ug, Uo, d["nelem"], 64)
     dflag = c["n_flagged"] - cnt_o[0]
-    print(f"box3d 64^3, 20 SSPRK3 steps: max-norm rel. diff {err.max():.2e}, t {tg:.6e} vs {to:.6e}, "
+    print(f"box3d 64^3, 20 SSPRK3 steps: max-norm rel. diff {err.max():.2e}, cell-local {loc.max():.2e}, t {tg:.6e} vs {to:.6e}, "
           f"activations {cnt_o[0]} (oracle) {dflag:+d} (CUDA - oracle), bad means {cnt_o[1]}/{c['n_bad_mean']}")
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-9 * to
     assert c["n_bad_mean"] == cnt_o[1] and c["n_c2p_fail"] == cnt_o[2]
-    # 60 limited stages (limited nodes hug the admissibility boundary, reading R16): the bound is the
-    # 10-step smooth-problem tolerance; the achieved value is printed (round 2: 5e-13)
-    assert err.max() <= 1e-9
-    assert abs(dflag) <= max(10, cnt_o[0] // 1000)
+    # 60 limited stages (limited nodes hug the admissibility boundary, reading R16); the achieved values are printed
+    assert err.max() <= TOL_64_GLOBAL and loc.max() <= TOL_64_LOCAL
+    assert abs(dflag) <= 2                       # 2.5 million activations on each side: achieved +0
 
 
 @pytest.mark.parametrize("nx,steps", [(64, 10), (512, 10)])

@@ -15,9 +15,12 @@ import pytest
 import oracle as O
 from paper_2205_00095_b200 import inputs as I
 
-from _util import B, gcfg, ocfg, relmax, to_dev
+from _util import B, cellmax, gcfg, ocfg, relmax, to_dev
 
 pytestmark = pytest.mark.gpu
+
+# three limited SSPRK3 steps: global max norm / cell-local norm (tests/_util.py), within 100x of the achieved values
+TOL_GLOBAL, TOL_LOCAL = 2e-11, 1e-10     # achieved over the 11 instantiations: <= 2.1e-13 / <= 1.9e-12
 
 CASES = {
     "3d_p3_n8": lambda: I.box3d(0, n=8, p=3, kmax=1),
@@ -63,10 +66,12 @@ def test_three_ssprk3_steps_with_limited_cells_match_oracle(name):
     assert cnt_o[0] > 0 and cnt_o[1] == c["n_bad_mean"] == 0 and cnt_o[2] == c["n_c2p_fail"] == 0
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-11 * to
     err = relmax(Ug, Uo)
+    nn = (d["order_p"] + 1) ** d["ndim"]
+    loc = cellmax(Ug, Uo, d["nelem"][:d["ndim"]], nn)
     dflag = c["n_flagged"] - cnt_o[0]
-    print(f"{name}: max-norm rel. diff {err.max():.2e}, activations {cnt_o[0]} (oracle) {dflag:+d} (CUDA - oracle)")
-    assert err.max() <= 1e-9, err
-    assert abs(dflag) <= max(2, cnt_o[0] // 100)
+    print(f"{name}: max-norm rel. diff {err.max():.2e}, cell-local {loc.max():.2e}, activations {cnt_o[0]} (oracle) {dflag:+d} (CUDA - oracle)")
+    assert err.max() <= TOL_GLOBAL and loc.max() <= TOL_LOCAL, (err, loc)
+    assert abs(dflag) <= 2                       # achieved: +0 on every instantiation
 
 
 def test_conserved_integrals_of_a_periodic_box_drift_at_roundoff_only():

@@ -124,8 +124,8 @@ def test_paper_riemann_problems_forty_steps_match_oracle(k):
     print(f"paper Riemann problem {k}: max-norm rel. diff {err.max():.2e}, activations {cnt_o[0]} / {c['n_flagged']}")
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to
     assert c["n_bad_mean"] == cnt_o[1] == 0 and c["n_c2p_fail"] == cnt_o[2] == 0
-    assert err.max() <= 1e-8
-    assert abs(c["n_flagged"] - cnt_o[0]) <= max(2, cnt_o[0] // 50)
+    assert err.max() <= 1e-9                      # achieved over the five problems: <= 1.6e-10
+    assert abs(c["n_flagged"] - cnt_o[0]) <= 2    # achieved: identical counts on all five
 
 
 # ------------------------------------------------------------------------------------------------
@@ -271,7 +271,27 @@ def test_paper_riemann_problems_with_the_shock_limiter_match_oracle(k):
     print(f"paper Riemann problem {k} + Moe limiter: max-norm rel. diff {err.max():.2e}, physicality activations "
           f"{cnt_o[0]} / {c['n_flagged']}, cells rescaled by the shock limiter {c['n_shock_limited']}")
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to and c["n_shock_limited"] > 0
-    assert err.max() <= 1e-8
+    assert err.max() <= 2e-11                     # achieved: <= 2.1e-13
+
+
+def test_paper_2d_riemann_problem_1_with_a_wider_energy_margin_closes_the_conditioning_gap():
+    """SURVEY reading R16: limited nodes sit at P/E ~ 1e-9 with the default eps_q = 1e-12, where two correct fp64
+    codes differ by ~eps E/P per recovery (the previous test's bound; achieved 4e-5).  With eps_q = 1e-6 the
+    physicality operator keeps P/E >~ 7e-7 and the same 15 steps agree to 2.3e-9 (measured in round 3): the gap is
+    conditioning of the problem at the admissibility boundary, not a difference between the two codes."""
+    d, W, _ = I.paper_riemann2d(1, n=24, p=2)
+    d = dict(d, eps_q=1e-6)
+    U = O.prim2con_batch(d["eos"], d["gamma_ad"], W.numpy())
+    Uo, to, cnt_o = O.step(ocfg(d), U, -0.2, 15)
+    ctx = B().Context(gcfg(d))
+    ctx.dgrhd_set_state(to_dev(U))
+    tg = ctx.dgrhd_step(-0.2, 15, t=0.0)
+    Ug = ctx.dgrhd_get_state().cpu().numpy()
+    c = ctx.dgrhd_get_counters()
+    err = relmax(Ug, Uo)[[0, 1, 2, 4]]
+    print(f"paper 2D Riemann problem 1, p=2, eps_q=1e-6: max-norm rel. diff {err.max():.2e}, activations {cnt_o[0]} / {c['n_flagged']}")
+    assert cnt_o[0] > 100 and c["n_flagged"] == cnt_o[0] and abs(tg - to) <= 1e-12 * to
+    assert err.max() <= 2e-7                      # achieved 2.3e-9 (4e-5 at eps_q = 1e-12)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -313,4 +333,4 @@ def test_paper_riemann_problem_with_the_minmod_limiter_matches_oracle():
     err = relmax(Ug, Uo)[[0, 1, 4]]
     print(f"paper Riemann problem 4 + minmod limiter: max-norm rel. diff {err.max():.2e}, cells rescaled {c['n_shock_limited']}")
     assert np.isfinite(Ug).all() and abs(tg - to) <= 1e-10 * to and c["n_shock_limited"] > 0
-    assert err.max() <= 1e-8
+    assert err.max() <= 2e-11                     # achieved: <= 2.1e-13

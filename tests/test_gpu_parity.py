@@ -352,7 +352,8 @@ def test_fixed_dt_steps_and_split_calls_agree():
 def test_config1_riemann_50_steps_limiter_active():
     """Config 1 (BASELINE.json configs[0]): parity of a shocked, limited run.  Limited nodes hug the
     admissibility boundary where the residual is ill-conditioned (R16): the state is compared in the
-    max norm at 1e-7 and the activation counts may differ at marginal cells -- both are reported."""
+    max norm at 1e-12 (achieved over the three seeds: 1.2e-14) and the activation counts, which could differ
+    at marginal cells, are held to 2 cells in total (achieved: identical) -- both are reported."""
     worst, dflag = 0.0, 0
     for seed in range(3):
         d, W = I.riemann1d(seed)
@@ -368,7 +369,7 @@ def test_config1_riemann_50_steps_limiter_active():
         worst = max(worst, relmax(Ug, Uo)[[0, 1, 4]].max())
         dflag += abs(c["n_flagged"] - cnt_o[0])
     print(f"config1: worst max-norm rel. diff {worst:.3e}, activation-count diff {dflag}")
-    assert worst <= 1e-7
+    assert worst <= 1e-12 and dflag <= 2
 
 
 def test_entropy_wave_converges_at_order_p_plus_1_on_gpu():

@@ -346,17 +346,24 @@ def parity_leg(b, torch, cfgd, U):
     m = min(10, min(nelem))
     rng = np.random.default_rng(1)
     orgs = [tuple([0] * nd), tuple(n - m // 2 for n in nelem)] + [tuple(rng.integers(0, n) for n in nelem) for _ in range(4)]
+    # a sub-box may wrap around a periodic axis only: on any other axis it is pulled back inside the mesh (elements on
+    # either side of a real boundary are not neighbours)
+    orgs = [tuple(int(o) if (cfgd["bc"][k] & 255) == 0 else int(min(o, nelem[k] - m)) for k, o in enumerate(org)) for org in orgs]
     h = [(cfgd["xmax"][d] - cfgd["xmin"][d]) / nelem[d] for d in range(nd)]
     sub = dict(cfgd, nelem=[m] * nd, bc=[1] * nd, xmin=[0.0] * nd, xmax=[m * h[d] for d in range(nd)])
     worst = 0.0
+    boxes = []
     for org in orgs:
         cols, inner = sub_box_cols(nelem, nn, org, m)
         Ro, _ = O.rhs(O.make_config(*cfg_args(sub), **cfg_kw(sub)), np.ascontiguousarray(Uh[:, cols]))
-        scale = np.maximum(np.max(np.abs(Ro[:, inner]), axis=1), 1e-300)
-        err = np.max(np.abs(R[:, cols][:, inner] - Ro[:, inner]), axis=1) / scale
-        act = np.max(np.abs(Ro[:, inner]), axis=1) > 1e-9      # rows that are ~0 (unused axes, uniform flow): absolute
-        worst = max(worst, float(err[act].max(initial=0.0)),
-                    float(np.max(np.abs(R[:, cols][:, inner] - Ro[:, inner])[~act], initial=0.0)))
+        boxes.append((cols, inner, Ro))
+    # max norm per variable relative to the largest residual of that variable over ALL sampled sub-boxes (SURVEY 8(c):
+    # the residual is compared in the global max norm; a sub-box of nearly uniform flow has no scale of its own)
+    scale = np.max([np.max(np.abs(Ro[:, inner]), axis=1) for _, inner, Ro in boxes], axis=0)
+    act = scale > 1e-9                                           # rows that are ~0 everywhere (unused axes): absolute
+    for cols, inner, Ro in boxes:
+        diff = np.max(np.abs(R[:, cols][:, inner] - Ro[:, inner]), axis=1)
+        worst = max(worst, float((diff[act] / scale[act]).max(initial=0.0)), float(diff[~act].max(initial=0.0)))
     ctx.close()
     return {"what": f"dgrhd_rhs of the timed configuration vs the oracle on {len(orgs)} sub-boxes of {m}^{nd} elements (interior)",
             "residual_max_rel_err": worst, "tolerance": 1e-11, "ok": bool(worst <= 1e-11)}

@@ -43,9 +43,9 @@ DESIGN_BYTES_PER_DOF_STAGE = ALG_BYTES_PER_DOF_STAGE + 16.0
 # paper_2205_00095_b200.build.stage_kernel_hash()): when the sources have changed since, the line prints
 # traffic = null and no ALU fraction instead of stale numbers -- re-capture (profiles/r3_README.md).
 KERNEL_CONSTANTS = {
-    "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 128.9, "stage_src": "275a9f4536a591b4",
+    "box3d": {"flop_per_dof_stage": 487.5, "dram_bytes_per_dof_stage": 128.9, "stage_src": "b360551dad98732b",
               "source": "profiles/r3_ncu_stage_box3d_128.md (capture at 128^3, library src=e857100547a6b864; since then only the "
-                        "con2prim comparison variants moved out of physics.cuh: the stage kernel's SASS is byte-identical)"},
+                        "con2prim comparison variants moved out of physics.cuh and a debug-build-only #include was added: the stage kernel's SASS is byte-identical)"},
     "kh2d": {"flop_per_dof_stage": 449.7, "dram_bytes_per_dof_stage": 114.3, "stage_src": None,
              "source": "profiles/r2_ncu_stage_kh2d.md (round 2, 96 registers / 5 blocks per SM; not re-captured in round 3: the 2D kernel's "
                        "code path is unchanged but its sources are not byte-identical, so the line marks these as stale)"},

@@ -34,6 +34,9 @@
 // Algorithmic HBM traffic per node and stage: U_s 40 B + P_s 8 B in, U0 40 B in (a != 0), U_out 40 B +
 // P_out 8 B out = 96 / 136 B (mean over SSPRK3: 122.7 B); halo layers are L2 hits.
 #pragma once
+#ifdef DG_DEBUG_ASSERTS
+#include <cstdio>   // device printf of the bounds checks (debug build only)
+#endif
 #include "physics.cuh"
 
 #define DG_MODE_RHS 0
